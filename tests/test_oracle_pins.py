@@ -1,0 +1,289 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (CPU only).
+
+Every test names the passage it pins (PAPER.md:<line>); see tests/golden/paper_closed_forms.txt.
+None of these re-types the oracle's own formula: they use closed forms, an independent literal
+Python enumeration (tests/literal_enum.py), numpy.linalg.det, and exact symmetries.
+"""
+import itertools
+import json
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+from literal_enum import typed_connected_sum, uniform_connected_sum, _sign_by_inversions, _cycles
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+RTOL = 1e-11
+
+
+def close(a, b, scale=None, rtol=RTOL):
+    s = max(abs(a), abs(b), 1e-300) if scale is None else scale
+    return abs(a - b) <= rtol * s
+
+
+# ---------------------------------------------------------------- closed forms
+@pytest.mark.parametrize("nf", [2, 3, 4])
+def test_eq83_singleton_closed_form(nf):
+    """PAPER.md:821-826 Eq. 83."""
+    rng = np.random.default_rng(100 + nf)
+    for _ in range(5):
+        A = rng.standard_normal((nf, 1, 1))
+        s = rng.standard_normal(nf)
+        a = A[:, 0, 0]
+        exact = 2 * sum(a[i] * a[j] for i in range(nf) for j in range(i + 1, nf)) + 2 * float(np.dot(s, a))
+        assert close(oracle.o1_connected(A, nf, s, sb=True), exact)
+        assert close(oracle.o3_alg3(A, s), exact)
+        assert close(oracle.o2b_polynomial(A, s)[0], exact)
+
+
+def test_n1_uniform_closed_form():
+    """n = 1, uniform: identity (two loops) minus the swap (one loop): (N_f^2 - N_f) A^2;
+    with a true-diagonal shift sigma/N_f the two shift placements add 2 N_f sigma A."""
+    for nf in (2, 3, 5):
+        A = np.array([[[0.7]]])
+        assert close(oracle.o1_connected(A, nf, None, sb=False), (nf * nf - nf) * 0.49)
+        assert close(oracle.o3_uniform(A[0], nf)[0], (nf * nf - nf) * 0.49)
+        sg = -0.3
+        exact = (nf * nf - nf) * 0.49 + 2 * nf * sg * 0.7
+        assert close(oracle.o1_connected(A, nf, [sg], sb=False), exact)
+        assert close(oracle.o3_uniform(A[0], nf, sg)[0], exact)
+
+
+def test_n2_su2_closed_form():
+    """Two spins: full sum = 2^n det(A)^2; removing the disconnected product of the
+    two singletons (Eq. 53) leaves C_{12} = 4 [ det(A)^2 - A11^2 A22^2 ]."""
+    rng = np.random.default_rng(7)
+    for _ in range(5):
+        A = rng.standard_normal((2, 2))
+        exact = 4 * ((A[0, 0] * A[1, 1] - A[0, 1] * A[1, 0]) ** 2 - A[0, 0] ** 2 * A[1, 1] ** 2)
+        assert close(oracle.o1_connected(A[None], 2, None, sb=False), exact)
+        assert close(oracle.o3_uniform(A, 2)[0], exact)
+        assert close(oracle.o2a_twospin(A, A)[-1], exact)
+
+
+def test_sign_conventions():
+    """PAPER.md:51 ((1)(2)(3,4) has sign (-1)^(4-3)) and Eq. 78 (sgn = (-1)^(2n-k))."""
+    p = (0, 1, 3, 2)
+    assert _sign_by_inversions(p) == -1.0 and len(_cycles(p)) == 3
+    for p in itertools.permutations(range(6)):
+        assert _sign_by_inversions(p) == (-1.0) ** (6 - len(_cycles(p)))
+
+
+# ---------------------------------------------------------------- literal enumeration
+@pytest.mark.parametrize("n,nf", [(1, 2), (2, 2), (2, 3), (3, 2)])
+def test_o1_matches_literal_typed_enumeration(n, nf):
+    """Eq. 58-63 written out with explicit colourings (pure Python) == oracle O1 == Alg. 3."""
+    rng = np.random.default_rng(10 * n + nf)
+    A = rng.standard_normal((nf, n, n))
+    s = rng.standard_normal(nf)
+    lit = typed_connected_sum(A, s, nf)
+    assert close(oracle.o1_connected(A, nf, s, sb=True), lit)
+    assert close(oracle.o3_alg3(A, s), lit)
+    lit0 = typed_connected_sum(A, None, nf)
+    assert close(oracle.o1_connected(A, nf, None, sb=True), lit0)
+    assert close(oracle.o3_alg3(A, None), lit0)
+
+
+@pytest.mark.parametrize("n,nf", [(2, 2), (2, 3), (3, 2), (3, 3)])
+def test_uniform_matches_literal_enumeration(n, nf):
+    rng = np.random.default_rng(20 * n + nf)
+    A = rng.standard_normal((n, n))
+    lit = uniform_connected_sum(A, nf)
+    assert close(oracle.o1_connected(A[None], nf, None, sb=False), lit)
+    assert close(oracle.o3_uniform(A, nf)[0], lit)
+
+
+# ---------------------------------------------------------------- determinant identities via numpy
+def _moment(Au, Ad, su, sd, T):
+    idx = [i for i in range(Au.shape[0]) if T >> i & 1]
+    if not idx:
+        return 1.0
+    k = len(idx)
+    return (2.0 ** k) * np.linalg.det(Au[np.ix_(idx, idx)] + sd * np.eye(k)) * \
+        np.linalg.det(Ad[np.ix_(idx, idx)] + su * np.eye(k))
+
+
+@pytest.mark.parametrize("shift", [False, True])
+def test_two_determinant_moment_cumulant(shift):
+    """PAPER.md:45/401 (product of two determinants), Eq. 49 (opposite-spin counterterm on the true
+    diagonal), Eq. 50 (scalar term, singletons only), Eq. 53 rearranged:
+        a(V) = sum_{S containing min V} c(S) a(V \\ S)
+    with a from numpy.linalg.det and c from the brute-force definition."""
+    rng = np.random.default_rng(31)
+    n = 3
+    A = rng.standard_normal((2, n, n))
+    su, sd = (0.4, -0.7) if shift else (0.0, 0.0)
+    sig = [su, sd] if shift else None
+    c = oracle.o1_all_subsets(A, 2, sig, sb=True)
+    cfull = {T: c[T - 1] + (2 * su * sd if bin(T).count("1") == 1 else 0.0) for T in range(1, 1 << n)}
+    for V in range(1, 1 << n):
+        anchor = V & -V
+        rest = V ^ anchor
+        total, sub = 0.0, rest
+        while True:
+            S = anchor | sub
+            total += cfull[S] * _moment(A[0], A[1], su, sd, V ^ S)
+            if sub == 0:
+                break
+            sub = (sub - 1) & rest
+        assert close(total, _moment(A[0], A[1], su, sd, V), rtol=1e-10)
+    assert np.allclose(oracle.o2a_twospin(A[0], A[1], su, sd), c, rtol=1e-10, atol=1e-12)
+
+
+# ---------------------------------------------------------------- tiers agree
+@pytest.mark.parametrize("n,nf", [(2, 2), (3, 3), (4, 2), (4, 3)])
+def test_all_tiers_agree_sb(n, nf):
+    """Theorem 1: Alg. 3 == S_n; polynomial route == SB-CoS."""
+    rng = np.random.default_rng(40 + 7 * n + nf)
+    A = rng.standard_normal((nf, n, n))
+    s = rng.standard_normal(nf) * 0.5
+    ref = oracle.o1_all_subsets(A, nf, s, sb=True)
+    poly = oracle.o2b_polynomial(A, s)
+    assert np.allclose(poly, ref, rtol=1e-10, atol=1e-11)
+    assert close(oracle.o3_alg3(A, s), ref[-1], rtol=1e-10)
+    if nf == 2:
+        assert np.allclose(oracle.o2a_twospin(A[0], A[1], s[0], s[1]), ref, rtol=1e-10, atol=1e-11)
+
+
+def test_tiers_agree_n5_bruteforce():
+    """north_star: oracle checked on n <= 5 (10! permutations)."""
+    rng = np.random.default_rng(55)
+    A = rng.standard_normal((2, 5, 5)) * 0.6
+    s = [0.3, -0.2]
+    ref = oracle.o1_connected(A, 2, s, sb=True)
+    assert close(oracle.o3_alg3(A, s), ref, rtol=1e-9)
+    assert close(oracle.o2a_twospin(A[0], A[1], s[0], s[1])[-1], ref, rtol=1e-9)
+    assert close(oracle.o2b_polynomial(A, s)[-1], ref, rtol=1e-9)
+    Au = A[:1]
+    refu = oracle.o1_connected(Au, 3, None, sb=False)
+    assert close(oracle.o3_uniform(Au[0], 3)[0], refu, rtol=1e-9)
+
+
+@pytest.mark.parametrize("n", [6, 8])
+def test_uniform_recurrence_vs_determinants_all_subsets(n):
+    """Eq. 8-15 all-subset readouts vs two-spin determinants + CDet on every subset (n beyond brute force)."""
+    rng = np.random.default_rng(60 + n)
+    A = rng.standard_normal((n, n)) * 0.5
+    rec = oracle.o3_uniform(A, 2, 0.0, all_subsets=True)
+    det = oracle.o2a_twospin(A, A)
+    M = oracle.o3_uniform(A, 2, 0.0, all_subsets=True, absolute=True)
+    assert np.all(np.abs(rec - det) <= 1e-10 * M)
+    single = oracle.o3_uniform(A, 2, 0.0, all_subsets=False)
+    assert abs(single[0] - det[-1]) <= 1e-10 * M[-1]
+
+
+def test_alg3_vs_polynomial_three_flavours_n6():
+    """BASELINE config 4's cross-check (n <= 6, determinant-polynomial + subset recursion)."""
+    rng = np.random.default_rng(66)
+    A = rng.standard_normal((3, 6, 6)) * 0.5
+    s = [0.2, 0.0, -0.2]
+    M = oracle.o3_alg3(A, s, absolute=True)
+    assert abs(oracle.o3_alg3(A, s) - oracle.o2b_polynomial(A, s)[-1]) <= 1e-10 * M
+
+
+# ---------------------------------------------------------------- reductions and symmetries
+@pytest.mark.parametrize("nf", [2, 3])
+def test_sb_reduces_to_uniform(nf):
+    """Eq. 33: equal blocks and equal sigma."""
+    rng = np.random.default_rng(70 + nf)
+    n = 3
+    A = rng.standard_normal((n, n))
+    Ab = np.repeat(A[None], nf, axis=0)
+    for sg in (0.0, 0.37):
+        sb = oracle.o1_connected(Ab, nf, [sg] * nf, sb=True)
+        un = oracle.o1_connected(A[None], nf, [sg] if sg else None, sb=False)
+        assert close(sb, un, rtol=1e-10)
+        assert close(oracle.o3_alg3(Ab, [sg] * nf), oracle.o3_uniform(A, nf, sg)[0], rtol=1e-10)
+
+
+def test_uniform_shift_is_true_diagonal_shift():
+    """only the TRUE one-cycle v -> v gets sigma/N_f; A[v, P(v)] keeps its value.  With two
+    spins this is Eq. 49: det(A + sigma 1)^2 on every subset, minus the scalar sigma^2 ... of Eq. 50."""
+    rng = np.random.default_rng(81)
+    n = 4
+    A = rng.standard_normal((n, n)) * 0.7
+    sg = 0.45
+    rec = oracle.o3_uniform(A, 2, sg, all_subsets=True)
+    # uniform N_f = 2 with closing weight sigma == SB with sigma_up = sigma_dn = sigma/... : Eq. 33 with N_f = 2
+    det = oracle.o2a_twospin(A, A, sg, sg)
+    assert np.allclose(rec, det, rtol=1e-10, atol=1e-11)
+
+
+def test_vertex_relabelling_and_scaling():
+    """S_n is a function of the unordered vertex set (relabel vertices) and homogeneous of degree 2n
+    under A -> cA, sigma -> c sigma (each of the 2n endpoints carries one factor)."""
+    rng = np.random.default_rng(90)
+    n, nf = 4, 3
+    A = rng.standard_normal((nf, n, n))
+    s = rng.standard_normal(nf)
+    ref = oracle.o3_alg3(A, s)
+    perm = [2, 0, 3, 1]
+    Ap = A[:, perm][:, :, perm]
+    assert close(oracle.o3_alg3(Ap, s), ref, rtol=1e-10)
+    assert close(oracle.o3_alg3(1.5 * A, 1.5 * s), ref * 1.5 ** (2 * n), rtol=1e-10)
+    cperm = [1, 2, 0]                                 # colours are summed: relabelling them is a symmetry
+    assert close(oracle.o3_alg3(A[cperm], s[cperm]), ref, rtol=1e-10)
+
+
+def test_principal_submatrix_property():
+    """each readout uses the principal submatrix of the envelope matrix."""
+    rng = np.random.default_rng(95)
+    n = 5
+    A = rng.standard_normal((n, n))
+    full = oracle.o3_uniform(A, 2, 0.0, all_subsets=True)
+    B = A.copy()
+    B[4, :] = rng.standard_normal(n)
+    B[:, 4] = rng.standard_normal(n)
+    other = oracle.o3_uniform(B, 2, 0.0, all_subsets=True)
+    for S in range(1, 1 << n):
+        if not S >> 4 & 1:
+            assert full[S - 1] == other[S - 1]
+        sub = [i for i in range(n) if S >> i & 1]
+        assert close(full[S - 1], oracle.o3_uniform(A[np.ix_(sub, sub)], 2)[0], rtol=1e-10)
+
+
+def test_sublattice_sum_tiers():
+    """Eq. 54-55: sum over sublattice assignments; two-spin honeycomb via SB N_f = 2 (reading G5)."""
+    rng = np.random.default_rng(97)
+    n, ns = 3, 2
+    G = rng.standard_normal((2, n * ns, n * ns)) * 0.6
+    s = (0.3, -0.3)
+    a = oracle.connected_reference(G, n, ns, 2, s, uniform=False, all_subsets=True, tier="o1")
+    b = oracle.connected_reference(G, n, ns, 2, s, uniform=False, all_subsets=True, tier="o3")
+    c = oracle.connected_reference(G, n, ns, 2, s, uniform=False, all_subsets=True, tier="o2a")
+    assert np.allclose(a, b, rtol=1e-10, atol=1e-12) and np.allclose(a, c, rtol=1e-10, atol=1e-12)
+
+
+def test_absolute_bound_dominates():
+    rng = np.random.default_rng(99)
+    A = rng.standard_normal((3, 4, 4))
+    s = rng.standard_normal(3)
+    M1 = oracle.o1_connected(A, 3, s, sb=True, absolute=True)
+    M3 = oracle.o3_alg3(A, s, absolute=True)
+    assert close(M1, M3, rtol=1e-10) and M1 >= abs(oracle.o3_alg3(A, s))
+
+
+# ---------------------------------------------------------------- structural counts of the printed recurrences
+def test_readout_layers_and_counts():
+    """2^n - 1 outputs, every one nonzero for a generic matrix."""
+    rng = np.random.default_rng(3)
+    n = 6
+    A = rng.standard_normal((n, n))
+    out = oracle.o3_uniform(A, 2, 0.0, all_subsets=True)
+    assert out.shape == ((1 << n) - 1,) and np.all(out != 0.0)
+
+
+# ---------------------------------------------------------------- stored regression anchors
+def test_golden_small_values():
+    with open(os.path.join(HERE, "golden", "oracle_small.json")) as f:
+        gold = json.load(f)
+    for case in gold["cases"]:
+        A = np.array(case["A"])
+        vals = np.array(case["values_by_bitmask"])
+        if case["mode"] == "uniform":
+            got = oracle.o3_uniform(A[0], case["n_flavors"], 0.0, all_subsets=True)
+        else:
+            got = oracle.o2b_polynomial(A, case["sigma"])
+        assert np.allclose(got, vals, rtol=1e-12, atol=1e-12), case["name"]
