@@ -1,0 +1,131 @@
+/*
+ * cos.h -- C-ABI of the B200-native CoS / SB-CoS DAG evaluator (arxiv 2507.12349, "CoS++").
+ *
+ * The library evaluates, for many Monte-Carlo configurations at once and in fp64, the connected
+ * Hubbard Feynman-diagram sum S_n of PAPER.md Eq. 63 (SB-CoS, Algorithm 3) or
+ * its flavour-uniform specialisation (Eq. 8-12), optionally for all 2^n-1
+ * vertex subsets (terminal readouts, Eq. 13-15), by walking a compiled layered DAG
+ * (Eq. 16).
+ *
+ * Conventions
+ *   n        perturbative order = interaction vertices (1..COS_MAX_N); endpoints 2n (Eq. 58).
+ *   N_f      number of flavours.
+ *   n_sub    sublattices per vertex: 1 (square) or 2 (honeycomb, sublattice-SUMMED, Eq. 4, 55).
+ *   d        n * n_sub; endpoint index a = i*n_sub + s for vertex i (0-based) on sublattice s.
+ *   block    one d x d propagator matrix; uniform mode has ONE block, SB mode N_f blocks.
+ *   "host"/"device" below says where a pointer must live.  All device pointers must belong to
+ *   the CUDA device that was current when cos_build / cos_tab_build was called.
+ *
+ * Errors: every function returns a status (COS_OK = 0); nothing throws or aborts across the ABI.
+ * cos_last_error() returns a thread-local human-readable message for the last failure.
+ * There is NO CPU fallback: without a CUDA device cos_build succeeds only in host-only mode
+ * (COS_BUILD_HOST_ONLY, used to inspect the compiled DAG) and cos_eval fails with COS_ECUDA.
+ */
+#ifndef COS_B200_H
+#define COS_B200_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define COS_MAX_N 12
+#define COS_MAX_COLOURS 4          /* SB mode: N_f <= 4 (colour carried in the state) */
+
+typedef struct cos_handle_s* cos_handle;     /* opaque: host DAG + device program + device workspace */
+typedef struct cos_tab_s*    cos_tab;        /* opaque: device propagator lookup table */
+typedef void*                cos_stream;     /* a cudaStream_t (0 / NULL = legacy default stream) */
+
+enum { COS_OK = 0, COS_EINVAL = 1, COS_ENOMEM = 2, COS_ECUDA = 3, COS_EUNSUPPORTED = 4 };
+enum { COS_LATTICE_SQUARE = 0, COS_LATTICE_HONEYCOMB = 1 };
+
+/* flags for cos_build_ex */
+enum { COS_BUILD_HOST_ONLY = 1 };            /* compile the DAG, do not touch CUDA (cos_eval then fails) */
+
+/* ---- (1) DAG compiler: PAPER.md:160-265 (canonical keys Eq. 17, 79-80; pruning Eq. 19-24) ----------
+ * Enumerates the reachable states (occupancy mask m_i in {0,(1,s),2}, head, endpoint, colour), prunes
+ * them against the requested readouts, layers them by total occupancy and uploads the per-layer
+ * program.
+ *   n, n_flavors    as above.
+ *   lattice         COS_LATTICE_SQUARE (n_sub=1) or COS_LATTICE_HONEYCOMB (n_sub=2).
+ *   shifts          host, may be NULL.
+ *                   NULL      -> uniform CoS: one propagator block, factor N_f per closed loop
+ *                                (Eq. 12, 15), no counterterm.
+ *                   non-NULL  -> SB-CoS: n_flavors blocks, shifts[lam] = sigma_lam = alpha_lam/U
+ *                                (shift-close weight), n_flavors values; colour sums
+ *                                replace N_f.  n_flavors <= COS_MAX_COLOURS.
+ *   readout_envelope 0 -> one output per configuration, the full-order value C_{[n]};
+ *                   n -> all 2^n-1 subset values (Eq. 5 with N = n); anything else: COS_EINVAL.
+ *   out             receives the handle; the caller releases it with cos_free.
+ * The values returned by cos_eval follow the physical convention of Eq. 83 (no shift-shift term).  */
+int cos_build(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope, cos_handle* out);
+int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope,
+                 int flags, cos_handle* out);
+
+/* ---- (3)+(4) layer propagation and terminal readouts: Eq. 16, Eq. 11-15 ----------------------------
+ *   G_dev    device, fp64, read-only: G_dev[((blk*d + a)*d + b) * batch + c] = propagator of block blk
+ *            from endpoint a to endpoint b (A[vbar, pi(v)bar] of Eq. 59) of configuration c;
+ *            the configuration index is the contiguous one.  blk < 1 (uniform) or N_f (SB).
+ *   batch    number of configurations (>= 0; 0 is a no-op).
+ *   out_dev  device, fp64, written: out_dev[k*batch + c]; k = 0 for readout_envelope = 0, otherwise
+ *            k = bitmask(S)-1 with bit i <-> vertex i (2^n-1 rows).
+ *   stream   CUDA stream the kernels are enqueued on.  The call is asynchronous: it returns after
+ *            enqueueing (launch errors only).  The handle owns a workspace that is grown lazily (a
+ *            synchronising cudaMalloc on first use / growth); one cos_eval in flight per handle.
+ * Large batches are processed in chunks that fit the workspace budget (cos_set_workspace_limit). */
+int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev, cos_stream stream);
+
+/* Releases host and device memory of the handle.  cos_free(NULL) is a no-op. */
+void cos_free(cos_handle h);
+
+/* Upper bound (bytes) for the layer-slab workspace of a handle; default 64 GiB. */
+int cos_set_workspace_limit(cos_handle h, long long bytes);
+
+/* ---- introspection (SURVEY.md section 5 "metrics") ------------------------------------------------- */
+enum {
+    COS_INFO_N_LAYERS = 0,        /* 2n */
+    COS_INFO_N_STATES = 1,        /* DAG states over all layers (Eq. 79 keys in the reduced form of DESIGN.md) */
+    COS_INFO_N_EDGES = 2,         /* DAG edges E1..E4, uncoalesced, colour fan-out included (Eq. 16) */
+    COS_INFO_N_READOUT_EDGES = 3, /* sum_S q_S, Eq. 15 / PAPER.md:156 */
+    COS_INFO_N_OUT = 4,           /* 1 or 2^n-1 */
+    COS_INFO_MAX_LAYER_STATES = 5,
+    COS_INFO_N_MASKS = 6,         /* occupancy masks (block count) */
+    COS_INFO_N_ROWS = 7,          /* (mask, head, colour) rows */
+    COS_INFO_N_FMA = 8,           /* fp64 FMAs the kernels execute per configuration */
+    COS_INFO_PROGRAM_BYTES = 9,   /* device bytes of the compiled program */
+    COS_INFO_D = 10,              /* d = n * n_sub */
+    COS_INFO_N_BLOCKS = 11,       /* propagator blocks expected in G_dev */
+    COS_INFO_N_STATES_UNPRUNED = 12,
+    COS_INFO_WORKSPACE_BYTES = 13,
+    COS_INFO_LAYER_STATES = 100,  /* + layer index */
+    COS_INFO_LAYER_EDGES = 200,   /* + layer index: edges leaving that layer (readout edges included) */
+    COS_INFO_LAYER_MASKS = 300    /* + layer index */
+};
+int cos_info(cos_handle h, int what, long long* value);
+
+const char* cos_last_error(void);
+
+/* ---- (2) propagator tabulation: PAPER.md:271-275 (Eq. 32), 415; readings G17-G18 of DESIGN.md --------
+ * cos_tab_build copies a host lookup table to the device.
+ *   table_host  host fp64, layout [n_blocks][n_sub*n_sub][L*L][n_tau]: value of g_blk^{s s'}(r, tau_k),
+ *               r = (dx, dy) = displacement FROM-endpoint minus TO-endpoint modulo L, index dx*L+dy,
+ *               tau_k = k*beta/(n_tau-1), k = 0..n_tau-1 (both ends).
+ * cos_tabulate fills G_dev (layout of cos_eval) for `batch` configurations:
+ *   A[(i,s),(j,s')] = sign * ((1-w) T[k] + w T[k+1]),  dtau = tau_i - tau_j; dtau <= 0 -> dtau += beta,
+ *   sign = -1 (anti-periodicity; equal times and i = j use 0^-);  u = dtau/(beta/(n_tau-1)),
+ *   k = min(floor(u), n_tau-2), w = u-k.
+ *   sites_dev   device int32 [n][2][batch]   lattice (square) or unit-cell (honeycomb) coordinates in [0,L)
+ *   tau_dev     device fp64  [n][batch]      imaginary times in [0, beta)
+ * Asynchronous on `stream`. */
+int cos_tab_build(int lattice, int L, int n_blocks, double beta, int n_tau, const double* table_host, cos_tab* out);
+int cos_tabulate(cos_tab tab, int n, const int* sites_dev, const double* tau_dev, long long batch,
+                 double* G_dev, cos_stream stream);
+void cos_tab_free(cos_tab tab);
+
+/* ---- measurement helper: fp64 FMA peak of the device (independent FMA chains, no memory traffic).
+ * Returns achieved FMA/s in *fma_per_s (synchronous; used by bench.py for the fp64 roofline leg). */
+int cos_measure_fp64_fma_peak(double* fma_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* COS_B200_H */

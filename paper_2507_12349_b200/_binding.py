@@ -1,0 +1,178 @@
+"""ctypes marshalling for include/cos.h.  Same function names as the C-ABI.
+
+Device arrays are torch CUDA tensors (PyTorch is used for device memory and streams only); the
+binding passes their data pointers and the current CUDA stream.  A missing shared library raises
+ImportError-like CosError loudly: there is no Python / CPU implementation behind these calls.
+"""
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libcos_b200.so")
+_lib = None
+
+COS_OK, COS_EINVAL, COS_ENOMEM, COS_ECUDA, COS_EUNSUPPORTED = 0, 1, 2, 3, 4
+COS_LATTICE_SQUARE, COS_LATTICE_HONEYCOMB = 0, 1
+COS_BUILD_HOST_ONLY = 1
+
+INFO = {
+    "n_layers": 0, "n_states": 1, "n_edges": 2, "n_readout_edges": 3, "n_out": 4, "max_layer_states": 5,
+    "n_masks": 6, "n_rows": 7, "n_fma": 8, "program_bytes": 9, "d": 10, "n_blocks": 11,
+    "n_states_unpruned": 12, "workspace_bytes": 13,
+    "layer_states": 100, "layer_edges": 200, "layer_masks": 300,
+}
+
+EXPORTS = [
+    "cos_build", "cos_build_ex", "cos_eval", "cos_free", "cos_set_workspace_limit", "cos_info",
+    "cos_last_error", "cos_tab_build", "cos_tabulate", "cos_tab_free", "cos_measure_fp64_fma_peak",
+]
+
+
+class CosError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("cos error %d: %s" % (code, msg))
+        self.code = code
+
+
+def lib_path():
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen libcos_b200.so (built by `python -m paper_2507_12349_b200.build` / __graft_entry__.build())."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise CosError(COS_ECUDA, "libcos_b200.so is missing at %s: build it with "
+                       "`python -m paper_2507_12349_b200.build` (there is no fallback implementation)" % _LIB_PATH)
+    lib = ctypes.CDLL(_LIB_PATH)
+    vp, ip, dp, llp = ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_longlong)
+    lib.cos_build.restype = ctypes.c_int
+    lib.cos_build.argtypes = [ip, ip, ip, dp, ip, ctypes.POINTER(vp)]
+    lib.cos_build_ex.restype = ctypes.c_int
+    lib.cos_build_ex.argtypes = [ip, ip, ip, dp, ip, ip, ctypes.POINTER(vp)]
+    lib.cos_eval.restype = ctypes.c_int
+    lib.cos_eval.argtypes = [vp, vp, ctypes.c_longlong, vp, vp]
+    lib.cos_free.restype = None
+    lib.cos_free.argtypes = [vp]
+    lib.cos_set_workspace_limit.restype = ctypes.c_int
+    lib.cos_set_workspace_limit.argtypes = [vp, ctypes.c_longlong]
+    lib.cos_info.restype = ctypes.c_int
+    lib.cos_info.argtypes = [vp, ip, llp]
+    lib.cos_last_error.restype = ctypes.c_char_p
+    lib.cos_last_error.argtypes = []
+    lib.cos_tab_build.restype = ctypes.c_int
+    lib.cos_tab_build.argtypes = [ip, ip, ip, ctypes.c_double, ip, vp, ctypes.POINTER(vp)]
+    lib.cos_tabulate.restype = ctypes.c_int
+    lib.cos_tabulate.argtypes = [vp, ip, vp, vp, ctypes.c_longlong, vp, vp]
+    lib.cos_tab_free.restype = None
+    lib.cos_tab_free.argtypes = [vp]
+    lib.cos_measure_fp64_fma_peak.restype = ctypes.c_int
+    lib.cos_measure_fp64_fma_peak.argtypes = [dp]
+    _lib = lib
+    return lib
+
+
+def cos_last_error():
+    return load_library().cos_last_error().decode("utf-8", "replace")
+
+
+def _check(rc):
+    if rc != COS_OK:
+        raise CosError(rc, cos_last_error())
+
+
+def _shifts_arg(shifts):
+    if shifts is None:
+        return None, None
+    arr = (ctypes.c_double * len(shifts))(*[float(s) for s in shifts])
+    return arr, ctypes.cast(arr, ctypes.POINTER(ctypes.c_double))
+
+
+def cos_build_ex(n, n_flavors, lattice, shifts, readout_envelope, flags=0):
+    """-> opaque handle (int).  shifts: None (uniform CoS) or a sequence of n_flavors sigma values (SB-CoS)."""
+    lib = load_library()
+    keep, p = _shifts_arg(shifts)
+    h = ctypes.c_void_p()
+    _check(lib.cos_build_ex(int(n), int(n_flavors), int(lattice), p, int(readout_envelope), int(flags), ctypes.byref(h)))
+    return h.value
+
+
+def cos_build(n, n_flavors, lattice, shifts, readout_envelope):
+    return cos_build_ex(n, n_flavors, lattice, shifts, readout_envelope, 0)
+
+
+def _stream_ptr(stream):
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return getattr(stream, "cuda_stream", stream)
+
+
+def _dev_ptr(t, dtype_name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and str(t.dtype) == dtype_name):
+        raise CosError(COS_EINVAL, "expected a contiguous CUDA tensor of dtype %s" % dtype_name)
+    return t.data_ptr()
+
+
+def cos_eval(handle, G_dev, batch, out_dev, stream=None):
+    """G_dev: torch.float64 CUDA tensor [n_blocks*d*d, batch] (batch contiguous); out_dev: [n_out, batch]."""
+    lib = load_library()
+    _check(lib.cos_eval(handle, _dev_ptr(G_dev, "torch.float64"), int(batch), _dev_ptr(out_dev, "torch.float64"),
+                        _stream_ptr(stream)))
+
+
+def cos_free(handle):
+    load_library().cos_free(handle)
+
+
+def cos_set_workspace_limit(handle, nbytes):
+    _check(load_library().cos_set_workspace_limit(handle, int(nbytes)))
+
+
+def cos_info(handle, what, layer=0):
+    code = INFO[what] if isinstance(what, str) else int(what)
+    if code >= 100:
+        code += int(layer)
+    v = ctypes.c_longlong(0)
+    _check(load_library().cos_info(handle, code, ctypes.byref(v)))
+    return v.value
+
+
+def cos_tab_build(lattice, L, n_blocks, beta, n_tau, table_host):
+    """table_host: C-contiguous numpy float64 [n_blocks][n_sub^2][L*L][n_tau]."""
+    import numpy as np
+    t = np.ascontiguousarray(table_host, dtype=np.float64)
+    tab = ctypes.c_void_p()
+    _check(load_library().cos_tab_build(int(lattice), int(L), int(n_blocks), float(beta), int(n_tau),
+                                        t.ctypes.data, ctypes.byref(tab)))
+    return tab.value
+
+
+def cos_tabulate(tab, n, sites_dev, tau_dev, batch, G_dev, stream=None):
+    _check(load_library().cos_tabulate(tab, int(n), _dev_ptr(sites_dev, "torch.int32"), _dev_ptr(tau_dev, "torch.float64"),
+                                       int(batch), _dev_ptr(G_dev, "torch.float64"), _stream_ptr(stream)))
+
+
+def cos_tab_free(tab):
+    load_library().cos_tab_free(tab)
+
+
+def cos_measure_fp64_fma_peak():
+    v = ctypes.c_double(0.0)
+    _check(load_library().cos_measure_fp64_fma_peak(ctypes.byref(v)))
+    return v.value
+
+
+def dag_summary(handle):
+    """Convenience: the cos_info counters as a dict (host data only)."""
+    keys = ["n_layers", "n_states", "n_edges", "n_readout_edges", "n_out", "max_layer_states", "n_masks",
+            "n_rows", "n_fma", "program_bytes", "d", "n_blocks", "n_states_unpruned"]
+    out = {k: cos_info(handle, k) for k in keys}
+    nl = out["n_layers"]
+    out["layer_states"] = [cos_info(handle, "layer_states", l) for l in range(nl)]
+    out["layer_edges"] = [cos_info(handle, "layer_edges", l) for l in range(nl)]
+    out["layer_masks"] = [cos_info(handle, "layer_masks", l) for l in range(nl)]
+    return out

@@ -1,0 +1,277 @@
+// cos_capi.cu -- the extern "C" boundary declared in include/cos.h.
+#include "../../include/cos.h"
+#include "cos_compile.h"
+#include "cos_kernels.cuh"
+
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+using namespace cosb;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string& msg) { g_err = msg; return code; }
+int cuda_fail(cudaError_t e, const char* what)
+{
+    g_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return e == cudaErrorMemoryAllocation ? COS_ENOMEM : COS_ECUDA;
+}
+
+struct DeviceLayer { uint32_t* words = nullptr; uint32_t* mask_off = nullptr; };
+
+int env_int(const char* name, int dflt)
+{
+    const char* s = getenv(name);
+    if (!s || !*s) return dflt;
+    return atoi(s);
+}
+
+}  // namespace
+
+struct cos_handle_s {
+    CompiledDag dag;
+    bool on_device = false;
+    int device = -1;
+    std::vector<DeviceLayer> dl;
+    size_t program_bytes = 0;
+    double* ws = nullptr;                 // two ping-pong layer slabs
+    size_t ws_bytes = 0;
+    long long ws_limit = 64ll << 30;
+    int masks_per_cta = 64;
+    int warps_per_cta = 8;
+};
+
+struct cos_tab_s {
+    double* T = nullptr;
+    int lattice = 0, L = 0, nsub = 1, n_blocks = 1, n_tau = 0;
+    double beta = 0.0;
+};
+
+extern "C" {
+
+const char* cos_last_error(void) { return g_err.c_str(); }
+
+int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope, int flags,
+                 cos_handle* out)
+{
+    if (!out) return fail(COS_EINVAL, "cos_build: out is NULL");
+    *out = nullptr;
+    if (n < 1 || n > COS_MAX_N) return fail(COS_EINVAL, "cos_build: n must be in [1, 12]");
+    if (n_flavors < 1) return fail(COS_EINVAL, "cos_build: n_flavors must be >= 1");
+    if (lattice != COS_LATTICE_SQUARE && lattice != COS_LATTICE_HONEYCOMB)
+        return fail(COS_EINVAL, "cos_build: unknown lattice");
+    if (readout_envelope != 0 && readout_envelope != n)
+        return fail(COS_EINVAL, "cos_build: readout_envelope must be 0 or n");
+    if (shifts && n_flavors > COS_MAX_COLOURS)
+        return fail(COS_EUNSUPPORTED, "cos_build: SB-CoS supports at most 4 flavours");
+    const int nsub = lattice == COS_LATTICE_HONEYCOMB ? 2 : 1;
+    if (n * nsub > 24) return fail(COS_EUNSUPPORTED, "cos_build: n * n_sub must be <= 24");
+
+    cos_handle_s* h = new (std::nothrow) cos_handle_s();
+    if (!h) return fail(COS_ENOMEM, "cos_build: out of host memory");
+    std::string err = compile_dag(n, n_flavors, nsub, shifts, readout_envelope == n, h->dag);
+    if (!err.empty()) { delete h; return fail(COS_ENOMEM, "cos_build: " + err); }
+
+    const CompiledDag& D = h->dag;
+    const size_t smem = layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d, D.has_shift);
+    if (smem > 227u * 1024u) {
+        delete h;
+        return fail(COS_EUNSUPPORTED, "cos_build: propagator tile does not fit the 227 KB shared memory of one SM");
+    }
+    // launch shape: keep >= 16 warps per SM when shared memory allows several CTAs per SM
+    h->warps_per_cta = env_int("COS_WARPS_PER_CTA", smem > 110u * 1024u ? 16 : 8);
+    h->masks_per_cta = env_int("COS_MASKS_PER_CTA", smem > 110u * 1024u ? 128 : 64);
+    if (h->masks_per_cta < 1) h->masks_per_cta = 1;
+
+    if (!(flags & COS_BUILD_HOST_ONLY)) {
+        int ndev = 0;
+        cudaError_t e = cudaGetDeviceCount(&ndev);
+        if (e != cudaSuccess || ndev == 0) {
+            delete h;
+            return fail(COS_ECUDA, "cos_build: no CUDA device (there is no CPU fallback; use COS_BUILD_HOST_ONLY to inspect the DAG)");
+        }
+        cudaGetDevice(&h->device);
+        e = configure_layer_kernels();
+        if (e != cudaSuccess) { delete h; return cuda_fail(e, "cos_build: cudaFuncSetAttribute"); }
+        h->dl.resize(D.layers.size());
+        for (size_t l = 0; l < D.layers.size(); ++l) {
+            const LayerProgram& P = D.layers[l];
+            const size_t wb = P.words.size() * sizeof(uint32_t), mb = P.mask_off.size() * sizeof(uint32_t);
+            if (wb == 0) continue;
+            e = cudaMalloc(&h->dl[l].words, wb);
+            if (e == cudaSuccess) e = cudaMalloc(&h->dl[l].mask_off, mb);
+            if (e == cudaSuccess) e = cudaMemcpy(h->dl[l].words, P.words.data(), wb, cudaMemcpyHostToDevice);
+            if (e == cudaSuccess) e = cudaMemcpy(h->dl[l].mask_off, P.mask_off.data(), mb, cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) { cos_free(h); return cuda_fail(e, "cos_build: uploading the layer program"); }
+            h->program_bytes += wb + mb;
+        }
+        h->on_device = true;
+        // the host copy of the program is no longer needed
+        for (auto& P : h->dag.layers) { std::vector<uint32_t>().swap(P.words); std::vector<uint32_t>().swap(P.mask_off); }
+    } else {
+        for (const auto& P : D.layers) h->program_bytes += (P.words.size() + P.mask_off.size()) * sizeof(uint32_t);
+    }
+    *out = h;
+    return COS_OK;
+}
+
+int cos_build(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope, cos_handle* out)
+{
+    return cos_build_ex(n, n_flavors, lattice, shifts, readout_envelope, 0, out);
+}
+
+void cos_free(cos_handle h)
+{
+    if (!h) return;
+    for (auto& l : h->dl) { if (l.words) cudaFree(l.words); if (l.mask_off) cudaFree(l.mask_off); }
+    if (h->ws) cudaFree(h->ws);
+    delete h;
+}
+
+int cos_set_workspace_limit(cos_handle h, long long bytes)
+{
+    if (!h || bytes <= 0) return fail(COS_EINVAL, "cos_set_workspace_limit: bad argument");
+    h->ws_limit = bytes;
+    return COS_OK;
+}
+
+int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev, cos_stream stream_)
+{
+    if (!h) return fail(COS_EINVAL, "cos_eval: handle is NULL");
+    if (batch < 0) return fail(COS_EINVAL, "cos_eval: negative batch");
+    if (batch == 0) return COS_OK;
+    if (!G_dev || !out_dev) return fail(COS_EINVAL, "cos_eval: NULL device pointer");
+    if (!h->on_device) return fail(COS_ECUDA, "cos_eval: handle was built host-only / without a CUDA device (no CPU fallback)");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const CompiledDag& D = h->dag;
+    const int NL = (int)D.layers.size();
+
+    // ---- batch chunking against the workspace budget: two slabs of max_layer_states x 32 doubles per tile
+    const long long tiles_total = (batch + TILE - 1) / TILE;
+    const size_t tile_bytes = (size_t)D.max_layer_states * TILE * sizeof(double) * 2;
+    long long tiles_chunk = (long long)((size_t)h->ws_limit / tile_bytes);
+    if (tiles_chunk < 1) tiles_chunk = 1;
+    if (tiles_chunk > tiles_total) tiles_chunk = tiles_total;
+    const int max_tiles_env = env_int("COS_TILES_PER_CHUNK", 0);
+    if (max_tiles_env > 0 && tiles_chunk > max_tiles_env) tiles_chunk = max_tiles_env;
+    const size_t need = tile_bytes * (size_t)tiles_chunk;
+    if (need > h->ws_bytes) {
+        if (h->ws) { cudaFree(h->ws); h->ws = nullptr; h->ws_bytes = 0; }
+        cudaError_t e = cudaMalloc(&h->ws, need);
+        if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, "cos_eval: workspace allocation"); }
+        h->ws_bytes = need;
+    }
+    double* slab[2] = {h->ws, h->ws + (size_t)D.max_layer_states * TILE * (size_t)tiles_chunk};
+
+    for (long long t0 = 0; t0 < tiles_total; t0 += tiles_chunk) {
+        const uint32_t tiles = (uint32_t)((tiles_total - t0 < tiles_chunk) ? (tiles_total - t0) : tiles_chunk);
+        cudaError_t e = launch_fill_ones(slab[0], (size_t)D.layers[0].n_states * TILE * tiles, stream);
+        if (e != cudaSuccess) return cuda_fail(e, "cos_eval: fill launch");
+        for (int l = 0; l < NL; ++l) {
+            const LayerProgram& P = D.layers[l];
+            LayerArgs a;
+            a.words = h->dl[l].words; a.mask_off = h->dl[l].mask_off;
+            a.n_masks = P.n_masks; a.masks_per_cta = (uint32_t)h->masks_per_cta;
+            a.X = slab[l & 1]; a.Y = slab[(l + 1) & 1];
+            a.S_src = P.n_states; a.S_dst = (l + 1 < NL) ? D.layers[l + 1].n_states : 0;
+            a.G = G_dev; a.batch = batch; a.b0 = t0 * TILE; a.out = out_dev;
+            a.d = D.d; a.n_slots = D.n_blocks * D.d * D.d;
+            a.neg_kappa = -D.kappa;
+            for (int c = 0; c < 4; ++c) a.shift[c] = (l == 0 ? -2.0 : -1.0) * D.sigma[c];
+            e = launch_layer(a, (int)D.max_L, D.nc, D.has_shift, tiles, h->warps_per_cta, stream);
+            if (e != cudaSuccess) return cuda_fail(e, "cos_eval: layer launch");
+        }
+    }
+    return COS_OK;
+}
+
+int cos_info(cos_handle h, int what, long long* value)
+{
+    if (!h || !value) return fail(COS_EINVAL, "cos_info: NULL argument");
+    const CompiledDag& D = h->dag;
+    const int NL = (int)D.layers.size();
+    if (what >= COS_INFO_LAYER_STATES && what < COS_INFO_LAYER_STATES + NL) { *value = D.layers[what - COS_INFO_LAYER_STATES].n_states; return COS_OK; }
+    if (what >= COS_INFO_LAYER_EDGES && what < COS_INFO_LAYER_EDGES + NL) {
+        const LayerProgram& P = D.layers[what - COS_INFO_LAYER_EDGES];
+        *value = (long long)(P.e1 + P.e2 + P.e3 + P.e4 + P.readout_edges); return COS_OK;
+    }
+    if (what >= COS_INFO_LAYER_MASKS && what < COS_INFO_LAYER_MASKS + NL) { *value = D.layers[what - COS_INFO_LAYER_MASKS].n_masks; return COS_OK; }
+    switch (what) {
+        case COS_INFO_N_LAYERS: *value = NL; break;
+        case COS_INFO_N_STATES: *value = (long long)D.n_states; break;
+        case COS_INFO_N_EDGES: *value = (long long)D.n_edges; break;
+        case COS_INFO_N_READOUT_EDGES: *value = (long long)D.n_readout_edges; break;
+        case COS_INFO_N_OUT: *value = D.n_out; break;
+        case COS_INFO_MAX_LAYER_STATES: *value = D.max_layer_states; break;
+        case COS_INFO_N_MASKS: *value = (long long)D.n_masks; break;
+        case COS_INFO_N_ROWS: *value = (long long)D.n_rows; break;
+        case COS_INFO_N_FMA: *value = (long long)D.n_fma; break;
+        case COS_INFO_PROGRAM_BYTES: *value = (long long)h->program_bytes; break;
+        case COS_INFO_D: *value = D.d; break;
+        case COS_INFO_N_BLOCKS: *value = D.n_blocks; break;
+        case COS_INFO_N_STATES_UNPRUNED: *value = (long long)D.n_states_unpruned; break;
+        case COS_INFO_WORKSPACE_BYTES: *value = (long long)h->ws_bytes; break;
+        default: return fail(COS_EINVAL, "cos_info: unknown query");
+    }
+    return COS_OK;
+}
+
+int cos_tab_build(int lattice, int L, int n_blocks, double beta, int n_tau, const double* table_host, cos_tab* out)
+{
+    if (!out) return fail(COS_EINVAL, "cos_tab_build: out is NULL");
+    *out = nullptr;
+    if (!table_host || L < 1 || n_blocks < 1 || n_tau < 2 || !(beta > 0.0) ||
+        (lattice != COS_LATTICE_SQUARE && lattice != COS_LATTICE_HONEYCOMB))
+        return fail(COS_EINVAL, "cos_tab_build: bad argument");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(COS_ECUDA, "cos_tab_build: no CUDA device");
+    cos_tab_s* t = new (std::nothrow) cos_tab_s();
+    if (!t) return fail(COS_ENOMEM, "cos_tab_build: out of host memory");
+    t->lattice = lattice; t->L = L; t->nsub = lattice == COS_LATTICE_HONEYCOMB ? 2 : 1;
+    t->n_blocks = n_blocks; t->n_tau = n_tau; t->beta = beta;
+    const size_t bytes = (size_t)n_blocks * t->nsub * t->nsub * L * L * n_tau * sizeof(double);
+    cudaError_t e = cudaMalloc(&t->T, bytes);
+    if (e == cudaSuccess) e = cudaMemcpy(t->T, table_host, bytes, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { if (t->T) cudaFree(t->T); delete t; cudaGetLastError(); return cuda_fail(e, "cos_tab_build"); }
+    *out = t;
+    return COS_OK;
+}
+
+int cos_tabulate(cos_tab tab, int n, const int* sites_dev, const double* tau_dev, long long batch, double* G_dev,
+                 cos_stream stream)
+{
+    if (!tab || n < 1 || n > COS_MAX_N || batch < 0) return fail(COS_EINVAL, "cos_tabulate: bad argument");
+    if (batch == 0) return COS_OK;
+    if (!sites_dev || !tau_dev || !G_dev) return fail(COS_EINVAL, "cos_tabulate: NULL device pointer");
+    TabArgs a;
+    a.T = tab->T; a.L = tab->L; a.nsub = tab->nsub; a.n_blocks = tab->n_blocks; a.n_tau = tab->n_tau; a.beta = tab->beta;
+    a.n = n; a.sites = sites_dev; a.tau = tau_dev; a.batch = batch; a.G = G_dev;
+    cudaError_t e = launch_tabulate(a, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "cos_tabulate: launch");
+    return COS_OK;
+}
+
+void cos_tab_free(cos_tab tab)
+{
+    if (!tab) return;
+    if (tab->T) cudaFree(tab->T);
+    delete tab;
+}
+
+int cos_measure_fp64_fma_peak(double* fma_per_s)
+{
+    if (!fma_per_s) return fail(COS_EINVAL, "cos_measure_fp64_fma_peak: NULL argument");
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(COS_ECUDA, "no CUDA device");
+    cudaError_t e = measure_fp64_fma(fma_per_s);
+    if (e != cudaSuccess) return cuda_fail(e, "cos_measure_fp64_fma_peak");
+    return COS_OK;
+}
+
+}  // extern "C"

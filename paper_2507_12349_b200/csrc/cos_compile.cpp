@@ -1,0 +1,286 @@
+// cos_compile.cpp -- host-side DAG compiler (north_star subsystem (1)).
+//
+// Enumerates the reachable states of the reduced CoS / SB-CoS recurrence (forward sets F_l, Eq. 19-20),
+// prunes them against the requested readouts (backward sets B_l, Eq. 21-24; K_l = F_l ^ B_l, Eq. 23),
+// numbers them layer by layer (layer = total occupancy - 1) and emits the per-layer block/row program
+// described in cos_compile.h.  Integer / structural work only; nothing numeric happens here.
+//
+// Transition rules (j ranges over labels >= r = min supp(m), Eq. 9-11):
+//   E1  continue into an untouched interaction j, every sublattice s_j : multiplicity 2   (Eq. 11, Lemma 7)
+//   E2  continue into the partner of a singly occupied interaction j   : multiplicity 1   (Eq. 11)
+//   E3  counterterm one-cycle at the partner of the current endpoint   : -sigma_lambda    (Eq. 60, 72, 77)
+//       (same destination as E2 with j = e; the kernel applies it as a diagonal correction)
+//   E4  close (-kappa G[e][h]) and open the canonical head j = min{i: m_i = 1}, every colour (Eq. 12, 70-71)
+//   readout when no interaction is singly occupied: out[S] += -kappa G[e][h] x               (Eq. 14-15)
+#include "cos_compile.h"
+
+#include <algorithm>
+#include <cstring>
+
+namespace cosb {
+namespace {
+
+struct JEntry {
+    uint8_t j_a;        // destination endpoint index (j, s_j)
+    uint8_t mult2;      // 1: multiplicity 2 (untouched interaction), 0: multiplicity 1
+    uint32_t dest_code; // mask code of the destination block
+};
+
+struct Builder {
+    int n, nsub, d, nc;
+    bool all_subsets, has_shift;
+    std::vector<int32_t> index_of;              // mask code -> mask id (-1: not reached)
+    std::vector<uint32_t> codes;                // mask id -> code (2 bits per interaction: 0, 1=(1,A), 2=(1,B), 3=full)
+    std::vector<uint32_t> alive;                // [id*d + h_a] bitmask over e_a of live states (colour-independent)
+    std::vector<uint32_t> row_base;             // [id*d + h_a] slab index of state (h_a, lambda=0, first e)
+    std::vector<std::vector<uint32_t>> by_layer;
+
+    static int cell(uint32_t code, int i) { return (code >> (2 * i)) & 3; }
+    int root(uint32_t code) const { for (int i = 0; i < n; ++i) if (cell(code, i)) return i; return n; }
+    int jmin(uint32_t code) const {             // canonical open interaction, Eq. 12
+        for (int i = 0; i < n; ++i) { int c = cell(code, i); if (c == 1 || c == 2) return i; }
+        return -1;
+    }
+    uint32_t full_set(uint32_t code) const {
+        uint32_t S = 0;
+        for (int i = 0; i < n; ++i) if (cell(code, i) == 3) S |= 1u << i;
+        return S;
+    }
+    uint32_t get_mask(uint32_t code, int layer) {
+        int32_t id = index_of[code];
+        if (id >= 0) return (uint32_t)id;
+        id = (int32_t)codes.size();
+        index_of[code] = id;
+        codes.push_back(code);
+        alive.resize((size_t)(id + 1) * d, 0u);
+        by_layer[layer].push_back((uint32_t)id);
+        return (uint32_t)id;
+    }
+    int jlist(uint32_t code, JEntry* out) const {
+        int k = 0;
+        for (int i = root(code); i < n; ++i) {
+            int c = cell(code, i);
+            if (c == 0) {
+                for (int s = 0; s < nsub; ++s) {
+                    out[k].j_a = (uint8_t)(i * nsub + s); out[k].mult2 = 1;
+                    out[k].dest_code = code | ((uint32_t)(1 + s) << (2 * i)); ++k;
+                }
+            } else if (c != 3) {
+                out[k].j_a = (uint8_t)(i * nsub + (c - 1)); out[k].mult2 = 0;
+                out[k].dest_code = code | (3u << (2 * i)); ++k;
+            }
+        }
+        return k;
+    }
+    uint32_t state_index(uint32_t id, int h_a, int lam, int e_a) const {
+        uint32_t a = alive[(size_t)id * d + h_a];
+        uint32_t L = (uint32_t)__builtin_popcount(a);
+        return row_base[(size_t)id * d + h_a] + (uint32_t)lam * L + (uint32_t)__builtin_popcount(a & ((1u << e_a) - 1u));
+    }
+};
+
+}  // namespace
+
+std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_subsets, CompiledDag& out)
+{
+    if (n < 1 || n > 12) return "n must be in [1, 12]";
+    if (nsub != 1 && nsub != 2) return "n_sub must be 1 or 2";
+    if (nf < 1) return "n_flavors must be >= 1";
+    if (sigma && nf > 4) return "SB mode supports at most 4 flavours";
+    if (n * nsub > 24) return "n * n_sub must be <= 24";
+
+    Builder b;
+    b.n = n; b.nsub = nsub; b.d = n * nsub; b.nc = sigma ? nf : 1;
+    b.all_subsets = all_subsets; b.has_shift = (sigma != nullptr);
+    const int d = b.d, nc = b.nc, NL = 2 * n;
+    try {
+        b.index_of.assign((size_t)1 << (2 * n), -1);
+        b.by_layer.assign(NL, {});
+
+        // ---- initial states (Eq. 66; reading G8 for the rooted branches): (r, s) head = endpoint, m = (1,s) e_r
+        for (int r = 0; r < (all_subsets ? n : 1); ++r)
+            for (int s = 0; s < nsub; ++s) {
+                uint32_t id = b.get_mask((uint32_t)(1 + s) << (2 * r), 0);
+                int a = r * nsub + s;
+                b.alive[(size_t)id * d + a] |= 1u << a;
+            }
+
+        // ---- forward reachability, Eq. 19-20
+        JEntry J[24];
+        for (int l = 0; l + 1 < NL; ++l) {
+            for (size_t k = 0; k < b.by_layer[l].size(); ++k) {
+                const uint32_t id = b.by_layer[l][k], code = b.codes[id];
+                const int nJ = b.jlist(code, J);
+                uint32_t dest[24];
+                for (int q = 0; q < nJ; ++q) dest[q] = b.get_mask(J[q].dest_code, l + 1);
+                for (int h = 0; h < d; ++h) {
+                    if (!b.alive[(size_t)id * d + h]) continue;
+                    for (int q = 0; q < nJ; ++q) b.alive[(size_t)dest[q] * d + h] |= 1u << J[q].j_a;
+                }
+                const int jm = b.jmin(code);
+                if (jm >= 0) {
+                    bool any = false;
+                    for (int h = 0; h < d; ++h) any = any || b.alive[(size_t)id * d + h];
+                    if (any) {
+                        const int fa = jm * nsub + (Builder::cell(code, jm) - 1);
+                        uint32_t did = b.get_mask(code | (3u << (2 * jm)), l + 1);
+                        b.alive[(size_t)did * d + fa] |= 1u << fa;
+                    }
+                }
+            }
+        }
+        uint64_t unpruned = 0;
+        for (uint32_t a : b.alive) unpruned += (uint64_t)__builtin_popcount(a) * nc;
+
+        // ---- backward productivity, Eq. 21-24, then K_l = F_l ^ B_l (Eq. 23)
+        const uint32_t FULL = (n == 16) ? 0xFFFFu : ((1u << n) - 1u);
+        std::vector<uint32_t> prod(b.alive.size(), 0u);
+        for (int l = NL - 1; l >= 0; --l) {
+            for (uint32_t id : b.by_layer[l]) {
+                const uint32_t code = b.codes[id];
+                const int jm = b.jmin(code);
+                const bool readout = (jm < 0) && (all_subsets || b.full_set(code) == FULL);
+                bool fresh_ok = false;
+                if (jm >= 0 && l + 1 < NL) {
+                    const int fa = jm * nsub + (Builder::cell(code, jm) - 1);
+                    int32_t did = b.index_of[code | (3u << (2 * jm))];
+                    fresh_ok = did >= 0 && ((prod[(size_t)did * d + fa] >> fa) & 1u);
+                }
+                const int nJ = (l + 1 < NL) ? b.jlist(code, J) : 0;
+                for (int h = 0; h < d; ++h) {
+                    const uint32_t a = b.alive[(size_t)id * d + h];
+                    if (!a) continue;
+                    bool p = readout || fresh_ok;
+                    for (int q = 0; q < nJ && !p; ++q) {
+                        int32_t did = b.index_of[J[q].dest_code];
+                        p = did >= 0 && ((prod[(size_t)did * d + h] >> J[q].j_a) & 1u);
+                    }
+                    prod[(size_t)id * d + h] = p ? a : 0u;
+                }
+            }
+        }
+        b.alive.swap(prod);
+        prod.clear(); prod.shrink_to_fit();
+
+        // ---- numbering: layer slab order = [block (by mask code)][head][colour][endpoint]
+        out = CompiledDag();
+        out.n = n; out.nf = nf; out.nsub = nsub; out.d = d; out.nc = nc;
+        out.n_blocks = sigma ? nf : 1;
+        out.uniform = (sigma == nullptr); out.all_subsets = all_subsets; out.has_shift = (sigma != nullptr);
+        out.kappa = sigma ? 1.0 : (double)nf;
+        out.n_out = all_subsets ? (int)FULL : 1;
+        for (int l = 0; l < nc && sigma; ++l) out.sigma[l] = sigma[l];
+        out.n_states_unpruned = unpruned;
+        out.layers.assign(NL, LayerProgram());
+        b.row_base.assign(b.alive.size(), 0u);
+        for (int l = 0; l < NL; ++l) {
+            auto& ids = b.by_layer[l];
+            std::vector<uint32_t> keep;
+            for (uint32_t id : ids) {
+                bool any = false;
+                for (int h = 0; h < d; ++h) any = any || b.alive[(size_t)id * d + h];
+                if (any) keep.push_back(id);
+            }
+            std::sort(keep.begin(), keep.end(), [&](uint32_t x, uint32_t y) { return b.codes[x] < b.codes[y]; });
+            ids.swap(keep);
+            uint64_t counter = 0;
+            for (uint32_t id : ids)
+                for (int h = 0; h < d; ++h) {
+                    const uint32_t a = b.alive[(size_t)id * d + h];
+                    if (!a) continue;
+                    b.row_base[(size_t)id * d + h] = (uint32_t)counter;
+                    counter += (uint64_t)__builtin_popcount(a) * nc;
+                }
+            if (counter >= DIDX_DEFER) return "layer too large for the 26-bit destination index";
+            out.layers[l].n_states = (uint32_t)counter;
+            out.layers[l].n_masks = (uint32_t)ids.size();
+        }
+
+        // ---- emission
+        const int HDR = out.hdr_words();
+        for (int l = 0; l < NL; ++l) {
+            LayerProgram& P = out.layers[l];
+            P.mask_off.reserve(P.n_masks + 1);
+            for (uint32_t id : b.by_layer[l]) {
+                const uint32_t code = b.codes[id];
+                const int jm = b.jmin(code);
+                const int nJ = (l + 1 < NL) ? b.jlist(code, J) : 0;
+                uint32_t flags = 0, fresh_a = 0, out_idx = 0;
+                int32_t fresh_did = -1;
+                if (jm >= 0 && l + 1 < NL) {
+                    fresh_a = (uint32_t)(jm * nsub + (Builder::cell(code, jm) - 1));
+                    fresh_did = b.index_of[code | (3u << (2 * jm))];
+                    if (fresh_did >= 0 && ((b.alive[(size_t)fresh_did * d + fresh_a] >> fresh_a) & 1u)) flags |= FLAG_FRESH;
+                }
+                if (jm < 0 && (all_subsets || b.full_set(code) == FULL)) {
+                    flags |= FLAG_READOUT;
+                    out_idx = all_subsets ? b.full_set(code) - 1u : 0u;
+                }
+                const bool need_close = flags != 0;
+                uint32_t n_rows = 0, Lmax = 0;
+                for (int h = 0; h < d; ++h) {
+                    const uint32_t a = b.alive[(size_t)id * d + h];
+                    if (a) { n_rows += nc; Lmax = std::max(Lmax, (uint32_t)__builtin_popcount(a)); }
+                }
+                const uint32_t e_words = (Lmax + 3) / 4, stride = 2 + e_words + (uint32_t)nJ;
+                if (stride > 32) return "row record exceeds 32 words";
+                if (P.words.size() + HDR + (size_t)n_rows * stride >= 0xFFFFFFFFull) return "layer program too large";
+                P.mask_off.push_back((uint32_t)P.words.size());
+                P.words.push_back(n_rows | ((uint32_t)nJ << 16) | (flags << 24));
+                P.words.push_back(stride | (e_words << 8) | (fresh_a << 16));
+                P.words.push_back(out_idx);
+                for (int lam = 0; lam < nc; ++lam)
+                    P.words.push_back((flags & FLAG_FRESH) ? b.state_index((uint32_t)fresh_did, (int)fresh_a, lam, (int)fresh_a)
+                                                            : DIDX_DEAD);
+                int32_t dest[24];
+                for (int q = 0; q < nJ; ++q) dest[q] = b.index_of[J[q].dest_code];
+                for (int h = 0; h < d; ++h) {
+                    const uint32_t a = b.alive[(size_t)id * d + h];
+                    if (!a) continue;
+                    const uint32_t L = (uint32_t)__builtin_popcount(a);
+                    for (int lam = 0; lam < nc; ++lam) {
+                        const size_t w_begin = P.words.size();
+                        P.words.push_back(b.row_base[(size_t)id * d + h] + (uint32_t)lam * L);
+                        P.words.push_back(L | ((uint32_t)h << 8) | ((uint32_t)lam << 16));
+                        uint32_t packed[6] = {0, 0, 0, 0, 0, 0};
+                        int k = 0;
+                        for (int e = 0; e < d; ++e)
+                            if ((a >> e) & 1u) { packed[k / 4] |= (uint32_t)e << (8 * (k % 4)); ++k; }
+                        for (uint32_t w = 0; w < e_words; ++w) P.words.push_back(packed[w]);
+                        uint32_t alive_j = 0;
+                        for (int q = 0; q < nJ; ++q) {
+                            uint32_t didx = DIDX_DEAD;
+                            const bool live = dest[q] >= 0 && ((b.alive[(size_t)dest[q] * d + h] >> J[q].j_a) & 1u);
+                            if (live) {
+                                ++alive_j;
+                                if ((flags & FLAG_FRESH) && (uint32_t)h == fresh_a && J[q].j_a == fresh_a) didx = DIDX_DEFER;
+                                else didx = b.state_index((uint32_t)dest[q], h, lam, J[q].j_a);
+                                if (J[q].mult2) P.e1 += L; else P.e2 += L;
+                            }
+                            P.words.push_back(didx | ((uint32_t)J[q].j_a << 26) | ((uint32_t)J[q].mult2 << 31));
+                        }
+                        if (b.has_shift && l + 1 < NL)      // E3: states whose current interaction is singly occupied
+                            for (int e = 0; e < d; ++e)
+                                if (((a >> e) & 1u)) { int c = Builder::cell(code, e / nsub); if (c == 1 || c == 2) P.e3 += 1; }
+                        if (flags & FLAG_FRESH) P.e4 += (uint64_t)L * nc;
+                        if (flags & FLAG_READOUT) P.readout_edges += L;
+                        P.n_fma += (uint64_t)L * (alive_j + (need_close ? 1u : 0u));
+                        (void)w_begin;
+                    }
+                }
+                P.n_rows += n_rows;
+                P.max_L = std::max(P.max_L, Lmax);
+            }
+            P.mask_off.push_back((uint32_t)P.words.size());
+            out.n_states += P.n_states; out.n_masks += P.n_masks; out.n_rows += P.n_rows;
+            out.n_edges += P.e1 + P.e2 + P.e3 + P.e4; out.n_readout_edges += P.readout_edges; out.n_fma += P.n_fma;
+            out.max_layer_states = std::max(out.max_layer_states, P.n_states);
+            out.max_L = std::max(out.max_L, P.max_L);
+        }
+    } catch (const std::bad_alloc&) {
+        return "out of host memory while compiling the DAG";
+    }
+    return "";
+}
+
+}  // namespace cosb

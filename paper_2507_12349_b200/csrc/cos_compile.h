@@ -1,0 +1,55 @@
+// cos_compile.h -- host-side DAG compiler of the CoS / SB-CoS recurrence (internal header).
+//
+// State of the reduced ("R-form") recurrence, Eq. 3-4, 8-12, 79-80:
+//     X = (h, s_h, e, s_e, lambda, m),   m_i in {0, (1,s), 2}
+// The compiler groups states by occupancy mask m ("block") and by (head, colour) ("row"); all
+// continuation sources of a destination are one row (tail-vector form) and every
+// destination state receives all of its contributions from ONE source block, which is what lets the
+// kernel write each state exactly once without atomics.
+#pragma once
+#include <cstdint>
+#include <string>
+#include <vector>
+
+namespace cosb {
+
+// ---- program stream format (u32 words), one stream per layer ---------------------------------------
+// block header (HDR_WORDS = 3 + nc words):
+//   w0 : n_rows[0:16) | nJ[16:24) | flags[24:32)        flags: bit0 FRESH (close-and-open target alive),
+//                                                               bit1 READOUT (terminal readout, Eq. 14-15)
+//   w1 : row_stride[0:8) | e_words[8:16) | fresh_a[16:24)
+//   w2 : out_idx (readout row of out_dev)
+//   w3..w3+nc-1 : destination state index (next layer) of the fresh-head state of colour lambda'
+// row (row_stride = 2 + e_words + nJ words):
+//   w0 : index of the row's first state in this layer's slab (row states are contiguous)
+//   w1 : L[0:8) | h_a[8:16) | lambda[16:24) | rflags[24:32)
+//   w2.. : e_a of the L states, one byte each
+//   then nJ words: dj = didx[0:26) | j_a[26:31) | mult2[31]   (destination index in the next layer,
+//        destination endpoint, multiplicity 2 - m_j of Lemma 7 as a flag)
+static const uint32_t DIDX_MASK = 0x03FFFFFFu;
+static const uint32_t DIDX_DEAD = 0x03FFFFFFu;     // destination pruned (Eq. 23)
+static const uint32_t DIDX_DEFER = 0x03FFFFFEu;    // merges with the fresh-head state (coalesced E2/E4 pair)
+static const uint32_t FLAG_FRESH = 1u, FLAG_READOUT = 2u;
+
+struct LayerProgram {
+    uint32_t n_states = 0, n_masks = 0, n_rows = 0, max_L = 0;
+    std::vector<uint32_t> words;
+    std::vector<uint32_t> mask_off;      // [n_masks + 1] word offsets of the block headers
+    uint64_t e1 = 0, e2 = 0, e3 = 0, e4 = 0, readout_edges = 0, n_fma = 0;
+};
+
+struct CompiledDag {
+    int n = 0, nf = 0, nsub = 1, d = 0, nc = 1, n_blocks = 1, n_out = 1;
+    bool uniform = true, all_subsets = false, has_shift = false;
+    double sigma[4] = {0, 0, 0, 0};
+    double kappa = 1.0;
+    std::vector<LayerProgram> layers;    // 2n layers; layer l holds the transitions l -> l+1 and the readouts at l
+    uint64_t n_states = 0, n_states_unpruned = 0, n_masks = 0, n_rows = 0, n_edges = 0, n_readout_edges = 0, n_fma = 0;
+    uint32_t max_layer_states = 0, max_L = 0;
+    int hdr_words() const { return 3 + nc; }
+};
+
+// Returns "" on success, else an error message.  n in [1,12]; nsub in {1,2}; sigma == nullptr -> uniform.
+std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_subsets, CompiledDag& out);
+
+}  // namespace cosb

@@ -1,0 +1,323 @@
+// cos_kernels.cu -- sm_100a kernels of the CoS / SB-CoS DAG evaluator.
+//
+//  cos_layer_kernel   north_star (3)+(4): one layer step x_t += c_e L[x_s] (Eq. 16) for every
+//                     state of the next layer, plus the terminal readouts of this layer (Eq. 14-15).
+//  cos_tabulate_kernel north_star (2): propagator lookup with linear tau-interpolation (Eq. 32).
+//  cos_fill_kernel    layer-0 initial states <- 1 (Eq. 66).
+//  fp64 FMA peak probe for the roofline report.
+//
+// Work decomposition of the layer kernel:
+//   lane  = configuration (32 per batch tile, the contiguous dimension of every array),
+//   warp  = one occupancy-mask block at a time: all rows (head, colour) of the block,
+//   CTA   = `masks_per_cta` blocks x one batch tile; the tile's propagator table G (all blocks, d x d,
+//           32 configurations) is staged once in shared memory.
+// For one row the L source values are loaded ONCE into registers (contiguous states, coalesced
+// 256-byte lines), every continuation destination is a length-L dot product against a column of
+// G in shared memory (1 LDS.64 + 1 DFMA per DAG edge), and the cycle-closing sum of the whole block is
+// accumulated in a register.  Every destination state is written exactly once: no atomics, no
+// second pass, HBM traffic = one read + one write per state.
+#include "cos_kernels.cuh"
+#include "cos_compile.h"
+
+namespace cosb {
+
+static const int MAX_WARPS = 16;
+
+// ------------------------------------------------------------------------------------------------------
+// One row of a block: L contiguous source states, nJ destinations.
+template <int L, int NC, bool SHIFT>
+__device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t base, const int h_a, const int lam,
+                                         const int nJ, const int e_words, const bool need_close,
+                                         const int d, const int n_slots,
+                                         const double* __restrict__ Xt, double* __restrict__ Yt,
+                                         const double* __restrict__ Gl, double& close, double (&sp)[NC])
+{
+    double x[L];
+    int goff[L];
+    const double* xp = Xt + (size_t)base * TILE;
+#pragma unroll
+    for (int k = 0; k < L; ++k) x[k] = __ldcs(xp + (size_t)k * TILE);
+#pragma unroll
+    for (int k = 0; k < L; ++k) {
+        const uint32_t ew = __shfl_sync(0xFFFFFFFFu, rw, 2 + (k >> 2));
+        const int e_k = (int)((ew >> (8 * (k & 3))) & 0xFFu);
+        goff[k] = ((lam * d + e_k) * d) * TILE;
+    }
+    if (need_close) {                       // cycle-closing factor G_lam[e][h] (Eq. 12, 15)
+        const double* gh = Gl + h_a * TILE;
+#pragma unroll
+        for (int k = 0; k < L; ++k) close = fma(gh[goff[k]], x[k], close);
+    }
+    for (int jj = 0; jj < nJ; ++jj) {
+        const uint32_t dj = __shfl_sync(0xFFFFFFFFu, rw, 2 + e_words + jj);
+        const uint32_t didx = dj & DIDX_MASK;
+        if (didx == DIDX_DEAD) continue;
+        const int j_a = (int)((dj >> 26) & 31u);
+        const double* gj = Gl + j_a * TILE;
+        const int jgoff = ((lam * d + j_a) * d) * TILE;          // row of G whose source endpoint is j itself
+        const double* gdiag = Gl + (n_slots + lam * d + j_a) * TILE;
+        double acc0 = 0.0, acc1 = 0.0;
+#pragma unroll
+        for (int k = 0; k < L; ++k) {
+            const double* p = gj + goff[k];
+            if (SHIFT) p = (goff[k] == jgoff) ? gdiag : p;      // E2 with e = j merged with the counterterm E3
+            if (k & 1) acc1 = fma(*p, x[k], acc1); else acc0 = fma(*p, x[k], acc0);
+        }
+        double acc = acc0 + acc1;
+        if (dj >> 31) acc += acc;                                // multiplicity 2 - m_j (Lemma 7)
+        if (didx == DIDX_DEFER) {
+#pragma unroll
+            for (int c = 0; c < NC; ++c) sp[c] = (c == lam) ? acc : sp[c];
+        } else {
+            Yt[(size_t)didx * TILE] = acc;
+        }
+    }
+}
+
+template <int MAXL, int NC, bool SHIFT>
+__global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerArgs a)
+{
+    extern __shared__ double Gs[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
+    const uint32_t tile = blockIdx.x;
+    const int HDR = 3 + NC;
+
+    // ---- stage the tile's propagator table: Gs[slot][lane]
+    const long long b = a.b0 + (long long)tile * TILE + lane;
+    const bool valid = b < a.batch;
+    for (int s = warp; s < a.n_slots; s += W)
+        Gs[s * TILE + lane] = valid ? __ldg(a.G + (size_t)s * (size_t)a.batch + (size_t)b) : 0.0;
+    __syncthreads();
+    if (SHIFT) {                             // shifted diagonal G_lam[a][a] + c3 sigma_lam (Eq. 49 / 72, 77)
+        for (int q = warp; q < NC * a.d; q += W) {
+            const int lam = q / a.d, e = q - lam * a.d;
+            const double sh = lam == 0 ? a.shift[0] : lam == 1 ? a.shift[1] : lam == 2 ? a.shift[2] : a.shift[3];
+            Gs[(a.n_slots + q) * TILE + lane] = Gs[((lam * a.d + e) * a.d + e) * TILE + lane] + sh;
+        }
+        __syncthreads();
+    }
+
+    const uint32_t m_begin = blockIdx.y * a.masks_per_cta;
+    const uint32_t m_end = min(a.n_masks, m_begin + a.masks_per_cta);
+    const double* Xt = a.X + (size_t)tile * a.S_src * TILE + lane;
+    double* Yt = a.Y + (size_t)tile * a.S_dst * TILE + lane;
+    const double* Gl = Gs + lane;
+
+    for (uint32_t mi = m_begin + warp; mi < m_end; mi += W) {
+        const uint32_t off = __ldg(a.mask_off + mi);
+        const uint32_t hw = (lane < HDR) ? __ldg(a.words + off + lane) : 0u;
+        const uint32_t w0 = __shfl_sync(0xFFFFFFFFu, hw, 0), w1 = __shfl_sync(0xFFFFFFFFu, hw, 1);
+        const int n_rows = (int)(w0 & 0xFFFFu), nJ = (int)((w0 >> 16) & 0xFFu);
+        const uint32_t flags = w0 >> 24;
+        const int stride = (int)(w1 & 0xFFu), e_words = (int)((w1 >> 8) & 0xFFu);
+        const bool need_close = flags != 0u;
+        double close = 0.0;
+        double sp[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) sp[c] = 0.0;
+
+        const uint32_t* rp = a.words + off + HDR;
+        uint32_t rw = (lane < stride) ? __ldg(rp + lane) : 0u;
+        for (int r = 0; r < n_rows; ++r) {
+            uint32_t rw_next = 0u;
+            if (r + 1 < n_rows && lane < stride) rw_next = __ldg(rp + (size_t)(r + 1) * stride + lane);
+            const uint32_t base = __shfl_sync(0xFFFFFFFFu, rw, 0), rh = __shfl_sync(0xFFFFFFFFu, rw, 1);
+            const int L = (int)(rh & 0xFFu), h_a = (int)((rh >> 8) & 0xFFu), lam = (int)((rh >> 16) & 0xFFu);
+#define COS_ROW_CASE(LL)                                                                                        \
+    case LL:                                                                                                    \
+        if (LL <= MAXL)                                                                                         \
+            row_body<(LL <= MAXL ? LL : 1), NC, SHIFT>(rw, base, h_a, lam, nJ, e_words, need_close, a.d,        \
+                                                       a.n_slots, Xt, Yt, Gl, close, sp);                       \
+        break;
+            switch (L) {
+                COS_ROW_CASE(1) COS_ROW_CASE(2) COS_ROW_CASE(3) COS_ROW_CASE(4) COS_ROW_CASE(5) COS_ROW_CASE(6)
+                COS_ROW_CASE(7) COS_ROW_CASE(8) COS_ROW_CASE(9) COS_ROW_CASE(10) COS_ROW_CASE(11) COS_ROW_CASE(12)
+                COS_ROW_CASE(13) COS_ROW_CASE(14) COS_ROW_CASE(15) COS_ROW_CASE(16) COS_ROW_CASE(17) COS_ROW_CASE(18)
+                COS_ROW_CASE(19) COS_ROW_CASE(20) COS_ROW_CASE(21) COS_ROW_CASE(22) COS_ROW_CASE(23) COS_ROW_CASE(24)
+                default: break;
+            }
+#undef COS_ROW_CASE
+            rw = rw_next;
+        }
+        if (flags & FLAG_FRESH) {            // close-and-open: fresh head of every colour (Eq. 12, 70-71)
+#pragma unroll
+            for (int c = 0; c < NC; ++c) {
+                const uint32_t didx = __shfl_sync(0xFFFFFFFFu, hw, 3 + c);
+                Yt[(size_t)didx * TILE] = fma(a.neg_kappa, close, sp[c]);
+            }
+        }
+        if (flags & FLAG_READOUT) {          // terminal readout O_S (Eq. 15): one block per subset S
+            const uint32_t out_idx = __shfl_sync(0xFFFFFFFFu, hw, 2);
+            if (valid) a.out[(size_t)out_idx * (size_t)a.batch + (size_t)b] = a.neg_kappa * close;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------
+typedef void (*layer_fn)(const LayerArgs);
+
+template <int MAXL>
+static layer_fn pick_nc(int nc, bool shift)
+{
+    if (!shift) {
+        switch (nc) {
+            case 1: return cos_layer_kernel<MAXL, 1, false>;
+            case 2: return cos_layer_kernel<MAXL, 2, false>;
+            case 3: return cos_layer_kernel<MAXL, 3, false>;
+            default: return cos_layer_kernel<MAXL, 4, false>;
+        }
+    }
+    switch (nc) {
+        case 1: return cos_layer_kernel<MAXL, 1, true>;
+        case 2: return cos_layer_kernel<MAXL, 2, true>;
+        case 3: return cos_layer_kernel<MAXL, 3, true>;
+        default: return cos_layer_kernel<MAXL, 4, true>;
+    }
+}
+
+static layer_fn pick_layer_fn(int max_L, int nc, bool shift)
+{
+    if (max_L <= 4) return pick_nc<4>(nc, shift);
+    if (max_L <= 8) return pick_nc<8>(nc, shift);
+    if (max_L <= 12) return pick_nc<12>(nc, shift);
+    if (max_L <= 20) return pick_nc<20>(nc, shift);
+    return pick_nc<24>(nc, shift);
+}
+
+size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift)
+{
+    return (size_t)(n_slots + (shift ? nc * d : 0)) * TILE * sizeof(double);
+}
+
+cudaError_t configure_layer_kernels()
+{
+    static const int Ls[5] = {4, 8, 12, 20, 24};
+    for (int i = 0; i < 5; ++i)
+        for (int nc = 1; nc <= 4; ++nc)
+            for (int sh = 0; sh < 2; ++sh) {
+                cudaError_t e = cudaFuncSetAttribute((const void*)pick_layer_fn(Ls[i], nc, sh != 0),
+                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+                if (e != cudaSuccess) return e;
+            }
+    return cudaSuccess;
+}
+
+cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
+                         cudaStream_t stream)
+{
+    if (a.n_masks == 0 || tiles == 0) return cudaSuccess;
+    if (warps_per_cta < 1) warps_per_cta = 1;
+    if (warps_per_cta > MAX_WARPS) warps_per_cta = MAX_WARPS;
+    const uint32_t chunks = (a.n_masks + a.masks_per_cta - 1) / a.masks_per_cta;
+    if (chunks > 65535u) return cudaErrorInvalidConfiguration;
+    dim3 grid(tiles, chunks, 1), block(32 * warps_per_cta, 1, 1);
+    layer_fn fn = pick_layer_fn(max_L, nc, shift);
+    fn<<<grid, block, layer_smem_bytes(a.n_slots, nc, a.d, shift), stream>>>(a);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------
+__global__ void cos_fill_kernel(double* __restrict__ X, size_t n)
+{
+    size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const size_t step = (size_t)gridDim.x * blockDim.x;
+    for (; i < n; i += step) X[i] = 1.0;
+}
+
+cudaError_t launch_fill_ones(double* X, size_t n, cudaStream_t stream)
+{
+    if (n == 0) return cudaSuccess;
+    size_t blocks = (n + 255) / 256;
+    if (blocks > 148 * 16) blocks = 148 * 16;
+    cos_fill_kernel<<<(unsigned)blocks, 256, 0, stream>>>(X, n);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Propagator tabulation (north_star (2)).  One thread = (configuration, ordered vertex pair (i, j));
+// it writes the n_blocks * n_sub^2 entries of that pair.  Arithmetic order is fixed with explicit
+// round-to-nearest intrinsics (no FMA contraction) so that the result is reproducible bit for bit.
+__global__ void cos_tabulate_kernel(const TabArgs a)
+{
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= a.batch) return;
+    const int pair = blockIdx.y, i = pair / a.n, j = pair - i * a.n;
+    const int xi = a.sites[((size_t)i * 2 + 0) * a.batch + c], yi = a.sites[((size_t)i * 2 + 1) * a.batch + c];
+    const int xj = a.sites[((size_t)j * 2 + 0) * a.batch + c], yj = a.sites[((size_t)j * 2 + 1) * a.batch + c];
+    int dx = (xi - xj) % a.L, dy = (yi - yj) % a.L;
+    if (dx < 0) dx += a.L;
+    if (dy < 0) dy += a.L;
+    const int r = dx * a.L + dy;
+    double dt = __dsub_rn(a.tau[(size_t)i * a.batch + c], a.tau[(size_t)j * a.batch + c]);
+    double sign = 1.0;
+    if (dt <= 0.0) { dt = __dadd_rn(dt, a.beta); sign = -1.0; }      // anti-periodic; equal times use 0^-
+    const double step = a.beta / (double)(a.n_tau - 1);
+    const double u = __ddiv_rn(dt, step);
+    int k = (int)floor(u);
+    if (k > a.n_tau - 2) k = a.n_tau - 2;
+    const double w = __dsub_rn(u, (double)k);
+    const int d = a.n * a.nsub, ns2 = a.nsub * a.nsub;
+    for (int blk = 0; blk < a.n_blocks; ++blk)
+        for (int s = 0; s < a.nsub; ++s)
+            for (int s2 = 0; s2 < a.nsub; ++s2) {
+                const double* t = a.T + (((size_t)blk * ns2 + (size_t)(s * a.nsub + s2)) * (size_t)(a.L * a.L) + r) * a.n_tau + k;
+                const double g = __dadd_rn(__dmul_rn(__dsub_rn(1.0, w), __ldg(t)), __dmul_rn(w, __ldg(t + 1)));
+                a.G[(((size_t)blk * d + (size_t)(i * a.nsub + s)) * d + (size_t)(j * a.nsub + s2)) * (size_t)a.batch + c] =
+                    __dmul_rn(sign, g);
+            }
+}
+
+cudaError_t launch_tabulate(const TabArgs& a, cudaStream_t stream)
+{
+    if (a.batch == 0) return cudaSuccess;
+    dim3 block(128, 1, 1), grid((unsigned)((a.batch + 127) / 128), (unsigned)(a.n * a.n), 1);
+    cos_tabulate_kernel<<<grid, block, 0, stream>>>(a);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------
+__global__ void cos_fp64_peak_kernel(double* sink, int iters, double a0, double b0)
+{
+    double acc[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) acc[q] = (double)(threadIdx.x + q);
+    const double a = a0, bb = b0;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int q = 0; q < 8; ++q) acc[q] = fma(acc[q], a, bb);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) s += acc[q];
+    if (s == 123.456) sink[0] = s;          // never true; keeps the chain alive
+}
+
+cudaError_t measure_fp64_fma(double* fma_per_s)
+{
+    double* sink = nullptr;
+    cudaError_t e = cudaMalloc(&sink, sizeof(double));
+    if (e != cudaSuccess) return e;
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0); cudaEventCreate(&t1);
+    const int blocks = 148 * 8, threads = 256, iters = 1 << 16;
+    cos_fp64_peak_kernel<<<blocks, threads>>>(sink, 1024, 0.999999, 1e-9);       // warm-up
+    double best = 0.0;
+    for (int rep = 0; rep < 3; ++rep) {
+        cudaEventRecord(t0);
+        cos_fp64_peak_kernel<<<blocks, threads>>>(sink, iters, 0.999999, 1e-9);
+        cudaEventRecord(t1);
+        e = cudaEventSynchronize(t1);
+        if (e != cudaSuccess) break;
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, t0, t1);
+        const double rate = (double)blocks * threads * 8.0 * (double)iters / (ms * 1e-3);
+        if (rate > best) best = rate;
+    }
+    cudaEventDestroy(t0); cudaEventDestroy(t1);
+    cudaFree(sink);
+    if (e == cudaSuccess) e = cudaGetLastError();
+    *fma_per_s = best;
+    return e;
+}
+
+}  // namespace cosb

@@ -1,0 +1,43 @@
+// cos_kernels.cuh -- launch interface between the C-ABI (cos_capi.cu) and the kernels (cos_kernels.cu).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+namespace cosb {
+
+static const int TILE = 32;              // configurations per batch tile = one warp, lane = configuration
+
+struct LayerArgs {
+    const uint32_t* words;               // layer program (cos_compile.h)
+    const uint32_t* mask_off;            // [n_masks+1]
+    uint32_t n_masks, masks_per_cta;
+    const double* X;                     // source slab  [tile][S_src][32]
+    double* Y;                           // destination slab [tile][S_dst][32]
+    uint32_t S_src, S_dst;
+    const double* G;                     // caller's propagators [n_slots][batch]
+    long long batch, b0;                 // total batch (row stride of G / out) and first configuration of this chunk
+    double* out;                         // caller's output [n_out][batch]
+    int d, n_slots;                      // n_slots = n_blocks * d * d
+    double neg_kappa;                    // -kappa: -N_f (uniform) or -1 (SB)
+    double shift[4];                     // c3 * sigma_lambda of THIS layer (c3 = -2 at layer 0, -1 after)
+};
+
+// Picks the instantiation (max row length, colours, shift) and launches one layer step.
+// grid = (tiles, ceil(n_masks / masks_per_cta)); returns cudaGetLastError().
+cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
+                         cudaStream_t stream);
+// Opt-in to > 48 KB dynamic shared memory for every instantiation (once per process).
+cudaError_t configure_layer_kernels();
+size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift);
+
+cudaError_t launch_fill_ones(double* X, size_t n_doubles, cudaStream_t stream);
+
+struct TabArgs {
+    const double* T; int L, nsub, n_blocks, n_tau; double beta;
+    int n; const int* sites; const double* tau; long long batch; double* G;
+};
+cudaError_t launch_tabulate(const TabArgs& a, cudaStream_t stream);
+
+cudaError_t measure_fp64_fma(double* fma_per_s);
+
+}  // namespace cosb
