@@ -1,0 +1,363 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the CoS / SB-CoS hot path on B200 (contract: see DESIGN.md section 7).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg4] [--impl ours|reference]
+
+One "step" = one pass of the whole hot path over one batch of synthetic configurations:
+propagator tabulation (A2) -> layer propagation (A3) -> terminal readouts (A4); the DAG compile (A1)
+happens once, outside the timed region.  `value` = configurations / s with the inputs (vertex sites and
+times) resident in HBM; `e2e` = the same through cos_eval_host with HOST buffers (copies inside the timed
+region).  N > 1 (torchrun): configurations are independent, so every rank runs its own batch (seed + rank),
+no data-path collective ("weak" scaling); value = all ranks' configurations / max-over-ranks time.
+
+`--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded sample of the same
+workload -- the paper ships no code, so the oracle is the reference arm.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+from cos_workloads import draw_vertices, get_config  # noqa: E402
+from cos_workloads.tables import table_for  # noqa: E402
+
+METRIC = "connected_sum_configs_per_s"
+UNIT = "configs/s"
+DEFAULT_WORKLOAD = "cfg4"       # n = 10: the order BASELINE.json's target is quoted on
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD, help="cfg1..cfg5 (BASELINE.json configs, 1-based)")
+    ap.add_argument("--batch", type=int, default=0, help="override the configuration count (0 = BASELINE's)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--layers", action="store_true", help="print the per-layer table to stderr")
+    return ap.parse_args()
+
+
+def workload_of(args, rank=0):
+    w = get_config(int(args.workload.replace("cfg", "")))
+    kw = {"seed": w.seed + 1000 * rank}
+    if args.batch:
+        kw["batch"] = args.batch
+    return w.scaled(**kw)
+
+
+def config_dict(w, n_gpus, extra=None):
+    c = {"workload": w.name, "n": w.n, "n_flavors": w.n_flavors, "lattice": "honeycomb" if w.lattice else "square",
+         "mode": "uniform" if w.alphas is None else "sb", "all_subsets": w.all_subsets, "batch_per_gpu": w.batch,
+         "global_batch": w.batch * n_gpus, "L": w.L, "beta": w.beta, "n_tau": w.n_tau, "seed": w.seed,
+         "parallelism": "batch-sharded x%d, no collective" % n_gpus}
+    if extra:
+        c.update(extra)
+    return c
+
+
+# ------------------------------------------------------------------------------------------ CPU oracle timing
+def _oracle_one(task):
+    """One configuration through the cheapest oracle tier that returns the workload's outputs."""
+    import oracle
+    G, n, n_sub, nf, sigmas, uniform, all_subsets = task
+    if uniform and n_sub == 1:
+        return oracle.o3_uniform(G[0], nf, 0.0, all_subsets)          # printed recurrence Eq. 8-15
+    if not uniform and n_sub == 1 and not all_subsets:
+        return oracle.o2b_polynomial(G, sigmas)[-1:]                  # polynomial route Eq. 34-38
+    tier = "o2a" if nf == 2 else "o2b"
+    return oracle.connected_reference(G, n, n_sub, nf, sigmas, uniform, all_subsets, tier=tier)
+
+
+def oracle_tier_name(w):
+    if w.alphas is None and w.n_sub == 1:
+        return "O3 uniform rooted recurrence (Eq. 8-15)"
+    if w.alphas is not None and w.n_sub == 1 and not w.all_subsets:
+        return "O2b determinant-polynomial route (Eq. 34-38)"
+    return "sum over sublattice assignments of %s" % ("O2a' two-determinant CDet" if w.n_flavors == 2 else "O2b")
+
+
+def time_oracle(w, n_sample, procs):
+    """Times the oracle as it stands on `n_sample` configurations of workload `w`, `procs` processes.
+    Returns (configs/s, seconds)."""
+    import multiprocessing as mp
+    import oracle
+    oracle.build_oracle()
+    ws = w.scaled(batch=n_sample)
+    table = table_for(ws)
+    v = draw_vertices(ws)
+    G = oracle.tabulate_reference(table, v["sites"], v["tau"])
+    tasks = [(np.ascontiguousarray(G[..., c]), w.n, w.n_sub, w.n_flavors, w.sigmas, w.alphas is None, w.all_subsets)
+             for c in range(n_sample)]
+    t0 = time.perf_counter()
+    if procs > 1:
+        with mp.get_context("fork").Pool(procs) as pool:
+            pool.map(_oracle_one, tasks, chunksize=1)
+    else:
+        for t in tasks:
+            _oracle_one(t)
+    dt = time.perf_counter() - t0
+    return n_sample / dt, dt
+
+
+ORACLE_SECONDS_PER_CONFIG = {"cfg1": 2e-4, "cfg2": 0.12, "cfg3": 4.0, "cfg4": 3.0, "cfg5": 16.0}   # rough, one core
+
+
+def oracle_sample_plan(args, target_core_seconds=20.0):
+    cores = os.cpu_count() or 1
+    procs = max(1, min(cores, 16))
+    per = ORACLE_SECONDS_PER_CONFIG.get(args.workload, 1.0)
+    n = int(max(procs, min(4096, target_core_seconds * procs / per / 4)))
+    n = max(procs, (n // procs) * procs)
+    if per * n / procs > 60:
+        n = procs
+    return n, procs
+
+
+# ------------------------------------------------------------------------------------------ clocks sampling
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.lines, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[3:7]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------ reference arm
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = workload_of(args)
+    n_sample, procs = oracle_sample_plan(args, target_core_seconds=8.0)
+    rates = []
+    for _ in range(args.warmup):
+        time_oracle(w, procs, procs)
+    t_total = 0.0
+    for _ in range(args.steps):
+        r, dt = time_oracle(w, n_sample, procs)
+        rates.append(r); t_total += dt
+    value = n_sample * args.steps / t_total
+    sample = "%d configurations of %s per step, %s, %d processes" % (n_sample, w.name, oracle_tier_name(w), procs)
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * t_total / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": config_dict(w, 1, {"sample_per_step": n_sample}),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": procs, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ------------------------------------------------------------------------------------------ our arm
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_2507_12349_b200 as cos
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    cos.load_library()
+
+    w = workload_of(args, rank)
+    B = w.batch
+    table = table_for(w)
+    v = draw_vertices(w)
+    tab = cos.cos_tab_build(w.lattice, w.L, table.n_blocks, w.beta, w.n_tau, table.data)
+    t0 = time.perf_counter()
+    h = cos.cos_build(w.n, w.n_flavors, w.lattice, w.sigmas, w.n if w.all_subsets else 0)
+    build_s = time.perf_counter() - t0
+    info = cos.dag_summary(h)
+    NL = info["n_layers"]
+    n_slots = info["n_blocks"] * info["d"] ** 2
+
+    sites_h = torch.from_numpy(v["sites"]).pin_memory()
+    tau_h = torch.from_numpy(v["tau"]).pin_memory()
+    out_h = torch.empty((w.n_out, B), dtype=torch.float64).pin_memory()
+    sites = sites_h.to(dev)
+    tau = tau_h.to(dev)
+    G = torch.empty((n_slots, B), dtype=torch.float64, device=dev)
+    out = torch.empty((w.n_out, B), dtype=torch.float64, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        cos.cos_tabulate(tab, w.n, sites, tau, B, G, stream)
+        cos.cos_eval(h, G, B, out, stream)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+
+    # ---- timed region 1: device-resident inputs, per-layer CUDA events recorded inside cos_eval
+    cos.cos_set_profiling(h, True)
+    cos.cos_get_layer_times(h)                      # clear
+    launches0 = cos.cos_info(h, "n_launches")
+    sampler = ClockSampler(local_rank)
+    if rank == 0:
+        sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    barrier()
+    ms_total = ev0.elapsed_time(ev1)
+    clocks = sampler.stop() if rank == 0 else None
+    layer_ms, n_prof = cos.cos_get_layer_times(h)
+    cos.cos_set_profiling(h, False)
+    launches = cos.cos_info(h, "n_launches") - launches0 + args.steps      # + one tabulation launch per step
+
+    # ---- timed region 2: end to end through the C-ABI with host buffers
+    for _ in range(2):
+        cos.cos_eval_host(h, tab, sites_h, tau_h, B, out_h, stream)
+    barrier()
+    ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev2.record(stream)
+    for _ in range(args.steps):
+        cos.cos_eval_host(h, tab, sites_h, tau_h, B, out_h, stream)
+    ev3.record(stream)
+    barrier()
+    ms_e2e = ev2.elapsed_time(ev3)
+    assert torch.equal(out_h, out.cpu()), "host-buffer pipeline and device pipeline disagree"
+    assert bool(torch.isfinite(out_h).all())
+
+    if world > 1:
+        t = torch.tensor([ms_total, ms_e2e, sum(layer_ms)], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total, ms_e2e, layer_sum = [float(x) for x in t.tolist()]
+    else:
+        layer_sum = sum(layer_ms)
+
+    if rank == 0:
+        K = args.steps
+        value = world * B * K / (ms_total * 1e-3)
+        e2e_value = world * B * K / (ms_e2e * 1e-3)
+        edges = info["n_edges"] + info["n_readout_edges"]
+        # ---- roofline of the dominant kernel (cos_layer_kernel, NL launches per step); DESIGN.md section 6
+        S = info["n_states"]
+        alg_bytes_step = (16 * S + 8 * n_slots + 8 * w.n_out) * B + info["program_bytes"]
+        layer_s_step = layer_sum * 1e-3 / max(n_prof, 1)
+        try:
+            peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+            peak_gbs, peak_src = float(peaks["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
+        except (OSError, KeyError, ValueError):
+            peak_gbs, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
+        achieved_gbs = alg_bytes_step / layer_s_step / 1e9
+        fma_peak = cos.cos_measure_fp64_fma_peak()
+        t_hbm = alg_bytes_step / (peak_gbs * 1e9)
+        t_fp64 = info["n_fma"] * B / fma_peak
+        roofline = {"bound": "hbm" if t_hbm >= t_fp64 else "alu", "kernel": "cos_layer_kernel",
+                    "achieved": achieved_gbs, "peak": peak_gbs, "unit": "GB/s", "frac": achieved_gbs / peak_gbs,
+                    "traffic": None, "peak_source": peak_src,
+                    "launches_per_step": NL, "kernel_ms_per_step": layer_s_step * 1e3,
+                    "kernel_share_of_step": layer_s_step * 1e3 / (ms_total / K),
+                    "algorithmic_bytes_per_step": alg_bytes_step,
+                    "t_roofline_hbm_ms": t_hbm * 1e3, "t_roofline_fp64_ms": t_fp64 * 1e3,
+                    "fp64_fma_peak_measured_tflops": 2 * fma_peak / 1e12,
+                    "fp64_fma_achieved_tflops": 2 * info["n_fma"] * B / layer_s_step / 1e12}
+        line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
+                "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "dtype": "f64", "data": "synthetic",
+                "config": config_dict(w, world, {"l2": "inputs larger than L2: the two layer slabs hold %.1f GB per step"
+                                                 % (16 * info["max_layer_states"] * B / 1e9),
+                                                 "dag": {k: info[k] for k in ("n_states", "n_edges", "n_readout_edges",
+                                                                               "n_fma", "max_layer_states", "program_bytes")},
+                                                 "build_s": build_s}),
+                "edge_evals_per_s": world * edges * B * K / (ms_total * 1e-3),
+                "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K,
+                        "h2d_bytes_per_step": B * w.n * (2 * 4 + 8), "d2h_bytes_per_step": B * w.n_out * 8},
+                "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
+        if not args.no_cpu_baseline and world == 1:
+            n_sample, procs = oracle_sample_plan(args)
+            rate, dt = time_oracle(workload_of(args), n_sample, procs)
+            line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": procs, "kind": "oracle", "seconds": dt,
+                                    "sample": "%d configurations of %s, %s" % (n_sample, w.name, oracle_tier_name(w))}
+        if args.layers:
+            sys.stderr.write("layer  states      ms/step   GB/s(alg)\n")
+            for l in range(NL):
+                s_in = info["layer_states"][l]
+                s_out = info["layer_states"][l + 1] if l + 1 < NL else 0
+                ms = layer_ms[l] / max(n_prof, 1)
+                gb = 8.0 * (s_in + s_out) * B / 1e9
+                sys.stderr.write("%3d %10d %10.4f %10.1f\n" % (l, s_in, ms, gb / (ms * 1e-3) if ms > 0 else 0.0))
+        print(json.dumps(line), flush=True)
+
+    cos.cos_free(h)
+    cos.cos_tab_free(tab)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -96,6 +96,7 @@ enum {
     COS_INFO_N_BLOCKS = 11,       /* propagator blocks expected in G_dev */
     COS_INFO_N_STATES_UNPRUNED = 12,
     COS_INFO_WORKSPACE_BYTES = 13,
+    COS_INFO_N_LAUNCHES = 14,     /* kernels launched through this handle so far (cos_eval / cos_eval_host) */
     COS_INFO_LAYER_STATES = 100,  /* + layer index */
     COS_INFO_LAYER_EDGES = 200,   /* + layer index: edges leaving that layer (readout edges included) */
     COS_INFO_LAYER_MASKS = 300    /* + layer index */
@@ -121,7 +122,25 @@ int cos_tabulate(cos_tab tab, int n, const int* sites_dev, const double* tau_dev
                  double* G_dev, cos_stream stream);
 void cos_tab_free(cos_tab tab);
 
-/* ---- measurement helper: fp64 FMA peak of the device (independent FMA chains, no memory traffic).
+/* ---- host-buffer pipeline: tabulate (2) + evaluate (3)+(4) for configurations that live in HOST memory.
+ *   sites_host  host int32 [n][2][batch], tau_host host fp64 [n][batch] (layouts of cos_tabulate; pinned memory
+ *               makes the copies asynchronous, pageable memory works too), out_host host fp64 [n_out][batch].
+ * Copies the inputs to a device staging area owned by the handle (grown lazily), runs cos_tabulate and cos_eval on
+ * `stream`, copies the result back and SYNCHRONISES the stream before returning.  n is the handle's order; the table
+ * must have the handle's number of propagator blocks and lattice.  Bytes moved per call:
+ * H2D batch*n*(2*4+8), D2H batch*n_out*8. */
+int cos_eval_host(cos_handle h, cos_tab tab, const int* sites_host, const double* tau_host, long long batch,
+                  double* out_host, cos_stream stream);
+
+/* ---- measurement helpers ------------------------------------------------------------------------------
+ * cos_set_profiling(h, 1): every later cos_eval brackets each layer launch with CUDA events on its stream.
+ * cos_get_layer_times synchronises on the recorded events, ADDS the elapsed milliseconds of layer l (summed over
+ * batch chunks and over all cos_eval calls since the last cos_get_layer_times) to ms[l] for l < n_layers, stores
+ * the number of profiled cos_eval calls in *n_evals, and clears the record.  ms is host memory, caller-zeroed. */
+int cos_set_profiling(cos_handle h, int on);
+int cos_get_layer_times(cos_handle h, int n_layers, double* ms, long long* n_evals);
+
+/* fp64 FMA peak of the device (independent FMA chains, no memory traffic).
  * Returns achieved FMA/s in *fma_per_s (synchronous; used by bench.py for the fp64 roofline leg). */
 int cos_measure_fp64_fma_peak(double* fma_per_s);
 

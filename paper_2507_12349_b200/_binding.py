@@ -18,13 +18,14 @@ COS_BUILD_HOST_ONLY = 1
 INFO = {
     "n_layers": 0, "n_states": 1, "n_edges": 2, "n_readout_edges": 3, "n_out": 4, "max_layer_states": 5,
     "n_masks": 6, "n_rows": 7, "n_fma": 8, "program_bytes": 9, "d": 10, "n_blocks": 11,
-    "n_states_unpruned": 12, "workspace_bytes": 13,
+    "n_states_unpruned": 12, "workspace_bytes": 13, "n_launches": 14,
     "layer_states": 100, "layer_edges": 200, "layer_masks": 300,
 }
 
 EXPORTS = [
     "cos_build", "cos_build_ex", "cos_eval", "cos_free", "cos_set_workspace_limit", "cos_info",
     "cos_last_error", "cos_tab_build", "cos_tabulate", "cos_tab_free", "cos_measure_fp64_fma_peak",
+    "cos_eval_host", "cos_set_profiling", "cos_get_layer_times",
 ]
 
 
@@ -68,6 +69,12 @@ def load_library():
     lib.cos_tabulate.argtypes = [vp, ip, vp, vp, ctypes.c_longlong, vp, vp]
     lib.cos_tab_free.restype = None
     lib.cos_tab_free.argtypes = [vp]
+    lib.cos_eval_host.restype = ctypes.c_int
+    lib.cos_eval_host.argtypes = [vp, vp, vp, vp, ctypes.c_longlong, vp, vp]
+    lib.cos_set_profiling.restype = ctypes.c_int
+    lib.cos_set_profiling.argtypes = [vp, ip]
+    lib.cos_get_layer_times.restype = ctypes.c_int
+    lib.cos_get_layer_times.argtypes = [vp, ip, dp, llp]
     lib.cos_measure_fp64_fma_peak.restype = ctypes.c_int
     lib.cos_measure_fp64_fma_peak.argtypes = [dp]
     _lib = lib
@@ -154,6 +161,34 @@ def cos_tab_build(lattice, L, n_blocks, beta, n_tau, table_host):
 def cos_tabulate(tab, n, sites_dev, tau_dev, batch, G_dev, stream=None):
     _check(load_library().cos_tabulate(tab, int(n), _dev_ptr(sites_dev, "torch.int32"), _dev_ptr(tau_dev, "torch.float64"),
                                        int(batch), _dev_ptr(G_dev, "torch.float64"), _stream_ptr(stream)))
+
+
+def _host_ptr(t, dtype_name):
+    import torch
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.is_contiguous() and str(t.dtype) == dtype_name):
+        raise CosError(COS_EINVAL, "expected a contiguous host tensor of dtype %s" % dtype_name)
+    return t.data_ptr()
+
+
+def cos_eval_host(handle, tab, sites_host, tau_host, batch, out_host, stream=None):
+    """Host-buffer pipeline: sites_host int32 [n,2,batch], tau_host fp64 [n,batch], out_host fp64 [n_out,batch]
+    (torch CPU tensors, ideally pinned).  Synchronises the stream before returning."""
+    _check(load_library().cos_eval_host(handle, tab, _host_ptr(sites_host, "torch.int32"),
+                                        _host_ptr(tau_host, "torch.float64"), int(batch),
+                                        _host_ptr(out_host, "torch.float64"), _stream_ptr(stream)))
+
+
+def cos_set_profiling(handle, on):
+    _check(load_library().cos_set_profiling(handle, int(bool(on))))
+
+
+def cos_get_layer_times(handle):
+    """-> (list of per-layer milliseconds accumulated since the last call, number of profiled cos_eval calls)."""
+    nl = cos_info(handle, "n_layers")
+    ms = (ctypes.c_double * nl)()
+    n = ctypes.c_longlong(0)
+    _check(load_library().cos_get_layer_times(handle, nl, ms, ctypes.byref(n)))
+    return list(ms), n.value
 
 
 def cos_tab_free(tab):

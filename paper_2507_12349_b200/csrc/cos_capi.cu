@@ -45,6 +45,15 @@ struct cos_handle_s {
     long long ws_limit = 64ll << 30;
     int masks_per_cta = 64;
     int warps_per_cta = 8;
+    long long n_launches = 0;
+    // profiling (cos_set_profiling): events[k*(NL+1) + l] brackets layer l of the k-th profiled chunk
+    bool profiling = false;
+    std::vector<cudaEvent_t> events;
+    size_t events_used = 0;
+    long long profiled_evals = 0;
+    // staging of cos_eval_host
+    int* st_sites = nullptr; double* st_tau = nullptr; double* st_G = nullptr; double* st_out = nullptr;
+    long long st_batch = 0;
 };
 
 struct cos_tab_s {
@@ -131,6 +140,11 @@ void cos_free(cos_handle h)
     if (!h) return;
     for (auto& l : h->dl) { if (l.words) cudaFree(l.words); if (l.mask_off) cudaFree(l.mask_off); }
     if (h->ws) cudaFree(h->ws);
+    for (cudaEvent_t e : h->events) cudaEventDestroy(e);
+    if (h->st_sites) cudaFree(h->st_sites);
+    if (h->st_tau) cudaFree(h->st_tau);
+    if (h->st_G) cudaFree(h->st_G);
+    if (h->st_out) cudaFree(h->st_out);
     delete h;
 }
 
@@ -169,10 +183,25 @@ int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev
     }
     double* slab[2] = {h->ws, h->ws + (size_t)D.max_layer_states * TILE * (size_t)tiles_chunk};
 
+    if (h->profiling) ++h->profiled_evals;
     for (long long t0 = 0; t0 < tiles_total; t0 += tiles_chunk) {
         const uint32_t tiles = (uint32_t)((tiles_total - t0 < tiles_chunk) ? (tiles_total - t0) : tiles_chunk);
         cudaError_t e = launch_fill_ones(slab[0], (size_t)D.layers[0].n_states * TILE * tiles, stream);
         if (e != cudaSuccess) return cuda_fail(e, "cos_eval: fill launch");
+        ++h->n_launches;
+        cudaEvent_t* ev = nullptr;
+        if (h->profiling) {
+            const size_t need_ev = h->events_used + (size_t)NL + 1;
+            while (h->events.size() < need_ev) {
+                cudaEvent_t x;
+                e = cudaEventCreate(&x);
+                if (e != cudaSuccess) return cuda_fail(e, "cos_eval: cudaEventCreate");
+                h->events.push_back(x);
+            }
+            ev = h->events.data() + h->events_used;
+            h->events_used = need_ev;
+            cudaEventRecord(ev[0], stream);
+        }
         for (int l = 0; l < NL; ++l) {
             const LayerProgram& P = D.layers[l];
             LayerArgs a;
@@ -186,8 +215,80 @@ int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev
             for (int c = 0; c < 4; ++c) a.shift[c] = (l == 0 ? -2.0 : -1.0) * D.sigma[c];
             e = launch_layer(a, (int)D.max_L, D.nc, D.has_shift, tiles, h->warps_per_cta, stream);
             if (e != cudaSuccess) return cuda_fail(e, "cos_eval: layer launch");
+            if (P.n_masks) ++h->n_launches;
+            if (ev) cudaEventRecord(ev[l + 1], stream);
         }
     }
+    return COS_OK;
+}
+
+int cos_set_profiling(cos_handle h, int on)
+{
+    if (!h) return fail(COS_EINVAL, "cos_set_profiling: handle is NULL");
+    h->profiling = on != 0;
+    return COS_OK;
+}
+
+int cos_get_layer_times(cos_handle h, int n_layers, double* ms, long long* n_evals)
+{
+    if (!h || !ms || n_layers < 0) return fail(COS_EINVAL, "cos_get_layer_times: bad argument");
+    const int NL = (int)h->dag.layers.size();
+    const size_t per = (size_t)NL + 1;
+    for (size_t k = 0; k + per <= h->events_used; k += per) {
+        cudaError_t e = cudaEventSynchronize(h->events[k + NL]);
+        if (e != cudaSuccess) return cuda_fail(e, "cos_get_layer_times: cudaEventSynchronize");
+        for (int l = 0; l < NL && l < n_layers; ++l) {
+            float t = 0.f;
+            e = cudaEventElapsedTime(&t, h->events[k + l], h->events[k + l + 1]);
+            if (e != cudaSuccess) return cuda_fail(e, "cos_get_layer_times: cudaEventElapsedTime");
+            ms[l] += (double)t;
+        }
+    }
+    if (n_evals) *n_evals = h->profiled_evals;
+    h->events_used = 0;
+    h->profiled_evals = 0;
+    return COS_OK;
+}
+
+int cos_eval_host(cos_handle h, cos_tab tab, const int* sites_host, const double* tau_host, long long batch,
+                  double* out_host, cos_stream stream_)
+{
+    if (!h || !tab) return fail(COS_EINVAL, "cos_eval_host: NULL handle");
+    if (batch < 0) return fail(COS_EINVAL, "cos_eval_host: negative batch");
+    if (batch == 0) return COS_OK;
+    if (!sites_host || !tau_host || !out_host) return fail(COS_EINVAL, "cos_eval_host: NULL host pointer");
+    if (!h->on_device) return fail(COS_ECUDA, "cos_eval_host: handle was built host-only (no CPU fallback)");
+    const CompiledDag& D = h->dag;
+    if (tab->n_blocks != D.n_blocks || tab->nsub != D.nsub)
+        return fail(COS_EINVAL, "cos_eval_host: table blocks / lattice do not match the handle");
+    cudaStream_t stream = (cudaStream_t)stream_;
+    const size_t B = (size_t)batch, n = (size_t)D.n;
+    const size_t b_sites = n * 2 * B * sizeof(int), b_tau = n * B * sizeof(double);
+    const size_t b_G = (size_t)D.n_blocks * D.d * D.d * B * sizeof(double), b_out = (size_t)D.n_out * B * sizeof(double);
+    if (batch > h->st_batch) {
+        if (h->st_sites) cudaFree(h->st_sites);
+        if (h->st_tau) cudaFree(h->st_tau);
+        if (h->st_G) cudaFree(h->st_G);
+        if (h->st_out) cudaFree(h->st_out);
+        h->st_sites = nullptr; h->st_tau = nullptr; h->st_G = nullptr; h->st_out = nullptr; h->st_batch = 0;
+        cudaError_t e = cudaMalloc(&h->st_sites, b_sites);
+        if (e == cudaSuccess) e = cudaMalloc(&h->st_tau, b_tau);
+        if (e == cudaSuccess) e = cudaMalloc(&h->st_G, b_G);
+        if (e == cudaSuccess) e = cudaMalloc(&h->st_out, b_out);
+        if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, "cos_eval_host: staging allocation"); }
+        h->st_batch = batch;
+    }
+    cudaError_t e = cudaMemcpyAsync(h->st_sites, sites_host, b_sites, cudaMemcpyHostToDevice, stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(h->st_tau, tau_host, b_tau, cudaMemcpyHostToDevice, stream);
+    if (e != cudaSuccess) return cuda_fail(e, "cos_eval_host: host-to-device copy");
+    int rc = cos_tabulate(tab, D.n, h->st_sites, h->st_tau, batch, h->st_G, stream_);
+    if (rc != COS_OK) return rc;
+    ++h->n_launches;
+    rc = cos_eval(h, h->st_G, batch, h->st_out, stream_);
+    if (rc != COS_OK) return rc;
+    e = cudaMemcpyAsync(out_host, h->st_out, b_out, cudaMemcpyDeviceToHost, stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+    if (e != cudaSuccess) return cuda_fail(e, "cos_eval_host: device-to-host copy");
     return COS_OK;
 }
 
@@ -217,6 +318,7 @@ int cos_info(cos_handle h, int what, long long* value)
         case COS_INFO_N_BLOCKS: *value = D.n_blocks; break;
         case COS_INFO_N_STATES_UNPRUNED: *value = (long long)D.n_states_unpruned; break;
         case COS_INFO_WORKSPACE_BYTES: *value = (long long)h->ws_bytes; break;
+        case COS_INFO_N_LAUNCHES: *value = h->n_launches; break;
         default: return fail(COS_EINVAL, "cos_info: unknown query");
     }
     return COS_OK;
