@@ -110,7 +110,7 @@ def time_oracle(w, n_sample, procs):
     return n_sample / dt, dt
 
 
-ORACLE_SECONDS_PER_CONFIG = {"cfg1": 2e-4, "cfg2": 0.12, "cfg3": 4.0, "cfg4": 3.0, "cfg5": 16.0}   # rough, one core
+ORACLE_SECONDS_PER_CONFIG = {"cfg1": 2e-4, "cfg2": 0.12, "cfg3": 16.0, "cfg4": 12.0, "cfg5": 16.0}   # rough, one core
 
 
 def oracle_sample_plan(args, target_core_seconds=20.0):

@@ -12,8 +12,8 @@
  *       by union-find over fermion edges plus interaction lines, explicit shift one-cycles,
  *       colour sums (Eq. 58-63; uniform: PAPER.md:45, 431).
  *   O2a two-spin determinant route + CDet subset recursion (Eq. 49-50,
- *       446-450 Eq. 53), long double.
- *   O2b flavour-polynomial route, Eq. 34-38, long double.
+ *       446-450 Eq. 53), __float128 (the paper needs double-double there).
+ *   O2b flavour-polynomial route, Eq. 34-38, __float128.
  *   O3  the recurrences as printed: Algorithm 3 (canonical key Eq. 79-80)
  *       and the uniform rooted recurrence with all-subset readouts (Eq. 8-15).
  *
@@ -167,35 +167,77 @@ double cos_o1_connected(int n, int nf, int sb, const double *A, const double *si
 }
 
 /* ------------------------------------------------------------------------------------------
- * O2: determinant routes (long double; the paper uses double-double there).
+ * O2: determinant routes.  Arithmetic type: __float128 (IEEE binary128, eps = 2^-113, gcc soft
+ * float).  The paper itself needs double-double for the determinant recursion: the
+ * subset recursion Eq. 53 / Eq. 38 subtracts products of disconnected parts whose magnitude
+ * c~(V) ~ (|V|-1)! prod_i a({i}) exceeds the connected value by > 10 orders at n = 10 on the
+ * benchmark inputs (|C| ~ 1e-15, c~ ~ 1e6), so x87 long double (eps = 5e-20) is NOT enough there.
+ *
+ * `absolute` != 0 replaces every determinant by the PERMANENT of the element-wise absolute matrix
+ * and sigma by |sigma| (same recursion): the sum of |weight| over the connected contractions this
+ * route enumerates, i.e. those in which the two endpoints of a vertex lie in cycles of DIFFERENT
+ * colour (Eq. 35 has no same-colour entry: those terms cancel identically in the signed sum,
+ * PAPER.md:291-296).  It is therefore a LOWER bound of the full cancellation scale M of O1 / O3
+ * with absolute = 1 (which also counts same-colour terms), used as a stricter acceptance scale
+ * where O1 / O3 are too slow.
  * ---------------------------------------------------------------------------------------- */
+typedef __float128 xreal;
+static xreal xabs(xreal x) { return x < 0 ? -x : x; }
 
 /* det of the principal submatrix A[T,T] + diag_add * 1, Gaussian elimination, partial pivoting */
-static long double ld_minor(int n, const double *A, uint32_t T, double diag_add)
+static xreal x_minor(int n, const double *A, uint32_t T, double diag_add)
 {
-    long double M[MAXN][MAXN];
+    xreal M[MAXN][MAXN];
     int idx[MAXN], k = 0, i, j, p;
     for (i = 0; i < n; ++i) if (T >> i & 1) idx[k++] = i;
-    if (k == 0) return 1.0L;
+    if (k == 0) return 1;
     for (i = 0; i < k; ++i)
         for (j = 0; j < k; ++j)
-            M[i][j] = (long double)A[idx[i] * n + idx[j]] + (i == j ? (long double)diag_add : 0.0L);
-    long double det = 1.0L;
+            M[i][j] = (xreal)A[idx[i] * n + idx[j]] + (i == j ? (xreal)diag_add : (xreal)0);
+    xreal det = 1;
     for (p = 0; p < k; ++p) {
         int piv = p;
-        for (i = p + 1; i < k; ++i) if (fabsl(M[i][p]) > fabsl(M[piv][p])) piv = i;
-        if (M[piv][p] == 0.0L) return 0.0L;
+        for (i = p + 1; i < k; ++i) if (xabs(M[i][p]) > xabs(M[piv][p])) piv = i;
+        if (M[piv][p] == 0) return 0;
         if (piv != p) {
-            for (j = 0; j < k; ++j) { long double t = M[p][j]; M[p][j] = M[piv][j]; M[piv][j] = t; }
+            for (j = 0; j < k; ++j) { xreal t = M[p][j]; M[p][j] = M[piv][j]; M[piv][j] = t; }
             det = -det;
         }
         det *= M[p][p];
         for (i = p + 1; i < k; ++i) {
-            long double f = M[i][p] / M[p][p];
+            xreal f = M[i][p] / M[p][p];
             for (j = p; j < k; ++j) M[i][j] -= f * M[p][j];
         }
     }
     return det;
+}
+
+/* permanent of |A[T,T]| + |diag_add| * 1 by its definition, expanded row by row over the set of
+ * columns already used:  P_r[cols] = sum_{j in cols} |M[r][j]| * P_{r-1}[cols \ j]  (k 2^k terms). */
+static xreal x_perm_abs(int n, const double *A, uint32_t T, double diag_add)
+{
+    int idx[MAXN], k = 0, i, j;
+    for (i = 0; i < n; ++i) if (T >> i & 1) idx[k++] = i;
+    if (k == 0) return 1;
+    static __thread xreal P[1u << MAXN];          /* binary128: the subset recursion cancels as hard as for det */
+    uint32_t cols, fullc = 1u << k;
+    P[0] = 1;
+    for (cols = 1; cols < fullc; ++cols) {
+        int r = __builtin_popcount(cols) - 1;         /* rows 0..r are matched with the columns in cols */
+        xreal acc = 0;
+        for (j = 0; j < k; ++j)
+            if (cols >> j & 1) {
+                xreal m = (xreal)fabs(A[idx[r] * n + idx[j]]) + (r == j ? (xreal)fabs(diag_add) : (xreal)0);
+                acc += m * P[cols ^ (1u << j)];
+            }
+        P[cols] = acc;
+    }
+    return P[fullc - 1];
+}
+
+static xreal x_minor_or_perm(int n, const double *A, uint32_t T, double diag_add, int absolute)
+{
+    return absolute ? x_perm_abs(n, A, T, diag_add) : x_minor(n, A, T, diag_add);
 }
 
 static int popc(uint32_t x) { return __builtin_popcount(x); }
@@ -203,17 +245,17 @@ static int popc(uint32_t x) { return __builtin_popcount(x); }
 /* CDet recursion Eq. 53 / Eq. 38: c(V) = a(V) - sum over PROPER subsets
  * S of V containing min V of c(S) a(V \ S); a(empty) = 1; increasing subset size.
  * a, c are arrays over bitmasks [2^n]; c[0] unused.                                              */
-static void cdet_recursion(int n, const long double *a, long double *c)
+static void cdet_recursion(int n, const xreal *a, xreal *c)
 {
     uint32_t full = (1u << n), V;
     int size;
-    c[0] = 0.0L;
+    c[0] = 0;
     for (size = 1; size <= n; ++size)
         for (V = 1; V < full; ++V) {
             if (popc(V) != size) continue;
             uint32_t anchor = V & (~V + 1u);          /* lowest set bit = min V */
             uint32_t rest = V ^ anchor, sub;
-            long double acc = a[V];
+            xreal acc = a[V];
             /* S = anchor | sub, sub a PROPER subset of rest (so that S != V) */
             for (sub = (rest - 1) & rest; ; sub = (sub - 1) & rest) {
                 if (rest == 0) break;
@@ -231,20 +273,22 @@ static void cdet_recursion(int n, const long double *a, long double *c)
  *   a(T) = 2^{|T|} det(A_up[T] + sig_dn 1) det(A_dn[T] + sig_up 1),   c by Eq. 53,
  * and the scalar term of Eq. 50 is removed from singletons: C({i}) = c({i}) - 2 sig_up sig_dn.
  * out[T-1] = C(T) for every nonempty T (bit i <-> vertex i).                                     */
-int cos_o2a_twospin(int n, const double *A_up, const double *A_dn, double sig_up, double sig_dn, double *out)
+int cos_o2a_twospin(int n, const double *A_up, const double *A_dn, double sig_up, double sig_dn, int absolute,
+                    double *out)
 {
     if (n < 1 || n > MAXN) return 1;
     uint32_t full = 1u << n, T;
-    long double *a = (long double *)malloc(sizeof(long double) * full);
-    long double *c = (long double *)malloc(sizeof(long double) * full);
+    xreal *a = (xreal *)malloc(sizeof(xreal) * full);
+    xreal *c = (xreal *)malloc(sizeof(xreal) * full);
     if (!a || !c) { free(a); free(c); return 2; }
-    a[0] = 1.0L;
+    a[0] = 1;
     for (T = 1; T < full; ++T)
-        a[T] = ldexpl(1.0L, popc(T)) * ld_minor(n, A_up, T, sig_dn) * ld_minor(n, A_dn, T, sig_up);
+        a[T] = (xreal)(double)(1u << popc(T)) * x_minor_or_perm(n, A_up, T, sig_dn, absolute) *
+               x_minor_or_perm(n, A_dn, T, sig_up, absolute);
     cdet_recursion(n, a, c);
     for (T = 1; T < full; ++T) {
-        long double v = c[T];
-        if (popc(T) == 1) v -= 2.0L * (long double)sig_up * (long double)sig_dn;
+        xreal v = c[T];
+        if (popc(T) == 1) v -= (xreal)2 * (xreal)absd(sig_up, absolute) * (xreal)absd(sig_dn, absolute);
         out[T - 1] = (double)v;
     }
     free(a); free(c);
@@ -258,19 +302,19 @@ int cos_o2a_twospin(int n, const double *A_up, const double *A_dn, double sig_up
  *   H(T)   = sum over local choices of prod_a d_a(S_a) prod_i L_i   (Eq. 36)
  *   C(T)   = H(T) - sum_{S proper, min T in S} C(S) H(T \ S)         (Eq. 38)                    */
 typedef struct {
-    int n, nf;
-    const long double *d;     /* [nf][2^n] */
+    int n, nf, absolute;
+    const xreal *d;           /* [nf][2^n] */
     const double *sigma;      /* [nf] or NULL (all zero) */
     uint32_t T;
     uint32_t S[MAXF];
-    long double acc;
+    xreal acc;
 } o2b_ctx;
 
-static void o2b_rec(o2b_ctx *c, int site, long double w)
+static void o2b_rec(o2b_ctx *c, int site, xreal w)
 {
     while (site < c->n && !(c->T >> site & 1)) ++site;
     if (site == c->n) {
-        int a; long double p = w;
+        int a; xreal p = w;
         for (a = 0; a < c->nf; ++a) p *= c->d[((size_t)a << c->n) + c->S[a]];
         c->acc += p;
         return;
@@ -280,36 +324,37 @@ static void o2b_rec(o2b_ctx *c, int site, long double w)
     for (a = 0; a < c->nf; ++a) {
         if (c->sigma && c->sigma[a] != 0.0) {         /* one flavour: 2 sigma_a */
             c->S[a] |= bit;
-            o2b_rec(c, site + 1, w * 2.0L * (long double)c->sigma[a]);
+            o2b_rec(c, site + 1, w * (xreal)2 * (xreal)absd(c->sigma[a], c->absolute));
             c->S[a] &= ~bit;
         }
         for (b = a + 1; b < c->nf; ++b) {             /* two flavours a<b: 2 */
             c->S[a] |= bit; c->S[b] |= bit;
-            o2b_rec(c, site + 1, w * 2.0L);
+            o2b_rec(c, site + 1, w * (xreal)2);
             c->S[a] &= ~bit; c->S[b] &= ~bit;
         }
     }
 }
 
-int cos_o2b_polynomial(int n, int nf, const double *A /*[nf][n][n]*/, const double *sigma, double *out)
+int cos_o2b_polynomial(int n, int nf, const double *A /*[nf][n][n]*/, const double *sigma, int absolute, double *out)
 {
     if (n < 1 || n > MAXN || nf < 2 || nf > MAXF) return 1;
     uint32_t full = 1u << n, T;
-    long double *d = (long double *)malloc(sizeof(long double) * full * nf);
-    long double *H = (long double *)malloc(sizeof(long double) * full);
-    long double *C = (long double *)malloc(sizeof(long double) * full);
+    xreal *d = (xreal *)malloc(sizeof(xreal) * full * nf);
+    xreal *H = (xreal *)malloc(sizeof(xreal) * full);
+    xreal *C = (xreal *)malloc(sizeof(xreal) * full);
     if (!d || !H || !C) { free(d); free(H); free(C); return 2; }
     int a;
     for (a = 0; a < nf; ++a)
-        for (T = 0; T < full; ++T) d[((size_t)a << n) + T] = ld_minor(n, A + (size_t)a * n * n, T, 0.0);
+        for (T = 0; T < full; ++T)
+            d[((size_t)a << n) + T] = x_minor_or_perm(n, A + (size_t)a * n * n, T, 0.0, absolute);
     o2b_ctx c;
     memset(&c, 0, sizeof c);
-    c.n = n; c.nf = nf; c.d = d; c.sigma = sigma;
-    H[0] = 1.0L;
+    c.n = n; c.nf = nf; c.d = d; c.sigma = sigma; c.absolute = absolute;
+    H[0] = 1;
     for (T = 1; T < full; ++T) {
-        c.T = T; c.acc = 0.0L;
+        c.T = T; c.acc = 0;
         memset(c.S, 0, sizeof c.S);
-        o2b_rec(&c, 0, 1.0L);
+        o2b_rec(&c, 0, 1);
         H[T] = c.acc;
     }
     cdet_recursion(n, H, C);

@@ -37,9 +37,9 @@ def _load():
         lib.cos_o1_connected.restype = ctypes.c_double
         lib.cos_o1_connected.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _dp, _dp, ctypes.c_int]
         lib.cos_o2a_twospin.restype = ctypes.c_int
-        lib.cos_o2a_twospin.argtypes = [ctypes.c_int, _dp, _dp, ctypes.c_double, ctypes.c_double, _dp]
+        lib.cos_o2a_twospin.argtypes = [ctypes.c_int, _dp, _dp, ctypes.c_double, ctypes.c_double, ctypes.c_int, _dp]
         lib.cos_o2b_polynomial.restype = ctypes.c_int
-        lib.cos_o2b_polynomial.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _dp, _dp]
+        lib.cos_o2b_polynomial.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _dp, ctypes.c_int, _dp]
         lib.cos_o3_alg3.restype = ctypes.c_double
         lib.cos_o3_alg3.argtypes = [ctypes.c_int, ctypes.c_int, _dp, _dp, ctypes.c_int, _llp, _llp]
         lib.cos_o3_uniform.restype = ctypes.c_int
@@ -71,24 +71,26 @@ def o1_connected(A, n_flavors, sigma=None, sb=True, absolute=False):
     return _load().cos_o1_connected(n, n_flavors, int(sb), pA, ps, int(absolute))
 
 
-def o2a_twospin(A_up, A_dn, sig_up=0.0, sig_dn=0.0):
-    """Two-spin determinants + CDet (Eq. 49-50, 53): all 2^n - 1 connected values."""
+def o2a_twospin(A_up, A_dn, sig_up=0.0, sig_dn=0.0, absolute=False):
+    """Two-spin determinants + CDet (Eq. 49-50, 53): all 2^n - 1 connected values (binary128 inside).
+    absolute=True: permanents of |A|, |sigma| -- a LOWER bound of the cancellation scale M (C file, O2 header)."""
     A_up, pu = _c(A_up)
     A_dn, pd = _c(A_dn)
     n = A_up.shape[0]
     out = np.zeros((1 << n) - 1)
-    rc = _load().cos_o2a_twospin(n, pu, pd, float(sig_up), float(sig_dn), out.ctypes.data_as(_dp))
+    rc = _load().cos_o2a_twospin(n, pu, pd, float(sig_up), float(sig_dn), int(absolute), out.ctypes.data_as(_dp))
     assert rc == 0
     return out
 
 
-def o2b_polynomial(A, sigma=None):
-    """Flavour-polynomial route Eq. 34-38 on A[N_f][n][n]: all 2^n - 1 connected values."""
+def o2b_polynomial(A, sigma=None, absolute=False):
+    """Flavour-polynomial route Eq. 34-38 on A[N_f][n][n]: all 2^n - 1 connected values (binary128 inside).
+    absolute=True: permanents of |A|, |sigma| -- a LOWER bound of the cancellation scale M (C file, O2 header)."""
     A, pA = _c(A)
     nf, n, _ = A.shape
     s, ps = _sig(sigma)
     out = np.zeros((1 << n) - 1)
-    rc = _load().cos_o2b_polynomial(n, nf, pA, ps, out.ctypes.data_as(_dp))
+    rc = _load().cos_o2b_polynomial(n, nf, pA, ps, int(absolute), out.ctypes.data_as(_dp))
     assert rc == 0
     return out
 
@@ -160,16 +162,16 @@ def connected_reference(G, n, n_sub, n_flavors, sigmas=None, uniform=True, all_s
                 else:
                     acc += o3_alg3(A, sigmas, absolute)
             elif tier == "o2a":
-                assert n_flavors == 2 and not absolute
+                assert n_flavors == 2
                 if uniform:
                     assert sigmas is None
-                    acc += o2a_twospin(A[0], A[0])[-1]
+                    acc += o2a_twospin(A[0], A[0], absolute=absolute)[-1]
                 else:
                     sg = (0.0, 0.0) if sigmas is None else sigmas
-                    acc += o2a_twospin(A[0], A[1], sg[0], sg[1])[-1]
+                    acc += o2a_twospin(A[0], A[1], sg[0], sg[1], absolute=absolute)[-1]
             elif tier == "o2b":
-                assert not uniform and not absolute
-                acc += o2b_polynomial(A, sigmas)[-1]
+                assert not uniform
+                acc += o2b_polynomial(A, sigmas, absolute=absolute)[-1]
             else:
                 raise ValueError(tier)
         out[k] = acc

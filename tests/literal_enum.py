@@ -46,8 +46,10 @@ def _cycles(p):
     return out
 
 
-def typed_connected_sum(A, sigma, n_flavors):
-    """S_n of Eq. 63.  A[lam][i][j] nested lists / arrays, sigma[lam] or None."""
+def typed_connected_sum(A, sigma, n_flavors, absolute=False, distinct_colours_only=False):
+    """S_n of Eq. 63.  A[lam][i][j] nested lists / arrays, sigma[lam] or None.
+    absolute: sum |weight| instead.  distinct_colours_only: keep only the terms in which the two endpoints
+    of every vertex that both lie in normal cycles have DIFFERENT colours (the terms Eq. 35 keeps)."""
     n = len(A[0])
     N = 2 * n
     total = 0.0
@@ -71,6 +73,10 @@ def typed_connected_sum(A, sigma, n_flavors):
                 for v in c:
                     cyc_index[v] = ci
             for colours in itertools.product(range(n_flavors), repeat=len(normal)):
+                if distinct_colours_only and any(
+                        v in cyc_index and (v + n) in cyc_index and
+                        colours[cyc_index[v]] == colours[cyc_index[v + n]] for v in range(n)):
+                    continue
                 w = sgn
                 for ci, c in enumerate(normal):
                     lam = colours[ci]
@@ -78,7 +84,7 @@ def typed_connected_sum(A, sigma, n_flavors):
                         w *= A[lam][v % n][p[v] % n]
                 for v in Zs:
                     w *= sigma[colours[cyc_index[(v + n) % N]]]      # Eq. 60
-                total += w
+                total += abs(w) if absolute else w
     return total
 
 

@@ -3,7 +3,7 @@ on the same seeded inputs.  Every test here needs a B200 (`-m gpu`).
 
 Acceptance bound (BASELINE.json north_star): |GPU - oracle| <= 1e-10 * M, M = the same sum evaluated
 on |G|, |sigma| with every sign dropped (oracle `absolute=True`).  Where M is too slow to compute
-(n >= 10) the test uses the STRICTER bound 1e-10 * |oracle value| (M >= |C| always).
+(n >= 10, SB) the test uses the STRICTER bound 1e-10 * M_lower_bound(...) <= 1e-10 * M.
 The tabulation step is compared bit for bit (both sides fix the rounding order).
 """
 import json
@@ -57,32 +57,21 @@ def check(got, ref, M, what):
     assert not bad.any(), (what, got[bad][:4], ref[bad][:4], M[bad][:4])
 
 
-def cdet_rounding_bound(A_up, A_dn, sig_up=0.0, sig_dn=0.0):
-    """A-priori rounding bound of the determinant route O2a itself (NOT an expected value): the CDet recursion
-    Eq. 53 evaluated with every term's magnitude, c~(V) = |a(V)| + sum c~(S) |a(V \\ S)|.  O2a works in long double
-    (eps = 2^-63), so |O2a - exact| <~ 1e-17 * c~(V); the paper itself needs extended precision there.
-    The comparison bound for this tier is therefore 1e-10 * M + 1e-17 * c~."""
-    n = A_up.shape[0]
-    full = 1 << n
-    a = np.ones(full)
-    for T in range(1, full):
-        idx = [i for i in range(n) if T >> i & 1]
-        du = np.linalg.det(A_up[np.ix_(idx, idx)] + sig_dn * np.eye(len(idx)))
-        dd = np.linalg.det(A_dn[np.ix_(idx, idx)] + sig_up * np.eye(len(idx)))
-        a[T] = abs(2.0 ** len(idx) * du * dd)
-    c = np.zeros(full)
-    for V in sorted(range(1, full), key=lambda x: bin(x).count("1")):
-        anchor = V & -V
-        rest = V ^ anchor
-        acc = a[V]
-        sub = (rest - 1) & rest
-        while rest:
-            acc += c[anchor | sub] * a[V ^ (anchor | sub)]
-            if sub == 0:
-                break
-            sub = (sub - 1) & rest
-        c[V] = acc
-    return c[1:]
+def M_lower_bound(G, n, n_sub, nf, uniform, n_assign=4, seed=0):
+    """A rigorous LOWER bound of the cancellation scale M (= the sum of |weight| over all connected typed
+    contractions, O1 / O3 with absolute=True) that stays cheap at n >= 10: every term of the uniform sum on
+    Abar[i][j] = min_lam |A_lam[i][j]| with N_f colours per cycle is dominated by the matching
+    SB term, the shift terms (Z nonempty, Eq. 60) are dropped, and of the n_sub^n sublattice assignments
+    (Eq. 55) only `n_assign` seeded ones are kept.  Using it in place of M makes the test STRICTER."""
+    rng = np.random.default_rng(seed)
+    G = np.abs(np.asarray(G))
+    assigns = [[0] * n] if n_sub == 1 else [list(rng.integers(0, n_sub, n)) for _ in range(n_assign)]
+    assigns = list({tuple(a) for a in assigns})
+    total = 0.0
+    for a in assigns:
+        Abar = oracle.subset_blocks(G, list(range(n)), list(a), n_sub).min(axis=0)
+        total += oracle.o3_uniform(Abar, nf, 0.0, False, absolute=True)[0]
+    return total
 
 
 def oracle_vector(G, c, n, n_sub, nf, sigmas, uniform, all_subsets, tier):
@@ -161,7 +150,7 @@ def test_uniform_all_subsets_vs_determinants(cos, n):
         A = np.ascontiguousarray(G[0, :, :, c])
         ref = oracle.o2a_twospin(A, A)
         M = oracle.o3_uniform(A, 2, 0.0, True, absolute=True)
-        check(got[:, c], ref, M + 1e-7 * cdet_rounding_bound(A, A), ("o2a", n, c))
+        check(got[:, c], ref, M, ("o2a", n, c))
         check(got[:, c], oracle.o3_uniform(A, 2, 0.0, True), M, ("o3", n, c))
 
 
@@ -201,8 +190,7 @@ def test_sb_two_spin_with_shifts_vs_determinants(cos):
         for S in (1, 2, 7, 100, 255):
             verts = [i for i in range(n) if S >> i & 1]
             As = oracle.subset_blocks(np.ascontiguousarray(G[..., c]), verts, [0] * len(verts), 1)
-            Mdet = cdet_rounding_bound(As[0], As[1], sig[0], sig[1])[-1]
-            check(got[S - 1, c], ref[S - 1], oracle.o3_alg3(As, sig, absolute=True) + 1e-7 * Mdet, ("o2a'", S, c))
+            check(got[S - 1, c], ref[S - 1], oracle.o3_alg3(As, sig, absolute=True), ("o2a'", S, c))
 
 
 def test_honeycomb_n6_vs_determinants(cos):
@@ -343,12 +331,12 @@ def test_config2_full_sampled(cos):
         A = np.ascontiguousarray(G[:, c].cpu().numpy().reshape(w.n, w.n))
         M = oracle.o3_uniform(A, 2, 0.0, True, absolute=True)
         check(got[:, c], oracle.o3_uniform(A, 2, 0.0, True), M, ("cfg2 o3", c))
-        check(got[:, c], oracle.o2a_twospin(A, A), M + 1e-7 * cdet_rounding_bound(A, A), ("cfg2 o2a", c))
+        check(got[:, c], oracle.o2a_twospin(A, A), M, ("cfg2 o2a", c))
 
 
 def test_config4_full_sampled(cos):
     """BASELINE config 4 at full size (n = 10, three flavours, 8192 configurations), sampled configurations
-    against the polynomial route Eq. 34-38; bound 1e-10 |C| (stricter than 1e-10 M)."""
+    against the polynomial route Eq. 34-38 (binary128); bound 1e-10 * (a lower bound of M)."""
     w = get_config(4)
     table, v, G = _tabulated(cos, w)
     got, info = _eval_workload(cos, w, G)
@@ -357,19 +345,28 @@ def test_config4_full_sampled(cos):
     for c in (0, 33, 8191):
         A = np.ascontiguousarray(G[:, c].cpu().numpy().reshape(3, w.n, w.n))
         ref = oracle.o2b_polynomial(A, w.sigmas)[-1]
-        check(got[0, c], ref, abs(ref), ("cfg4", c))
+        check(got[0, c], ref, M_lower_bound(A, w.n, 1, 3, False), ("cfg4", c))
+
+
+def _o3_uniform_abs_su2(A):
+    return oracle.o3_uniform(A, 2, 0.0, False, absolute=True)[0]
 
 
 def test_config5_full(cos):
-    """BASELINE config 5 at full size (n = 12, 64 configurations) against O2a; bound 1e-10 |C|."""
+    """BASELINE config 5 at full size (n = 12, 64 configurations): every configuration against O2a (binary128),
+    bound 1e-10 M with M from the printed recurrence on |A| (O3 absolute, ~14 s each: run in a process pool)."""
+    import multiprocessing as mp
     w = get_config(5)
     table, v, G = _tabulated(cos, w)
     got, info = _eval_workload(cos, w, G)
     assert (info["n_states"], info["n_edges"], info["n_readout_edges"]) == (7280663, 57677458, 133)
+    Gh = G.cpu().numpy().reshape(w.n, w.n, w.batch)
+    mats = [np.ascontiguousarray(Gh[:, :, c]) for c in range(w.batch)]
+    with mp.get_context("fork").Pool(min(16, os.cpu_count() or 1)) as pool:
+        Ms = pool.map(_o3_uniform_abs_su2, mats, chunksize=1)
     for c in range(w.batch):
-        A = np.ascontiguousarray(G[:, c].cpu().numpy().reshape(w.n, w.n))
-        ref = oracle.o2a_twospin(A, A)[-1]
-        check(got[0, c], ref, abs(ref), ("cfg5", c))
+        ref = oracle.o2a_twospin(mats[c], mats[c])[-1]
+        check(got[0, c], ref, Ms[c], ("cfg5", c))
 
 
 def test_config3_reduced_batch(cos):
@@ -383,4 +380,4 @@ def test_config3_reduced_batch(cos):
     for c in (0, 95):
         Gc = np.ascontiguousarray(G[:, c].cpu().numpy().reshape(2, w.d, w.d))
         ref = oracle.connected_reference(Gc, w.n, 2, 2, w.sigmas, False, False, tier="o2a")[0]
-        check(got[0, c], ref, abs(ref), ("cfg3", c))
+        check(got[0, c], ref, M_lower_bound(Gc, w.n, 2, 2, False, n_assign=4, seed=c), ("cfg3", c))

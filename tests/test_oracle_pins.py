@@ -265,6 +265,42 @@ def test_absolute_bound_dominates():
     assert close(M1, M3, rtol=1e-10) and M1 >= abs(oracle.o3_alg3(A, s))
 
 
+@pytest.mark.parametrize("n,nf", [(1, 2), (2, 2), (2, 3), (3, 2)])
+def test_o2_absolute_is_the_distinct_colour_part_of_M(n, nf):
+    """O2 with absolute=True (permanents) == literal sum of |weight| over the contractions Eq. 35 keeps
+    (PAPER.md:291-296), hence <= the full cancellation scale M of O1 / O3."""
+    rng = np.random.default_rng(300 + 10 * n + nf)
+    A = rng.standard_normal((nf, n, n))
+    s = rng.standard_normal(nf)
+    lit = typed_connected_sum(A, s, nf, absolute=True, distinct_colours_only=True)
+    got = oracle.o2b_polynomial(A, s, absolute=True)[-1]
+    assert close(got, lit)
+    M = oracle.o1_connected(A, nf, s, sb=True, absolute=True)
+    assert got <= M * (1 + 1e-12) and close(M, typed_connected_sum(A, s, nf, absolute=True))
+    if nf == 2:
+        assert close(oracle.o2a_twospin(A[0], A[1], s[0], s[1], absolute=True)[-1], lit)
+    # signed sum restricted to the same terms == the full signed sum: same-colour terms cancel identically
+    assert close(typed_connected_sum(A, s, nf, distinct_colours_only=True), typed_connected_sum(A, s, nf), scale=M)
+
+
+def test_determinant_route_precision_at_n10():
+    """the determinant recursion needs more than fp64/x87 precision.  On benchmark-shaped
+    propagators (diagonal -rho ~ -0.5, off-diagonal ~ 1e-2) at n = 10 the connected value is ~ 1e-28 while the
+    recursion's terms are O(1): O2a (binary128) must agree with the printed recurrence O3 (fp64, no cancellation
+    beyond M) to 1e-10 M -- an x87 long double O2a misses by > 10 orders of magnitude here."""
+    from cos_workloads import draw_vertices, get_config
+    from cos_workloads.tables import table_for
+    w = get_config(5).scaled(batch=2)
+    G = oracle.tabulate_reference(table_for(w), **{k: v for k, v in draw_vertices(w).items() if k in ("sites", "tau")})
+    for c in range(2):
+        A = np.ascontiguousarray(G[0, :10, :10, c])
+        M = oracle.o3_uniform(A, 2, 0.0, False, absolute=True)[0]
+        a, b = oracle.o2a_twospin(A, A)[-1], oracle.o3_uniform(A, 2)[0]
+        assert abs(a - b) <= 1e-10 * M and abs(a) < 1e-3 * M
+        As = np.stack([A, A])
+        assert abs(oracle.o2b_polynomial(As, None)[-1] - b) <= 1e-10 * M
+
+
 # ---------------------------------------------------------------- structural counts of the printed recurrences
 def test_readout_layers_and_counts():
     """2^n - 1 outputs, every one nonzero for a generic matrix."""
