@@ -43,8 +43,8 @@ struct cos_handle_s {
     double* ws = nullptr;                 // two ping-pong layer slabs
     size_t ws_bytes = 0;
     long long ws_limit = 64ll << 30;
-    int masks_per_cta = 64;
-    int warps_per_cta = 8;
+    int masks_per_cta = 0;
+    int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148, prefetch = 1;
     long long n_launches = 0;
     // profiling (cos_set_profiling): events[k*(NL+1) + l] brackets layer l of the k-th profiled chunk
     bool profiling = false;
@@ -89,14 +89,13 @@ int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int re
 
     const CompiledDag& D = h->dag;
     const size_t smem = layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d, D.has_shift);
-    if (smem > 227u * 1024u) {
+    if (smem > 227u * 1024u - 64u) {
         delete h;
         return fail(COS_EUNSUPPORTED, "cos_build: propagator tile does not fit the 227 KB shared memory of one SM");
     }
-    // launch shape: keep >= 16 warps per SM when shared memory allows several CTAs per SM
-    h->warps_per_cta = env_int("COS_WARPS_PER_CTA", smem > 110u * 1024u ? 16 : 8);
-    h->masks_per_cta = env_int("COS_MASKS_PER_CTA", smem > 110u * 1024u ? 128 : 64);
-    if (h->masks_per_cta < 1) h->masks_per_cta = 1;
+    h->warps_per_cta = 8;
+    h->masks_per_cta = env_int("COS_MASKS_PER_CTA", 0);        // 0: chosen per layer in cos_eval
+    h->prefetch = env_int("COS_PREFETCH", 1);
 
     if (!(flags & COS_BUILD_HOST_ONLY)) {
         int ndev = 0;
@@ -108,6 +107,11 @@ int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int re
         cudaGetDevice(&h->device);
         e = configure_layer_kernels();
         if (e != cudaSuccess) { delete h; return cuda_fail(e, "cos_build: cudaFuncSetAttribute"); }
+        // launch shape: the CTA size that keeps the most warps resident per SM for this instantiation
+        e = pick_layer_warps((int)D.max_L, D.nc, D.has_shift, smem, &h->warps_per_cta, &h->ctas_per_sm);
+        if (e != cudaSuccess) { delete h; return cuda_fail(e, "cos_build: occupancy query"); }
+        h->warps_per_cta = env_int("COS_WARPS_PER_CTA", h->warps_per_cta);
+        cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
         h->dl.resize(D.layers.size());
         for (size_t l = 0; l < D.layers.size(); ++l) {
             const LayerProgram& P = D.layers[l];
@@ -206,7 +210,18 @@ int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev
             const LayerProgram& P = D.layers[l];
             LayerArgs a;
             a.words = h->dl[l].words; a.mask_off = h->dl[l].mask_off;
-            a.n_masks = P.n_masks; a.masks_per_cta = (uint32_t)h->masks_per_cta;
+            a.n_masks = P.n_masks;
+            {   // blocks per CTA: amortise the table staging (<= 64 blocks) but keep >= 4 waves of CTAs on the GPU
+                long long mpc = h->masks_per_cta;
+                if (mpc <= 0) {
+                    mpc = (long long)P.n_masks * tiles / ((long long)h->n_sm * h->ctas_per_sm * 4);
+                    if (mpc > 64) mpc = 64;
+                    if (mpc < 2 * h->warps_per_cta) mpc = 2 * h->warps_per_cta;
+                }
+                while ((P.n_masks + mpc - 1) / mpc > 65535) mpc *= 2;
+                a.masks_per_cta = (uint32_t)mpc;
+            }
+            a.prefetch = h->prefetch;
             a.X = slab[l & 1]; a.Y = slab[(l + 1) & 1];
             a.S_src = P.n_states; a.S_dst = (l + 1 < NL) ? D.layers[l + 1].n_states : 0;
             a.G = G_dev; a.batch = batch; a.b0 = t0 * TILE; a.out = out_dev;

@@ -200,7 +200,7 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_s
         const int HDR = out.hdr_words();
         for (int l = 0; l < NL; ++l) {
             LayerProgram& P = out.layers[l];
-            P.mask_off.reserve(P.n_masks + 1);
+            P.mask_off.reserve(2 * (size_t)P.n_masks + 2);
             for (uint32_t id : b.by_layer[l]) {
                 const uint32_t code = b.codes[id];
                 const int jm = b.jmin(code);
@@ -226,6 +226,12 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_s
                 if (stride > 32) return "row record exceeds 32 words";
                 if (P.words.size() + HDR + (size_t)n_rows * stride >= 0xFFFFFFFFull) return "layer program too large";
                 P.mask_off.push_back((uint32_t)P.words.size());
+                {   // first state of the block in the layer slab (block states are contiguous)
+                    uint32_t first = P.n_states;
+                    for (int h = 0; h < d; ++h)
+                        if (b.alive[(size_t)id * d + h]) { first = b.row_base[(size_t)id * d + h]; break; }
+                    P.mask_off.push_back(first);
+                }
                 P.words.push_back(n_rows | ((uint32_t)nJ << 16) | (flags << 24));
                 P.words.push_back(stride | (e_words << 8) | (fresh_a << 16));
                 P.words.push_back(out_idx);
@@ -241,11 +247,12 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_s
                     for (int lam = 0; lam < nc; ++lam) {
                         const size_t w_begin = P.words.size();
                         P.words.push_back(b.row_base[(size_t)id * d + h] + (uint32_t)lam * L);
-                        P.words.push_back(L | ((uint32_t)h << 8) | ((uint32_t)lam << 16));
+                        const uint32_t kh = ((a >> h) & 1u) ? (uint32_t)__builtin_popcount(a & ((1u << h) - 1u)) : 0xFFu;
+                        P.words.push_back(L | ((uint32_t)h << 8) | ((uint32_t)lam << 16) | (kh << 24));
                         uint32_t packed[6] = {0, 0, 0, 0, 0, 0};
                         int k = 0;
-                        for (int e = 0; e < d; ++e)
-                            if ((a >> e) & 1u) { packed[k / 4] |= (uint32_t)e << (8 * (k % 4)); ++k; }
+                        for (int e = 0; e < d; ++e)      // byte = lam*d + e_a: row index of G_lam[e_a][.] in the staged table
+                            if ((a >> e) & 1u) { packed[k / 4] |= (uint32_t)(lam * d + e) << (8 * (k % 4)); ++k; }
                         for (uint32_t w = 0; w < e_words; ++w) P.words.push_back(packed[w]);
                         uint32_t alive_j = 0;
                         for (int q = 0; q < nJ; ++q) {
@@ -272,6 +279,8 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_s
                 P.max_L = std::max(P.max_L, Lmax);
             }
             P.mask_off.push_back((uint32_t)P.words.size());
+            P.mask_off.push_back(P.n_states);
+            P.words.resize(P.words.size() + 64, 0u);          // padding: the kernel reads whole 32-word windows
             out.n_states += P.n_states; out.n_masks += P.n_masks; out.n_rows += P.n_rows;
             out.n_edges += P.e1 + P.e2 + P.e3 + P.e4; out.n_readout_edges += P.readout_edges; out.n_fma += P.n_fma;
             out.max_layer_states = std::max(out.max_layer_states, P.n_states);

@@ -22,8 +22,9 @@ namespace cosb {
 //   w3..w3+nc-1 : destination state index (next layer) of the fresh-head state of colour lambda'
 // row (row_stride = 2 + e_words + nJ words):
 //   w0 : index of the row's first state in this layer's slab (row states are contiguous)
-//   w1 : L[0:8) | h_a[8:16) | lambda[16:24) | rflags[24:32)
-//   w2.. : e_a of the L states, one byte each
+//   w1 : L[0:8) | h_a[8:16) | lambda[16:24) | k_h[24:32)   k_h = position of the state with e_a == h_a in the
+//        row (0xFF: none); its cycle-closing factor G[h][h] must not carry the counterterm
+//   w2.. : lambda*d + e_a of the L states, one byte each (row of G_lambda[e_a][.] in the staged table)
 //   then nJ words: dj = didx[0:26) | j_a[26:31) | mult2[31]   (destination index in the next layer,
 //        destination endpoint, multiplicity 2 - m_j of Lemma 7 as a flag)
 static const uint32_t DIDX_MASK = 0x03FFFFFFu;
@@ -34,7 +35,7 @@ static const uint32_t FLAG_FRESH = 1u, FLAG_READOUT = 2u;
 struct LayerProgram {
     uint32_t n_states = 0, n_masks = 0, n_rows = 0, max_L = 0;
     std::vector<uint32_t> words;
-    std::vector<uint32_t> mask_off;      // [n_masks + 1] word offsets of the block headers
+    std::vector<uint32_t> mask_off;      // [n_masks + 1][2]: {word offset of the block header, first state of the block}
     uint64_t e1 = 0, e2 = 0, e3 = 0, e4 = 0, readout_edges = 0, n_fma = 0;
 };
 

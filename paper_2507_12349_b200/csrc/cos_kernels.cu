@@ -23,45 +23,60 @@ namespace cosb {
 
 static const int MAX_WARPS = 16;
 
+__device__ __forceinline__ double lds64(uint32_t addr)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
 // ------------------------------------------------------------------------------------------------------
 // One row of a block: L contiguous source states, nJ destinations.
+//   rw       this lane's word of the row record (lane k holds word k)
+//   gs_lane  shared-memory byte address of Gs[0][lane]; row (lambda, e) of the table starts at
+//            gs_lane + (lambda*d + e) * dstride, entry j at + j*256 (dstride = d*256 bytes)
+//   gd_lane  shared-memory byte address of the plain diagonal Gd[0][lane] (SHIFT only)
+// Inner loop per DAG edge: one integer add (address), one LDS.64, one DFMA.
 template <int L, int NC, bool SHIFT>
-__device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t base, const int h_a, const int lam,
+__device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, const double* __restrict__ xp,
                                          const int nJ, const int e_words, const bool need_close,
-                                         const int d, const int n_slots,
-                                         const double* __restrict__ Xt, double* __restrict__ Yt,
-                                         const double* __restrict__ Gl, double& close, double (&sp)[NC])
+                                         const uint32_t d, const uint32_t gs_lane, const uint32_t gd_lane,
+                                         double* __restrict__ Yt, double& close, double (&sp)[NC])
 {
     double x[L];
-    int goff[L];
-    const double* xp = Xt + (size_t)base * TILE;
+    uint32_t ra[L];
 #pragma unroll
     for (int k = 0; k < L; ++k) x[k] = __ldcs(xp + (size_t)k * TILE);
+    const uint32_t dstride = d * (TILE * 8u);
 #pragma unroll
     for (int k = 0; k < L; ++k) {
         const uint32_t ew = __shfl_sync(0xFFFFFFFFu, rw, 2 + (k >> 2));
-        const int e_k = (int)((ew >> (8 * (k & 3))) & 0xFFu);
-        goff[k] = ((lam * d + e_k) * d) * TILE;
+        ra[k] = ((ew >> (8 * (k & 3))) & 0xFFu) * dstride + gs_lane;
     }
-    if (need_close) {                       // cycle-closing factor G_lam[e][h] (Eq. 12, 15)
-        const double* gh = Gl + h_a * TILE;
+    const int lam = (int)((rh >> 16) & 0xFFu);
+    if (need_close) {                       // cycle-closing factor G_lam[e][h] (Eq. 12, 15), never shifted
+        const uint32_t h_a = (rh >> 8) & 0xFFu, hoff = h_a * (TILE * 8u);
+        const int kh = (int)(rh >> 24);
+        const uint32_t pd = gd_lane + ((uint32_t)lam * d + h_a) * (TILE * 8u);
+        double c0 = 0.0, c1 = 0.0;
 #pragma unroll
-        for (int k = 0; k < L; ++k) close = fma(gh[goff[k]], x[k], close);
+        for (int k = 0; k < L; ++k) {
+            uint32_t p = ra[k] + hoff;
+            if (SHIFT) p = (k == kh) ? pd : p;
+            if (k & 1) c1 = fma(lds64(p), x[k], c1); else c0 = fma(lds64(p), x[k], c0);
+        }
+        close += c0 + c1;
     }
     for (int jj = 0; jj < nJ; ++jj) {
         const uint32_t dj = __shfl_sync(0xFFFFFFFFu, rw, 2 + e_words + jj);
         const uint32_t didx = dj & DIDX_MASK;
         if (didx == DIDX_DEAD) continue;
-        const int j_a = (int)((dj >> 26) & 31u);
-        const double* gj = Gl + j_a * TILE;
-        const int jgoff = ((lam * d + j_a) * d) * TILE;          // row of G whose source endpoint is j itself
-        const double* gdiag = Gl + (n_slots + lam * d + j_a) * TILE;
+        const uint32_t joff = (dj >> 18) & 0x1F00u;              // j_a * 256 bytes
         double acc0 = 0.0, acc1 = 0.0;
 #pragma unroll
         for (int k = 0; k < L; ++k) {
-            const double* p = gj + goff[k];
-            if (SHIFT) p = (goff[k] == jgoff) ? gdiag : p;      // E2 with e = j merged with the counterterm E3
-            if (k & 1) acc1 = fma(*p, x[k], acc1); else acc0 = fma(*p, x[k], acc0);
+            if (k & 1) acc1 = fma(lds64(ra[k] + joff), x[k], acc1); else acc0 = fma(lds64(ra[k] + joff), x[k], acc0);
         }
         double acc = acc0 + acc1;
         if (dj >> 31) acc += acc;                                // multiplicity 2 - m_j (Lemma 7)
@@ -69,7 +84,7 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t base,
 #pragma unroll
             for (int c = 0; c < NC; ++c) sp[c] = (c == lam) ? acc : sp[c];
         } else {
-            Yt[(size_t)didx * TILE] = acc;
+            __stcs(Yt + (size_t)didx * TILE, acc);
         }
     }
 }
@@ -78,6 +93,7 @@ template <int MAXL, int NC, bool SHIFT>
 __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerArgs a)
 {
     extern __shared__ double Gs[];
+    __shared__ unsigned int s_next;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
     const uint32_t tile = blockIdx.x;
     const int HDR = 3 + NC;
@@ -85,14 +101,20 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
     // ---- stage the tile's propagator table: Gs[slot][lane]
     const long long b = a.b0 + (long long)tile * TILE + lane;
     const bool valid = b < a.batch;
+    if (threadIdx.x == 0) s_next = 0u;
     for (int s = warp; s < a.n_slots; s += W)
         Gs[s * TILE + lane] = valid ? __ldg(a.G + (size_t)s * (size_t)a.batch + (size_t)b) : 0.0;
     __syncthreads();
-    if (SHIFT) {                             // shifted diagonal G_lam[a][a] + c3 sigma_lam (Eq. 49 / 72, 77)
+    if (SHIFT) {
+        // continuation into the partner of the current endpoint (E2 with j = e) always comes with the
+        // counterterm one-cycle E3 at the same destination: fold c3*sigma_lam into the diagonal of the
+        // staged table (Eq. 49 / 72, 77) and keep the plain diagonal for the cycle-closing factor.
         for (int q = warp; q < NC * a.d; q += W) {
             const int lam = q / a.d, e = q - lam * a.d;
             const double sh = lam == 0 ? a.shift[0] : lam == 1 ? a.shift[1] : lam == 2 ? a.shift[2] : a.shift[3];
-            Gs[(a.n_slots + q) * TILE + lane] = Gs[((lam * a.d + e) * a.d + e) * TILE + lane] + sh;
+            const double g = Gs[((lam * a.d + e) * a.d + e) * TILE + lane];
+            Gs[(a.n_slots + q) * TILE + lane] = g;
+            Gs[((lam * a.d + e) * a.d + e) * TILE + lane] = g + sh;
         }
         __syncthreads();
     }
@@ -100,12 +122,40 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
     const uint32_t m_begin = blockIdx.y * a.masks_per_cta;
     const uint32_t m_end = min(a.n_masks, m_begin + a.masks_per_cta);
     const double* Xt = a.X + (size_t)tile * a.S_src * TILE + lane;
+    const char* Xt0 = (const char*)(a.X + (size_t)tile * a.S_src * TILE);
     double* Yt = a.Y + (size_t)tile * a.S_dst * TILE + lane;
-    const double* Gl = Gs + lane;
+    const uint32_t gs_lane = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)lane * 8u;
+    const uint32_t gd_lane = gs_lane + (uint32_t)a.n_slots * (TILE * 8u);
+    const uint2* mtab = (const uint2*)a.mask_off;
 
-    for (uint32_t mi = m_begin + warp; mi < m_end; mi += W) {
-        const uint32_t off = __ldg(a.mask_off + mi);
-        const uint32_t hw = (lane < HDR) ? __ldg(a.words + off + lane) : 0u;
+    // blocks are handed to warps dynamically (block sizes vary); a warp fetches the program window of its
+    // NEXT block and prefetches that block's source states into L2 before it works on the current one.
+    uint32_t mi = 0;
+    if (lane == 0) mi = atomicAdd(&s_next, 1u);
+    mi = __shfl_sync(0xFFFFFFFFu, mi, 0) + m_begin;
+    uint32_t off = 0, hw = 0, rw = 0;
+    if (mi < m_end) {
+        off = __ldg(&mtab[mi].x);
+        hw = __ldg(a.words + off + lane);
+        rw = __ldg(a.words + off + HDR + lane);
+    }
+    while (mi < m_end) {
+        uint32_t mi_n = 0;
+        if (lane == 0) mi_n = atomicAdd(&s_next, 1u);
+        mi_n = __shfl_sync(0xFFFFFFFFu, mi_n, 0) + m_begin;
+        uint32_t off_n = 0, hw_n = 0, rw_n = 0;
+        if (mi_n < m_end) {
+            const uint2 mt = __ldg(&mtab[mi_n]);
+            off_n = mt.x;
+            hw_n = __ldg(a.words + off_n + lane);
+            rw_n = __ldg(a.words + off_n + HDR + lane);
+            if (a.prefetch) {
+                const uint32_t first = mt.y, lines = (__ldg(&mtab[mi_n + 1].y) - first) * 2u;   // 128-byte lines
+                const char* p0 = Xt0 + (size_t)first * (TILE * 8);
+                for (uint32_t i = lane; i < lines; i += 32) prefetch_l2(p0 + (size_t)i * 128);
+            }
+        }
+
         const uint32_t w0 = __shfl_sync(0xFFFFFFFFu, hw, 0), w1 = __shfl_sync(0xFFFFFFFFu, hw, 1);
         const int n_rows = (int)(w0 & 0xFFFFu), nJ = (int)((w0 >> 16) & 0xFFu);
         const uint32_t flags = w0 >> 24;
@@ -117,17 +167,17 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
         for (int c = 0; c < NC; ++c) sp[c] = 0.0;
 
         const uint32_t* rp = a.words + off + HDR;
-        uint32_t rw = (lane < stride) ? __ldg(rp + lane) : 0u;
         for (int r = 0; r < n_rows; ++r) {
             uint32_t rw_next = 0u;
-            if (r + 1 < n_rows && lane < stride) rw_next = __ldg(rp + (size_t)(r + 1) * stride + lane);
+            if (r + 1 < n_rows) rw_next = __ldg(rp + (size_t)(r + 1) * stride + lane);
             const uint32_t base = __shfl_sync(0xFFFFFFFFu, rw, 0), rh = __shfl_sync(0xFFFFFFFFu, rw, 1);
-            const int L = (int)(rh & 0xFFu), h_a = (int)((rh >> 8) & 0xFFu), lam = (int)((rh >> 16) & 0xFFu);
+            const int L = (int)(rh & 0xFFu);
+            const double* xp = Xt + (size_t)base * TILE;
 #define COS_ROW_CASE(LL)                                                                                        \
     case LL:                                                                                                    \
         if (LL <= MAXL)                                                                                         \
-            row_body<(LL <= MAXL ? LL : 1), NC, SHIFT>(rw, base, h_a, lam, nJ, e_words, need_close, a.d,        \
-                                                       a.n_slots, Xt, Yt, Gl, close, sp);                       \
+            row_body<(LL <= MAXL ? LL : 1), NC, SHIFT>(rw, rh, xp, nJ, e_words, need_close, (uint32_t)a.d,      \
+                                                       gs_lane, gd_lane, Yt, close, sp);                        \
         break;
             switch (L) {
                 COS_ROW_CASE(1) COS_ROW_CASE(2) COS_ROW_CASE(3) COS_ROW_CASE(4) COS_ROW_CASE(5) COS_ROW_CASE(6)
@@ -143,13 +193,14 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
                 const uint32_t didx = __shfl_sync(0xFFFFFFFFu, hw, 3 + c);
-                Yt[(size_t)didx * TILE] = fma(a.neg_kappa, close, sp[c]);
+                __stcs(Yt + (size_t)didx * TILE, fma(a.neg_kappa, close, sp[c]));
             }
         }
         if (flags & FLAG_READOUT) {          // terminal readout O_S (Eq. 15): one block per subset S
             const uint32_t out_idx = __shfl_sync(0xFFFFFFFFu, hw, 2);
             if (valid) a.out[(size_t)out_idx * (size_t)a.batch + (size_t)b] = a.neg_kappa * close;
         }
+        mi = mi_n; off = off_n; hw = hw_n; rw = rw_n;
     }
 }
 
@@ -196,9 +247,27 @@ cudaError_t configure_layer_kernels()
         for (int nc = 1; nc <= 4; ++nc)
             for (int sh = 0; sh < 2; ++sh) {
                 cudaError_t e = cudaFuncSetAttribute((const void*)pick_layer_fn(Ls[i], nc, sh != 0),
-                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 64);
                 if (e != cudaSuccess) return e;
             }
+    return cudaSuccess;
+}
+
+// Warps per CTA that maximise the resident warps per SM for this instantiation and shared-memory size
+// (ties: the smaller CTA, which leaves more CTAs per SM to overlap the table staging of one with the work of others).
+cudaError_t pick_layer_warps(int max_L, int nc, bool shift, size_t smem, int* warps_per_cta, int* ctas_per_sm)
+{
+    static const int cand[6] = {4, 6, 8, 10, 12, 16};
+    layer_fn fn = pick_layer_fn(max_L, nc, shift);
+    int best_w = 0, best_total = 0, best_ctas = 0;
+    for (int i = 0; i < 6; ++i) {
+        int nb = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)fn, cand[i] * 32, smem);
+        if (e != cudaSuccess) return e;
+        if (nb * cand[i] > best_total) { best_total = nb * cand[i]; best_w = cand[i]; best_ctas = nb; }
+    }
+    if (best_w == 0) return cudaErrorInvalidConfiguration;
+    *warps_per_cta = best_w; *ctas_per_sm = best_ctas;
     return cudaSuccess;
 }
 

@@ -9,7 +9,7 @@ static const int TILE = 32;              // configurations per batch tile = one 
 
 struct LayerArgs {
     const uint32_t* words;               // layer program (cos_compile.h)
-    const uint32_t* mask_off;            // [n_masks+1]
+    const uint32_t* mask_off;            // [n_masks+1][2]: {header word offset, first state}
     uint32_t n_masks, masks_per_cta;
     const double* X;                     // source slab  [tile][S_src][32]
     double* Y;                           // destination slab [tile][S_dst][32]
@@ -19,6 +19,7 @@ struct LayerArgs {
     double* out;                         // caller's output [n_out][batch]
     int d, n_slots;                      // n_slots = n_blocks * d * d
     double neg_kappa;                    // -kappa: -N_f (uniform) or -1 (SB)
+    int prefetch;                        // 1: prefetch the next block's source states into L2
     double shift[4];                     // c3 * sigma_lambda of THIS layer (c3 = -2 at layer 0, -1 after)
 };
 
@@ -29,6 +30,7 @@ cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, uint
 // Opt-in to > 48 KB dynamic shared memory for every instantiation (once per process).
 cudaError_t configure_layer_kernels();
 size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift);
+cudaError_t pick_layer_warps(int max_L, int nc, bool shift, size_t smem, int* warps_per_cta, int* ctas_per_sm);
 
 cudaError_t launch_fill_ones(double* X, size_t n_doubles, cudaStream_t stream);
 
