@@ -283,12 +283,8 @@ def run_ours(args):
     assert torch.equal(out_h, out.cpu()), "host-buffer pipeline and device pipeline disagree"
     assert bool(torch.isfinite(out_h).all())
 
-    if world > 1:
-        t = torch.tensor([ms_total, ms_e2e, sum(layer_ms)], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total, ms_e2e, layer_sum = [float(x) for x in t.tolist()]
-    else:
-        layer_sum = sum(layer_ms)
+    from paper_2507_12349_b200.sharding import max_over_ranks
+    ms_total, ms_e2e, layer_sum = max_over_ranks([ms_total, ms_e2e, sum(layer_ms)], device=dev)
 
     if rank == 0:
         K = args.steps

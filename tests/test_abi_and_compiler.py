@@ -1,0 +1,121 @@
+"""CPU-only checks of the boundary and the host DAG compiler: the shared library loads and exports every symbol
+include/cos.h declares, argument errors come back as status codes, and the compiled DAG (COS_BUILD_HOST_ONLY: no
+CUDA call) has the structure the paper fixes (3^n masks, 2^n - 1 readouts, readout layers, Lemma 2) and the R-form
+sizes of SURVEY.md 8(a).  No compute call is made here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def cos():
+    from paper_2507_12349_b200 import build as b
+    b.build()
+    import paper_2507_12349_b200 as cos_mod
+    cos_mod.load_library()
+    return cos_mod
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "cos.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(cos_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(cos):
+    lib = ctypes.CDLL(cos.lib_path())
+    names = declared_symbols()
+    assert "cos_build" in names and "cos_eval" in names and "cos_free" in names and len(names) >= 14
+    for name in names:
+        assert hasattr(lib, name), name
+    assert sorted(cos.EXPORTS) == names          # the binding wraps exactly the declared entry points
+
+
+def test_argument_errors_are_status_codes(cos):
+    for args in [(0, 2, 0, None, 0), (13, 2, 0, None, 0), (4, 0, 0, None, 0), (4, 2, 7, None, 0), (4, 2, 0, None, 3),
+                 (4, 5, 0, [0.1] * 5, 0)]:
+        with pytest.raises(cos.CosError) as ei:
+            cos.cos_build_ex(*args, flags=cos.COS_BUILD_HOST_ONLY)
+        assert ei.value.code in (cos.COS_EINVAL, cos.COS_EUNSUPPORTED)
+        assert cos.cos_last_error()
+    cos.cos_free(None)                           # no-op by contract
+
+
+def test_no_cpu_fallback(cos):
+    """Without a CUDA device cos_build must fail loudly; a host-only handle refuses to evaluate."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("CPU-box check")
+    with pytest.raises(cos.CosError) as ei:
+        cos.cos_build(4, 2, 0, None, 0)
+    assert ei.value.code == cos.COS_ECUDA
+    h = cos.cos_build_ex(4, 2, 0, None, 0, flags=cos.COS_BUILD_HOST_ONLY)
+    lib = cos.load_library()
+    rc = lib.cos_eval(h, ctypes.c_void_p(8), 1, ctypes.c_void_p(8), None)
+    assert rc == cos.COS_ECUDA
+    cos.cos_free(h)
+
+
+SIZES = [  # (n, nf, lattice, shifts, all_subsets) -> (states, edges, readout edges, max layer): SURVEY.md 8(a) [probe]
+    ((4, 2, 0, None, False), (191, 522, 13, 49)),
+    ((8, 2, 0, None, True), (61353, 313828, 3839, 10517)),
+    ((10, 2, 0, None, False), (589979, 3913410, 91, 95353)),
+    ((10, 2, 0, None, True), (815831, 5212505, 24063, 126237)),
+    ((10, 3, 0, (0.2, 0.0, -0.2), False), (1769937, 16020777, 273, 286059)),
+    ((6, 3, 0, (0.2, 0.0, -0.2), False), (9465, 59205, None, 1983)),
+    ((6, 2, 1, (0.3, -0.3), False), (67524, 465976, None, 15344)),
+    ((5, 2, 0, None, False), (795, 2699, None, 177)),
+]
+
+
+@pytest.mark.parametrize("args,want", SIZES)
+def test_rform_sizes(cos, args, want):
+    n, nf, lat, sh, allsub = args
+    h = cos.cos_build_ex(n, nf, lat, sh, n if allsub else 0, flags=cos.COS_BUILD_HOST_ONLY)
+    try:
+        info = cos.dag_summary(h)
+        got = (info["n_states"], info["n_edges"], info["n_readout_edges"], info["max_layer_states"])
+        for g, w in zip(got, want):
+            assert w is None or g == w, (got, want)
+        assert info["n_layers"] == 2 * n
+        assert sum(info["layer_states"]) == info["n_states"]
+    finally:
+        cos.cos_free(h)
+
+
+def test_structure_fixed_by_the_paper(cos):
+    """3^n masks minus the unreachable ones never exceeds 3^n; all-subset readouts are 2^n - 1
+    (PAPER.md:156); n = 4 per-layer state counts of SURVEY.md 8(a); single-output uses only root 0."""
+    n = 4
+    h1 = cos.cos_build_ex(n, 2, 0, None, 0, flags=cos.COS_BUILD_HOST_ONLY)
+    h2 = cos.cos_build_ex(n, 2, 0, None, n, flags=cos.COS_BUILD_HOST_ONLY)
+    try:
+        i1, i2 = cos.dag_summary(h1), cos.dag_summary(h2)
+        assert i1["layer_states"] == [1, 4, 15, 33, 46, 49, 30, 13]
+        assert i2["layer_states"] == [4, 10, 26, 49, 57, 56, 30, 13]
+        assert i1["n_out"] == 1 and i2["n_out"] == 2 ** n - 1
+        assert i2["n_masks"] <= 3 ** n and i1["n_masks"] <= 3 ** n
+        assert i2["n_readout_edges"] == 4 + 18 + 28 + 13
+        assert i1["n_states_unpruned"] >= i1["n_states"]
+    finally:
+        cos.cos_free(h1)
+        cos.cos_free(h2)
+
+
+def test_sb_colour_scaling(cos):
+    """SB mode carries the colour in the state: states = N_f x (uniform states) for the same lattice / readout, and
+    shift edges exist only with shifts (Eq. 79-80)."""
+    hu = cos.cos_build_ex(6, 3, 0, None, 0, flags=cos.COS_BUILD_HOST_ONLY)
+    hs = cos.cos_build_ex(6, 3, 0, (0.1, 0.2, 0.3), 0, flags=cos.COS_BUILD_HOST_ONLY)
+    try:
+        iu, is_ = cos.dag_summary(hu), cos.dag_summary(hs)
+        assert is_["n_states"] == 3 * iu["n_states"]
+        assert is_["n_blocks"] == 3 and iu["n_blocks"] == 1
+        assert is_["n_edges"] > 3 * iu["n_edges"]        # + E3 and the colour fan-out of E4
+    finally:
+        cos.cos_free(hu)
+        cos.cos_free(hs)
