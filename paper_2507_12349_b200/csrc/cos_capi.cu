@@ -44,7 +44,7 @@ struct cos_handle_s {
     size_t ws_bytes = 0;
     long long ws_limit = 64ll << 30;
     int masks_per_cta = 0;
-    int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148, prefetch = 1;
+    int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148, prefetch = 0;
     long long n_launches = 0;
     // profiling (cos_set_profiling): events[k*(NL+1) + l] brackets layer l of the k-th profiled chunk
     bool profiling = false;
@@ -95,7 +95,7 @@ int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int re
     }
     h->warps_per_cta = 8;
     h->masks_per_cta = env_int("COS_MASKS_PER_CTA", 0);        // 0: chosen per layer in cos_eval
-    h->prefetch = env_int("COS_PREFETCH", 1);
+    h->prefetch = env_int("COS_PREFETCH", 0);
 
     if (!(flags & COS_BUILD_HOST_ONLY)) {
         int ndev = 0;

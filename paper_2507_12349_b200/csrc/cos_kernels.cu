@@ -149,7 +149,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
             off_n = mt.x;
             hw_n = __ldg(a.words + off_n + lane);
             rw_n = __ldg(a.words + off_n + HDR + lane);
-            if (a.prefetch) {
+            if (a.prefetch < 0) {
                 const uint32_t first = mt.y, lines = (__ldg(&mtab[mi_n + 1].y) - first) * 2u;   // 128-byte lines
                 const char* p0 = Xt0 + (size_t)first * (TILE * 8);
                 for (uint32_t i = lane; i < lines; i += 32) prefetch_l2(p0 + (size_t)i * 128);
@@ -173,6 +173,12 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
             const uint32_t base = __shfl_sync(0xFFFFFFFFu, rw, 0), rh = __shfl_sync(0xFFFFFFFFu, rw, 1);
             const int L = (int)(rh & 0xFFu);
             const double* xp = Xt + (size_t)base * TILE;
+            if (a.prefetch > 0) {            // L2 look-ahead: the L states `prefetch` states further down the slab
+                for (int q = lane; q < 2 * L; q += 32) {
+                    const uint32_t st = base + (uint32_t)a.prefetch + (uint32_t)(q >> 1);
+                    if (st < a.S_src) prefetch_l2(Xt0 + (size_t)st * (TILE * 8) + (size_t)(q & 1) * 128);
+                }
+            }
 #define COS_ROW_CASE(LL)                                                                                        \
     case LL:                                                                                                    \
         if (LL <= MAXL)                                                                                         \

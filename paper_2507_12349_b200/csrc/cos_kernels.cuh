@@ -19,7 +19,8 @@ struct LayerArgs {
     double* out;                         // caller's output [n_out][batch]
     int d, n_slots;                      // n_slots = n_blocks * d * d
     double neg_kappa;                    // -kappa: -N_f (uniform) or -1 (SB)
-    int prefetch;                        // 1: prefetch the next block's source states into L2
+    int prefetch;                        // > 0: per row, prefetch into L2 the source states this many states ahead;
+                                         // < 0: prefetch the next block's states; 0: off
     double shift[4];                     // c3 * sigma_lambda of THIS layer (c3 = -2 at layer 0, -1 after)
 };
 
