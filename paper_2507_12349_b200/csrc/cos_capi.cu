@@ -44,7 +44,7 @@ struct cos_handle_s {
     size_t ws_bytes = 0;
     long long ws_limit = 64ll << 30;
     int masks_per_cta = 0;
-    int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148, prefetch = 0;
+    int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148, prefetch = 0, ring = 0;
     long long n_launches = 0;
     // profiling (cos_set_profiling): events[k*(NL+1) + l] brackets layer l of the k-th profiled chunk
     bool profiling = false;
@@ -88,8 +88,8 @@ int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int re
     if (!err.empty()) { delete h; return fail(COS_ENOMEM, "cos_build: " + err); }
 
     const CompiledDag& D = h->dag;
-    const size_t smem = layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d, D.has_shift);
-    if (smem > 227u * 1024u - 64u) {
+    const size_t smem = layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d, D.has_shift, 0, 0);
+    if (smem > LAYER_SMEM_MAX) {
         delete h;
         return fail(COS_EUNSUPPORTED, "cos_build: propagator tile does not fit the 227 KB shared memory of one SM");
     }
@@ -108,9 +108,15 @@ int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int re
         e = configure_layer_kernels();
         if (e != cudaSuccess) { delete h; return cuda_fail(e, "cos_build: cudaFuncSetAttribute"); }
         // launch shape: the CTA size that keeps the most warps resident per SM for this instantiation
-        e = pick_layer_warps((int)D.max_L, D.nc, D.has_shift, smem, &h->warps_per_cta, &h->ctas_per_sm);
+        e = pick_layer_shape((int)D.max_L, D.nc, D.d, D.n_blocks * D.d * D.d, D.has_shift, env_int("COS_RING", 0),
+                             &h->ring, &h->warps_per_cta, &h->ctas_per_sm);
         if (e != cudaSuccess) { delete h; return cuda_fail(e, "cos_build: occupancy query"); }
-        h->warps_per_cta = env_int("COS_WARPS_PER_CTA", h->warps_per_cta);
+        {   // experiment override; the ring must still fit
+            const int w = env_int("COS_WARPS_PER_CTA", h->warps_per_cta);
+            if (w >= 1 && w <= 24 &&
+                layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d, D.has_shift, h->ring, w) <= LAYER_SMEM_MAX)
+                h->warps_per_cta = w;
+        }
         cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
         h->dl.resize(D.layers.size());
         for (size_t l = 0; l < D.layers.size(); ++l) {
@@ -211,11 +217,17 @@ int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev
             LayerArgs a;
             a.words = h->dl[l].words; a.mask_off = h->dl[l].mask_off;
             a.n_masks = P.n_masks;
-            {   // blocks per CTA: amortise the table staging (<= 64 blocks) but keep >= 4 waves of CTAs on the GPU
+            {   // blocks per CTA: amortise the table staging but keep >= 4 waves of CTAs on the GPU
                 long long mpc = h->masks_per_cta;
                 if (mpc <= 0) {
                     mpc = (long long)P.n_masks * tiles / ((long long)h->n_sm * h->ctas_per_sm * 4);
-                    if (mpc > 64) mpc = 64;
+                    // staging the table costs one 256-byte line per slot and CTA; a block moves ~30 lines each way:
+                    // about one block per staged slot keeps the staging share at a few percent
+                    long long cap = D.n_blocks * D.d * D.d + (D.has_shift ? D.nc * D.d : 0);
+                    if (cap < 64) cap = 64;
+                    if (cap > 1024) cap = 1024;
+                    cap = env_int("COS_MASKS_CAP", (int)cap);
+                    if (mpc > cap) mpc = cap;
                     if (mpc < 2 * h->warps_per_cta) mpc = 2 * h->warps_per_cta;
                 }
                 while ((P.n_masks + mpc - 1) / mpc > 65535) mpc *= 2;
@@ -228,7 +240,7 @@ int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev
             a.d = D.d; a.n_slots = D.n_blocks * D.d * D.d;
             a.neg_kappa = -D.kappa;
             for (int c = 0; c < 4; ++c) a.shift[c] = (l == 0 ? -2.0 : -1.0) * D.sigma[c];
-            e = launch_layer(a, (int)D.max_L, D.nc, D.has_shift, tiles, h->warps_per_cta, stream);
+            e = launch_layer(a, (int)D.max_L, D.nc, D.has_shift, h->ring, tiles, h->warps_per_cta, stream);
             if (e != cudaSuccess) return cuda_fail(e, "cos_eval: layer launch");
             if (P.n_masks) ++h->n_launches;
             if (ev) cudaEventRecord(ev[l + 1], stream);

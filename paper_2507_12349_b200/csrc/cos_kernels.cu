@@ -22,6 +22,9 @@
 namespace cosb {
 
 static const int MAX_WARPS = 16;
+// CTA size bound per instantiation: the long-row kernels (honeycomb, d = 20) are shared-memory limited to one CTA
+// per SM, so they take 24 warps (<= 85 registers) instead of 16.
+__host__ __device__ constexpr int max_warps_of(int maxl) { return maxl == 20 ? 24 : MAX_WARPS; }
 
 __device__ __forceinline__ double lds64(uint32_t addr)
 {
@@ -30,6 +33,14 @@ __device__ __forceinline__ double lds64(uint32_t addr)
     return v;
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// asynchronous 8-byte global -> shared copy (LDGSTS): no register staging, completion by commit / wait groups
+__device__ __forceinline__ void cp_async8(uint32_t dst, const void* src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 // ------------------------------------------------------------------------------------------------------
 // One row of a block: L contiguous source states, nJ destinations.
@@ -37,17 +48,25 @@ __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefe
 //   gs_lane  shared-memory byte address of Gs[0][lane]; row (lambda, e) of the table starts at
 //            gs_lane + (lambda*d + e) * dstride, entry j at + j*256 (dstride = d*256 bytes)
 //   gd_lane  shared-memory byte address of the plain diagonal Gd[0][lane] (SHIFT only)
+//   RING = 0 the L source values are loaded from global memory (xp);
+//   RING > 0 they were copied ahead of time into this warp's shared-memory ring (ring_lane, stream position o)
 // Inner loop per DAG edge: one integer add (address), one LDS.64, one DFMA.
-template <int L, int NC, bool SHIFT>
+template <int L, int NC, bool SHIFT, int RING>
 __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, const double* __restrict__ xp,
+                                         const uint32_t ring_lane, const uint32_t o,
                                          const int nJ, const int e_words, const bool need_close,
                                          const uint32_t d, const uint32_t gs_lane, const uint32_t gd_lane,
                                          double* __restrict__ Yt, double& close, double (&sp)[NC])
 {
     double x[L];
     uint32_t ra[L];
+    if (RING > 0) {
 #pragma unroll
-    for (int k = 0; k < L; ++k) x[k] = __ldcs(xp + (size_t)k * TILE);
+        for (int k = 0; k < L; ++k) x[k] = lds64(ring_lane + (((o + (uint32_t)k) & (uint32_t)(RING - 1)) << 8));
+    } else {
+#pragma unroll
+        for (int k = 0; k < L; ++k) x[k] = __ldcs(xp + (size_t)k * TILE);
+    }
     const uint32_t dstride = d * (TILE * 8u);
 #pragma unroll
     for (int k = 0; k < L; ++k) {
@@ -89,8 +108,8 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
     }
 }
 
-template <int MAXL, int NC, bool SHIFT>
-__global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerArgs a)
+template <int MAXL, int NC, bool SHIFT, int RING>
+__global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(const LayerArgs a)
 {
     extern __shared__ double Gs[];
     __shared__ unsigned int s_next;
@@ -98,12 +117,21 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
     const uint32_t tile = blockIdx.x;
     const int HDR = 3 + NC;
 
-    // ---- stage the tile's propagator table: Gs[slot][lane]
+    const uint32_t gs_lane = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)lane * 8u;
+    const uint32_t gd_lane = gs_lane + (uint32_t)a.n_slots * (TILE * 8u);
+    const uint32_t n_tab = (uint32_t)a.n_slots + (SHIFT ? (uint32_t)(NC * a.d) : 0u);
+    const uint32_t ring_lane = gs_lane + (n_tab + (uint32_t)warp * (uint32_t)(RING > 0 ? RING : 0)) * (TILE * 8u);
+
+    // ---- stage the tile's propagator table Gs[slot][lane] with asynchronous copies (all in flight at once)
     const long long b = a.b0 + (long long)tile * TILE + lane;
     const bool valid = b < a.batch;
     if (threadIdx.x == 0) s_next = 0u;
-    for (int s = warp; s < a.n_slots; s += W)
-        Gs[s * TILE + lane] = valid ? __ldg(a.G + (size_t)s * (size_t)a.batch + (size_t)b) : 0.0;
+    for (int s = warp; s < a.n_slots; s += W) {
+        if (valid) cp_async8(gs_lane + (uint32_t)s * (TILE * 8u), a.G + (size_t)s * (size_t)a.batch + (size_t)b);
+        else Gs[s * TILE + lane] = 0.0;
+    }
+    cp_async_commit();
+    cp_async_wait<0>();
     __syncthreads();
     if (SHIFT) {
         // continuation into the partner of the current endpoint (E2 with j = e) always comes with the
@@ -124,32 +152,39 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
     const double* Xt = a.X + (size_t)tile * a.S_src * TILE + lane;
     const char* Xt0 = (const char*)(a.X + (size_t)tile * a.S_src * TILE);
     double* Yt = a.Y + (size_t)tile * a.S_dst * TILE + lane;
-    const uint32_t gs_lane = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)lane * 8u;
-    const uint32_t gd_lane = gs_lane + (uint32_t)a.n_slots * (TILE * 8u);
     const uint2* mtab = (const uint2*)a.mask_off;
 
-    // blocks are handed to warps dynamically (block sizes vary); a warp fetches the program window of its
-    // NEXT block and prefetches that block's source states into L2 before it works on the current one.
+    // Blocks are handed to warps dynamically (block sizes vary).  A warp always knows its current AND its next
+    // block: the next block's program window is fetched early, and (RING > 0) the source states of both are
+    // streamed, in slab order, through the warp's shared-memory ring up to RING states ahead of the row in work.
+    //   stream coordinate = running count of the source states of the blocks this warp has taken;
+    //   current block: coordinates [s0, s1), slab index = coordinate + d0;  next block: [s1, s1 + c1), + d1.
     uint32_t mi = 0;
     if (lane == 0) mi = atomicAdd(&s_next, 1u);
     mi = __shfl_sync(0xFFFFFFFFu, mi, 0) + m_begin;
     uint32_t off = 0, hw = 0, rw = 0;
+    uint32_t s1 = 0, d0 = 0, d1 = 0, c1 = 0, front = 0;
+    bool primed = false;
     if (mi < m_end) {
-        off = __ldg(&mtab[mi].x);
+        const uint2 mt = __ldg(&mtab[mi]);
+        off = mt.x;
         hw = __ldg(a.words + off + lane);
         rw = __ldg(a.words + off + HDR + lane);
+        if (RING > 0) { d1 = mt.y; c1 = __ldg(&mtab[mi + 1].y) - mt.y; }     // becomes the current block below
     }
     while (mi < m_end) {
         uint32_t mi_n = 0;
         if (lane == 0) mi_n = atomicAdd(&s_next, 1u);
         mi_n = __shfl_sync(0xFFFFFFFFu, mi_n, 0) + m_begin;
         uint32_t off_n = 0, hw_n = 0, rw_n = 0;
+        if (RING > 0) { d0 = d1; s1 += c1; c1 = 0; }                        // next -> current
         if (mi_n < m_end) {
             const uint2 mt = __ldg(&mtab[mi_n]);
             off_n = mt.x;
             hw_n = __ldg(a.words + off_n + lane);
             rw_n = __ldg(a.words + off_n + HDR + lane);
-            if (a.prefetch < 0) {
+            if (RING > 0) { c1 = __ldg(&mtab[mi_n + 1].y) - mt.y; d1 = mt.y - s1; }
+            if (RING == 0 && a.prefetch < 0) {
                 const uint32_t first = mt.y, lines = (__ldg(&mtab[mi_n + 1].y) - first) * 2u;   // 128-byte lines
                 const char* p0 = Xt0 + (size_t)first * (TILE * 8);
                 for (uint32_t i = lane; i < lines; i += 32) prefetch_l2(p0 + (size_t)i * 128);
@@ -173,7 +208,22 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
             const uint32_t base = __shfl_sync(0xFFFFFFFFu, rw, 0), rh = __shfl_sync(0xFFFFFFFFu, rw, 1);
             const int L = (int)(rh & 0xFFu);
             const double* xp = Xt + (size_t)base * TILE;
-            if (a.prefetch > 0) {            // L2 look-ahead: the L states `prefetch` states further down the slab
+            uint32_t o = 0;
+            if (RING > 0) {
+                // top the ring up to RING states past the start of this row (never past the next block), then
+                // wait for everything but the copies just issued: this row's states were issued a row earlier
+                // (RING >= 2 * MAXL), so they have landed.
+                o = base - d0;
+                const uint32_t hi = min(o + (uint32_t)RING, s1 + c1);
+                while (front < hi) {
+                    const uint32_t g = front + (front < s1 ? d0 : d1);
+                    cp_async8(ring_lane + ((front & (uint32_t)(RING - 1)) << 8), Xt + (size_t)g * TILE);
+                    ++front;
+                }
+                cp_async_commit();
+                if (primed) cp_async_wait<1>(); else cp_async_wait<0>();      // the very first row has no earlier step
+                primed = true;
+            } else if (a.prefetch > 0) {     // L2 look-ahead: the L states `prefetch` states further down the slab
                 for (int q = lane; q < 2 * L; q += 32) {
                     const uint32_t st = base + (uint32_t)a.prefetch + (uint32_t)(q >> 1);
                     if (st < a.S_src) prefetch_l2(Xt0 + (size_t)st * (TILE * 8) + (size_t)(q & 1) * 128);
@@ -182,8 +232,8 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
 #define COS_ROW_CASE(LL)                                                                                        \
     case LL:                                                                                                    \
         if (LL <= MAXL)                                                                                         \
-            row_body<(LL <= MAXL ? LL : 1), NC, SHIFT>(rw, rh, xp, nJ, e_words, need_close, (uint32_t)a.d,      \
-                                                       gs_lane, gd_lane, Yt, close, sp);                        \
+            row_body<(LL <= MAXL ? LL : 1), NC, SHIFT, RING>(rw, rh, xp, ring_lane, o, nJ, e_words, need_close, \
+                                                             (uint32_t)a.d, gs_lane, gd_lane, Yt, close, sp);   \
         break;
             switch (L) {
                 COS_ROW_CASE(1) COS_ROW_CASE(2) COS_ROW_CASE(3) COS_ROW_CASE(4) COS_ROW_CASE(5) COS_ROW_CASE(6)
@@ -208,42 +258,51 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
         }
         mi = mi_n; off = off_n; hw = hw_n; rw = rw_n;
     }
+    if (RING > 0) cp_async_wait<0>();
 }
 
 // ------------------------------------------------------------------------------------------------------
 typedef void (*layer_fn)(const LayerArgs);
 
-template <int MAXL>
+template <int MAXL, int RING>
 static layer_fn pick_nc(int nc, bool shift)
 {
     if (!shift) {
         switch (nc) {
-            case 1: return cos_layer_kernel<MAXL, 1, false>;
-            case 2: return cos_layer_kernel<MAXL, 2, false>;
-            case 3: return cos_layer_kernel<MAXL, 3, false>;
-            default: return cos_layer_kernel<MAXL, 4, false>;
+            case 1: return cos_layer_kernel<MAXL, 1, false, RING>;
+            case 2: return cos_layer_kernel<MAXL, 2, false, RING>;
+            case 3: return cos_layer_kernel<MAXL, 3, false, RING>;
+            default: return cos_layer_kernel<MAXL, 4, false, RING>;
         }
     }
     switch (nc) {
-        case 1: return cos_layer_kernel<MAXL, 1, true>;
-        case 2: return cos_layer_kernel<MAXL, 2, true>;
-        case 3: return cos_layer_kernel<MAXL, 3, true>;
-        default: return cos_layer_kernel<MAXL, 4, true>;
+        case 1: return cos_layer_kernel<MAXL, 1, true, RING>;
+        case 2: return cos_layer_kernel<MAXL, 2, true, RING>;
+        case 3: return cos_layer_kernel<MAXL, 3, true, RING>;
+        default: return cos_layer_kernel<MAXL, 4, true, RING>;
     }
 }
 
-static layer_fn pick_layer_fn(int max_L, int nc, bool shift)
+// ring = 0: source rows loaded straight into registers; ring = LAYER_RING: streamed through shared memory
+// (needs LAYER_RING >= 2 * MAXL, so only the max_L <= 12 instantiations have it).
+static layer_fn pick_layer_fn(int max_L, int nc, bool shift, int ring)
 {
-    if (max_L <= 4) return pick_nc<4>(nc, shift);
-    if (max_L <= 8) return pick_nc<8>(nc, shift);
-    if (max_L <= 12) return pick_nc<12>(nc, shift);
-    if (max_L <= 20) return pick_nc<20>(nc, shift);
-    return pick_nc<24>(nc, shift);
+    if (ring > 0) {
+        if (max_L <= 4) return pick_nc<4, LAYER_RING>(nc, shift);
+        if (max_L <= 8) return pick_nc<8, LAYER_RING>(nc, shift);
+        if (max_L <= 12) return pick_nc<12, LAYER_RING>(nc, shift);
+        return nullptr;
+    }
+    if (max_L <= 4) return pick_nc<4, 0>(nc, shift);
+    if (max_L <= 8) return pick_nc<8, 0>(nc, shift);
+    if (max_L <= 12) return pick_nc<12, 0>(nc, shift);
+    if (max_L <= 20) return pick_nc<20, 0>(nc, shift);
+    return pick_nc<24, 0>(nc, shift);
 }
 
-size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift)
+size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift, int ring, int warps_per_cta)
 {
-    return (size_t)(n_slots + (shift ? nc * d : 0)) * TILE * sizeof(double);
+    return (size_t)(n_slots + (shift ? nc * d : 0) + (ring > 0 ? ring * warps_per_cta : 0)) * TILE * sizeof(double);
 }
 
 cudaError_t configure_layer_kernels()
@@ -251,43 +310,62 @@ cudaError_t configure_layer_kernels()
     static const int Ls[5] = {4, 8, 12, 20, 24};
     for (int i = 0; i < 5; ++i)
         for (int nc = 1; nc <= 4; ++nc)
-            for (int sh = 0; sh < 2; ++sh) {
-                cudaError_t e = cudaFuncSetAttribute((const void*)pick_layer_fn(Ls[i], nc, sh != 0),
-                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024 - 64);
-                if (e != cudaSuccess) return e;
-            }
+            for (int sh = 0; sh < 2; ++sh)
+                for (int ring = 0; ring <= LAYER_RING; ring += LAYER_RING) {
+                    layer_fn fn = pick_layer_fn(Ls[i], nc, sh != 0, ring);
+                    if (!fn) continue;
+                    cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                                         (int)LAYER_SMEM_MAX);
+                    if (e != cudaSuccess) return e;
+                }
     return cudaSuccess;
 }
 
-// Warps per CTA that maximise the resident warps per SM for this instantiation and shared-memory size
-// (ties: the smaller CTA, which leaves more CTAs per SM to overlap the table staging of one with the work of others).
-cudaError_t pick_layer_warps(int max_L, int nc, bool shift, size_t smem, int* warps_per_cta, int* ctas_per_sm)
+// Launch shape for this instantiation: ring or not, warps per CTA.
+//   ring path  (max_L <= 12 and the table leaves room for >= 8 rings): the CTA size with the most resident warps
+//              per SM counting each warp's ring; look-ahead, not occupancy, hides the HBM latency there.
+//   direct path: the CTA size that maximises resident warps per SM (ties: the smaller CTA).
+cudaError_t pick_layer_shape(int max_L, int nc, int d, int n_slots, bool shift, int want_ring, int* ring,
+                             int* warps_per_cta, int* ctas_per_sm)
 {
-    static const int cand[6] = {4, 6, 8, 10, 12, 16};
-    layer_fn fn = pick_layer_fn(max_L, nc, shift);
-    int best_w = 0, best_total = 0, best_ctas = 0;
-    for (int i = 0; i < 6; ++i) {
-        int nb = 0;
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)fn, cand[i] * 32, smem);
-        if (e != cudaSuccess) return e;
-        if (nb * cand[i] > best_total) { best_total = nb * cand[i]; best_w = cand[i]; best_ctas = nb; }
+    static const int cand[8] = {4, 6, 8, 10, 12, 16, 20, 24};
+    const int max_w = max_warps_of(max_L <= 4 ? 4 : max_L <= 8 ? 8 : max_L <= 12 ? 12 : max_L <= 20 ? 20 : 24);
+    for (int pass = 0; pass < 2; ++pass) {
+        const int rg = (pass == 0) ? LAYER_RING : 0;
+        if (pass == 0 && (want_ring == 0 || max_L > 12)) continue;
+        layer_fn fn = pick_layer_fn(max_L, nc, shift, rg);
+        if (!fn) continue;
+        int best_w = 0, best_total = 0, best_ctas = 0;
+        for (int i = 0; i < 8; ++i) {
+            const size_t smem = layer_smem_bytes(n_slots, nc, d, shift, rg, cand[i]);
+            if (smem > LAYER_SMEM_MAX || cand[i] > max_w) continue;
+            int nb = 0;
+            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)fn, cand[i] * 32, smem);
+            if (e != cudaSuccess) return e;
+            if (nb * cand[i] > best_total) { best_total = nb * cand[i]; best_w = cand[i]; best_ctas = nb; }
+        }
+        if (best_w == 0 || (pass == 0 && best_total < 8)) continue;
+        *ring = rg; *warps_per_cta = best_w; *ctas_per_sm = best_ctas;
+        return cudaSuccess;
     }
-    if (best_w == 0) return cudaErrorInvalidConfiguration;
-    *warps_per_cta = best_w; *ctas_per_sm = best_ctas;
-    return cudaSuccess;
+    return cudaErrorInvalidConfiguration;
 }
 
-cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
-                         cudaStream_t stream)
+cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, int ring, uint32_t tiles,
+                         int warps_per_cta, cudaStream_t stream)
 {
     if (a.n_masks == 0 || tiles == 0) return cudaSuccess;
     if (warps_per_cta < 1) warps_per_cta = 1;
-    if (warps_per_cta > MAX_WARPS) warps_per_cta = MAX_WARPS;
+    const int max_w = max_warps_of(max_L <= 4 ? 4 : max_L <= 8 ? 8 : max_L <= 12 ? 12 : max_L <= 20 ? 20 : 24);
+    if (warps_per_cta > max_w) warps_per_cta = max_w;
     const uint32_t chunks = (a.n_masks + a.masks_per_cta - 1) / a.masks_per_cta;
     if (chunks > 65535u) return cudaErrorInvalidConfiguration;
     dim3 grid(tiles, chunks, 1), block(32 * warps_per_cta, 1, 1);
-    layer_fn fn = pick_layer_fn(max_L, nc, shift);
-    fn<<<grid, block, layer_smem_bytes(a.n_slots, nc, a.d, shift), stream>>>(a);
+    layer_fn fn = pick_layer_fn(max_L, nc, shift, ring);
+    if (!fn) return cudaErrorInvalidConfiguration;
+    const size_t smem = layer_smem_bytes(a.n_slots, nc, a.d, shift, ring, warps_per_cta);
+    if (smem > LAYER_SMEM_MAX) return cudaErrorInvalidConfiguration;
+    fn<<<grid, block, smem, stream>>>(a);
     return cudaGetLastError();
 }
 

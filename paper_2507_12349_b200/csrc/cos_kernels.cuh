@@ -6,6 +6,8 @@
 namespace cosb {
 
 static const int TILE = 32;              // configurations per batch tile = one warp, lane = configuration
+static const int LAYER_RING = 32;        // states per warp of the shared-memory source ring (>= 2 * 12)
+static const size_t LAYER_SMEM_MAX = 227 * 1024 - 64;
 
 struct LayerArgs {
     const uint32_t* words;               // layer program (cos_compile.h)
@@ -26,12 +28,13 @@ struct LayerArgs {
 
 // Picks the instantiation (max row length, colours, shift) and launches one layer step.
 // grid = (tiles, ceil(n_masks / masks_per_cta)); returns cudaGetLastError().
-cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
-                         cudaStream_t stream);
+cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, int ring, uint32_t tiles,
+                         int warps_per_cta, cudaStream_t stream);
 // Opt-in to > 48 KB dynamic shared memory for every instantiation (once per process).
 cudaError_t configure_layer_kernels();
-size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift);
-cudaError_t pick_layer_warps(int max_L, int nc, bool shift, size_t smem, int* warps_per_cta, int* ctas_per_sm);
+size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift, int ring, int warps_per_cta);
+cudaError_t pick_layer_shape(int max_L, int nc, int d, int n_slots, bool shift, int want_ring, int* ring,
+                             int* warps_per_cta, int* ctas_per_sm);
 
 cudaError_t launch_fill_ones(double* X, size_t n_doubles, cudaStream_t stream);
 
