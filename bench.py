@@ -32,6 +32,9 @@ from cos_workloads.tables import table_for  # noqa: E402
 
 METRIC = "connected_sum_configs_per_s"
 UNIT = "configs/s"
+# DRAM bytes (read + write) of the layer-kernel launches of ONE step, from a committed ncu capture; per workload at its
+# BASELINE batch.  None = not captured.
+NCU_DRAM_BYTES_PER_STEP = {"cfg4_square_sb3_n10": (231.887e9, 8192, "profiles/r01c_dram_traffic_step.md")}
 DEFAULT_WORKLOAD = "cfg4"       # n = 10: the order BASELINE.json's target is quoted on
 
 
@@ -301,12 +304,17 @@ def run_ours(args):
         except (OSError, KeyError, ValueError):
             peak_gbs, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
         achieved_gbs = alg_bytes_step / layer_s_step / 1e9
+        traffic, traffic_src = None, None
+        cap = NCU_DRAM_BYTES_PER_STEP.get(w.name)
+        if cap and cap[1] == B:
+            traffic, traffic_src = cap[0] / NL, cap[2] + " (per launch = step total / %d launches)" % NL
         fma_peak = cos.cos_measure_fp64_fma_peak()
         t_hbm = alg_bytes_step / (peak_gbs * 1e9)
         t_fp64 = info["n_fma"] * B / fma_peak
         roofline = {"bound": "hbm" if t_hbm >= t_fp64 else "alu", "kernel": "cos_layer_kernel",
                     "achieved": achieved_gbs, "peak": peak_gbs, "unit": "GB/s", "frac": achieved_gbs / peak_gbs,
-                    "traffic": None, "peak_source": peak_src,
+                    "traffic": traffic, "traffic_source": traffic_src, "peak_source": peak_src,
+                    "algorithmic_bytes_per_launch": alg_bytes_step / NL,
                     "launches_per_step": NL, "kernel_ms_per_step": layer_s_step * 1e3,
                     "kernel_share_of_step": layer_s_step * 1e3 / (ms_total / K),
                     "algorithmic_bytes_per_step": alg_bytes_step,

@@ -111,7 +111,7 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
 template <int MAXL, int NC, bool SHIFT, int RING>
 __global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(const LayerArgs a)
 {
-    extern __shared__ double Gs[];
+    extern __shared__ __align__(128) double Gs[];
     __shared__ unsigned int s_next;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
     const uint32_t tile = blockIdx.x;
