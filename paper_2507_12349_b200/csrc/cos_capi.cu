@@ -44,7 +44,7 @@ struct cos_handle_s {
     size_t ws_bytes = 0;
     long long ws_limit = 64ll << 30;
     int masks_per_cta = 0;
-    int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148, prefetch = 0, ring = 0;
+    int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148, prefetch = 0, ring = 0, pdl = 1;
     long long n_launches = 0;
     // profiling (cos_set_profiling): events[k*(NL+1) + l] brackets layer l of the k-th profiled chunk
     bool profiling = false;
@@ -96,6 +96,7 @@ int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int re
     h->warps_per_cta = 8;
     h->masks_per_cta = env_int("COS_MASKS_PER_CTA", 0);        // 0: chosen per layer in cos_eval
     h->prefetch = env_int("COS_PREFETCH", 0);
+    h->pdl = env_int("COS_PDL", 1);
 
     if (!(flags & COS_BUILD_HOST_ONLY)) {
         int ndev = 0;
@@ -234,6 +235,7 @@ int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev
                 a.masks_per_cta = (uint32_t)mpc;
             }
             a.prefetch = h->prefetch;
+            a.pdl = (h->pdl && l > 0 && !h->profiling) ? 1 : 0;   // per-layer events need serialised layers
             a.X = slab[l & 1]; a.Y = slab[(l + 1) & 1];
             a.S_src = P.n_states; a.S_dst = (l + 1 < NL) ? D.layers[l + 1].n_states : 0;
             a.G = G_dev; a.batch = batch; a.b0 = t0 * TILE; a.out = out_dev;

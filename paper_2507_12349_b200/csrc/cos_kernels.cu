@@ -122,6 +122,9 @@ __global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(cons
     const uint32_t n_tab = (uint32_t)a.n_slots + (SHIFT ? (uint32_t)(NC * a.d) : 0u);
     const uint32_t ring_lane = gs_lane + (n_tab + (uint32_t)warp * (uint32_t)(RING > 0 ? RING : 0)) * (TILE * 8u);
 
+    // Programmatic dependent launch: let the next layer's grid start (it only stages its table, which no layer
+    // writes) while this grid drains; this grid in turn touches the slabs only after the previous one has completed.
+    if (a.pdl) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
     // ---- stage the tile's propagator table Gs[slot][lane] with asynchronous copies (all in flight at once)
     const long long b = a.b0 + (long long)tile * TILE + lane;
     const bool valid = b < a.batch;
@@ -147,6 +150,7 @@ __global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(cons
         __syncthreads();
     }
 
+    if (a.pdl) asm volatile("griddepcontrol.wait;" ::: "memory");
     const uint32_t m_begin = blockIdx.y * a.masks_per_cta;
     const uint32_t m_end = min(a.n_masks, m_begin + a.masks_per_cta);
     const double* Xt = a.X + (size_t)tile * a.S_src * TILE + lane;
@@ -365,8 +369,17 @@ cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, int 
     if (!fn) return cudaErrorInvalidConfiguration;
     const size_t smem = layer_smem_bytes(a.n_slots, nc, a.d, shift, ring, warps_per_cta);
     if (smem > LAYER_SMEM_MAX) return cudaErrorInvalidConfiguration;
-    fn<<<grid, block, smem, stream>>>(a);
-    return cudaGetLastError();
+    if (!a.pdl) {
+        fn<<<grid, block, smem, stream>>>(a);
+        return cudaGetLastError();
+    }
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, fn, a);
 }
 
 // ------------------------------------------------------------------------------------------------------

@@ -23,6 +23,7 @@ struct LayerArgs {
     double neg_kappa;                    // -kappa: -N_f (uniform) or -1 (SB)
     int prefetch;                        // > 0: per row, prefetch into L2 the source states this many states ahead;
                                          // < 0: prefetch the next block's states; 0: off
+    int pdl;                             // 1: launched with programmatic stream serialization (layers > 0)
     double shift[4];                     // c3 * sigma_lambda of THIS layer (c3 = -2 at layer 0, -1 after)
 };
 
