@@ -61,6 +61,14 @@ int cos_build(int n, int n_flavors, int lattice, const double* shifts, int reado
 int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope,
                  int flags, cos_handle* out);
 
+/* Partial readout sets ("allowed orders U", Eq. 6; requested-output pruning Eq. 21-24):
+ * all-subset layout (2^n-1 output rows, k = bitmask(S)-1), but only subsets whose order |S| has its bit set in
+ * order_mask (bit k <-> |S| = k, 1 <= k <= n) are computed; states that reach no requested readout are pruned
+ * (K_l = F_l ^ B_l, Eq. 23) and the rows of the other subsets are written as zeros by cos_eval.
+ * order_mask without a bit in [1, n]: COS_EINVAL. */
+int cos_build_orders(int n, int n_flavors, int lattice, const double* shifts, unsigned int order_mask, int flags,
+                     cos_handle* out);
+
 /* ---- (3)+(4) layer propagation and terminal readouts: Eq. 16, Eq. 11-15 ----------------------------
  *   G_dev    device, fp64, read-only: G_dev[((blk*d + a)*d + b) * batch + c] = propagator of block blk
  *            from endpoint a to endpoint b (A[vbar, pi(v)bar] of Eq. 59) of configuration c;
@@ -97,6 +105,7 @@ enum {
     COS_INFO_N_STATES_UNPRUNED = 12,
     COS_INFO_WORKSPACE_BYTES = 13,
     COS_INFO_N_LAUNCHES = 14,     /* kernels launched through this handle so far (cos_eval / cos_eval_host) */
+    COS_INFO_ORDER_MASK = 15,     /* requested orders of an all-subset handle (0 for single-output handles) */
     COS_INFO_LAYER_STATES = 100,  /* + layer index */
     COS_INFO_LAYER_EDGES = 200,   /* + layer index: edges leaving that layer (readout edges included) */
     COS_INFO_LAYER_MASKS = 300    /* + layer index */
@@ -131,6 +140,20 @@ void cos_tab_free(cos_tab tab);
  * H2D batch*n*(2*4+8), D2H batch*n_out*8. */
 int cos_eval_host(cos_handle h, cos_tab tab, const int* sites_host, const double* tau_host, long long batch,
                   double* out_host, cos_stream stream);
+
+/* ---- many-configuration heat-bath weights: Eq. 6-7 -------------------------------------
+ * Phi_S = lambda_{|S|} C_S Q_S (Eq. 6),  W = sum_{S, |S| in U} |Phi_S| / binom(n, |S|) (Eq. 7), per configuration.
+ *   n            envelope size N (1..COS_MAX_N)
+ *   order_mask   allowed orders U (bit k <-> |S| = k); 0 = every order
+ *   lambda_host  host fp64 [n+1]: lambda_k at index k (index 0 unused)
+ *   C_dev        device fp64 [2^n-1][batch]: connected values, the layout cos_eval writes (k = bitmask(S)-1)
+ *   Q_dev        device fp64 [2^n-1][batch] conditional densities Q_{S-bar|S}, or NULL for Q = 1
+ *                (the paper takes Q from the sampler, ref. [15]; it is an input here)
+ *   W_dev        device fp64 [batch], written
+ *   Phi_dev      device fp64 [2^n-1][batch] signed fluxes, written (zeros outside U), or NULL to skip
+ * One thread per configuration adds the subsets in increasing bitmask order (deterministic).  Asynchronous. */
+int cos_flux_weights(int n, unsigned int order_mask, const double* lambda_host, const double* C_dev,
+                     const double* Q_dev, long long batch, double* W_dev, double* Phi_dev, cos_stream stream);
 
 /* ---- measurement helpers ------------------------------------------------------------------------------
  * cos_set_profiling(h, 1): every later cos_eval brackets each layer launch with CUDA events on its stream.

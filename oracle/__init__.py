@@ -5,5 +5,5 @@ paper_2507_12349_b200/ imports this package, and this package imports nothing fr
 """
 from .cos_oracle import (  # noqa: F401
     build_oracle, o1_connected, o1_all_subsets, o2a_twospin, o2b_polynomial,
-    o3_alg3, o3_uniform, connected_reference, tabulate_reference, subset_blocks,
+    o3_alg3, o3_uniform, connected_reference, tabulate_reference, subset_blocks, flux_weights,
 )

@@ -214,3 +214,28 @@ def tabulate_reference(table, sites, tau):
                         g = (1.0 - w) * tab[r, k] + w * tab[r, k + 1]
                         G[lam, i * ns + s, j * ns + s2, cols] = sign * g
     return G
+
+
+# ------------------------------------------------------------------ many-configuration weights (Eq. 6-7)
+def flux_weights(C, Q, lambdas, order_mask=0):
+    """Signed fluxes and heat-bath normalisation of ONE envelope, written out from PAPER.md:106-113:
+        Phi_S = lambda_{|S|} C_{|S|}(V_S) Q_{S-bar|S}          for |S| in the allowed orders U     (Eq. 6)
+        W     = sum_{S subset [N], |S| in U} |Phi_S| / binom(N, |S|)                              (Eq. 7)
+    C, Q: arrays [2^N - 1] indexed by bitmask(S) - 1 (Q None -> 1); lambdas[k] = lambda_k, k = 0..N;
+    order_mask bit k <-> k in U (0 = every order).  Returns (W, Phi[2^N - 1]) with Phi = 0 outside U."""
+    import math
+    C = np.asarray(C, dtype=np.float64)
+    N = int(round(math.log2(C.shape[0] + 1)))
+    assert (1 << N) - 1 == C.shape[0]
+    phi = np.zeros_like(C)
+    W = 0.0
+    for S in range(1, 1 << N):
+        k = bin(S).count("1")
+        if order_mask and not (order_mask >> k) & 1:
+            continue
+        p = lambdas[k] * C[S - 1]
+        if Q is not None:
+            p = p * Q[S - 1]
+        phi[S - 1] = p
+        W += abs(p) / math.comb(N, k)
+    return W, phi

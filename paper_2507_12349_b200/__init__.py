@@ -8,6 +8,6 @@ from ._binding import (  # noqa: F401
     CosError, lib_path, load_library,
     cos_build, cos_build_ex, cos_eval, cos_free, cos_info, cos_last_error, cos_set_workspace_limit,
     cos_tab_build, cos_tabulate, cos_tab_free, cos_measure_fp64_fma_peak,
-    cos_eval_host, cos_set_profiling, cos_get_layer_times, EXPORTS,
+    cos_eval_host, cos_set_profiling, cos_get_layer_times, cos_build_orders, cos_flux_weights, EXPORTS,
     dag_summary,
 )

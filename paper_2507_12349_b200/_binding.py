@@ -18,14 +18,14 @@ COS_BUILD_HOST_ONLY = 1
 INFO = {
     "n_layers": 0, "n_states": 1, "n_edges": 2, "n_readout_edges": 3, "n_out": 4, "max_layer_states": 5,
     "n_masks": 6, "n_rows": 7, "n_fma": 8, "program_bytes": 9, "d": 10, "n_blocks": 11,
-    "n_states_unpruned": 12, "workspace_bytes": 13, "n_launches": 14,
+    "n_states_unpruned": 12, "workspace_bytes": 13, "n_launches": 14, "order_mask": 15,
     "layer_states": 100, "layer_edges": 200, "layer_masks": 300,
 }
 
 EXPORTS = [
     "cos_build", "cos_build_ex", "cos_eval", "cos_free", "cos_set_workspace_limit", "cos_info",
     "cos_last_error", "cos_tab_build", "cos_tabulate", "cos_tab_free", "cos_measure_fp64_fma_peak",
-    "cos_eval_host", "cos_set_profiling", "cos_get_layer_times",
+    "cos_eval_host", "cos_set_profiling", "cos_get_layer_times", "cos_build_orders", "cos_flux_weights",
 ]
 
 
@@ -75,6 +75,10 @@ def load_library():
     lib.cos_set_profiling.argtypes = [vp, ip]
     lib.cos_get_layer_times.restype = ctypes.c_int
     lib.cos_get_layer_times.argtypes = [vp, ip, dp, llp]
+    lib.cos_build_orders.restype = ctypes.c_int
+    lib.cos_build_orders.argtypes = [ip, ip, ip, dp, ctypes.c_uint, ip, ctypes.POINTER(vp)]
+    lib.cos_flux_weights.restype = ctypes.c_int
+    lib.cos_flux_weights.argtypes = [ip, ctypes.c_uint, dp, vp, vp, ctypes.c_longlong, vp, vp, vp]
     lib.cos_measure_fp64_fma_peak.restype = ctypes.c_int
     lib.cos_measure_fp64_fma_peak.argtypes = [dp]
     _lib = lib
@@ -104,6 +108,25 @@ def cos_build_ex(n, n_flavors, lattice, shifts, readout_envelope, flags=0):
     h = ctypes.c_void_p()
     _check(lib.cos_build_ex(int(n), int(n_flavors), int(lattice), p, int(readout_envelope), int(flags), ctypes.byref(h)))
     return h.value
+
+
+def cos_build_orders(n, n_flavors, lattice, shifts, order_mask, flags=0):
+    """All-subset layout restricted to the allowed orders: bit k of order_mask <-> subsets with |S| = k."""
+    lib = load_library()
+    keep, p = _shifts_arg(shifts)
+    h = ctypes.c_void_p()
+    _check(lib.cos_build_orders(int(n), int(n_flavors), int(lattice), p, int(order_mask), int(flags), ctypes.byref(h)))
+    return h.value
+
+
+def cos_flux_weights(n, order_mask, lambdas, C_dev, Q_dev, batch, W_dev, Phi_dev=None, stream=None):
+    """W[c] = sum_{|S| in U} |lambda_|S| C_S Q_S| / binom(n, |S|) (PAPER.md Eq. 6-7).  lambdas: n+1 floats (index = order);
+    C_dev / Q_dev / Phi_dev: torch.float64 CUDA tensors [2^n-1, batch] (Q_dev, Phi_dev may be None); W_dev: [batch]."""
+    lam = (ctypes.c_double * (int(n) + 1))(*[float(x) for x in lambdas])
+    _check(load_library().cos_flux_weights(
+        int(n), int(order_mask), ctypes.cast(lam, ctypes.POINTER(ctypes.c_double)), _dev_ptr(C_dev, "torch.float64"),
+        None if Q_dev is None else _dev_ptr(Q_dev, "torch.float64"), int(batch), _dev_ptr(W_dev, "torch.float64"),
+        None if Phi_dev is None else _dev_ptr(Phi_dev, "torch.float64"), _stream_ptr(stream)))
 
 
 def cos_build(n, n_flavors, lattice, shifts, readout_envelope):
@@ -204,7 +227,7 @@ def cos_measure_fp64_fma_peak():
 def dag_summary(handle):
     """Convenience: the cos_info counters as a dict (host data only)."""
     keys = ["n_layers", "n_states", "n_edges", "n_readout_edges", "n_out", "max_layer_states", "n_masks",
-            "n_rows", "n_fma", "program_bytes", "d", "n_blocks", "n_states_unpruned"]
+            "n_rows", "n_fma", "program_bytes", "d", "n_blocks", "n_states_unpruned", "order_mask"]
     out = {k: cos_info(handle, k) for k in keys}
     nl = out["n_layers"]
     out["layer_states"] = [cos_info(handle, "layer_states", l) for l in range(nl)]

@@ -66,8 +66,27 @@ extern "C" {
 
 const char* cos_last_error(void) { return g_err.c_str(); }
 
+static int build_impl(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope,
+                      unsigned int order_mask, int flags, cos_handle* out);
+
 int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope, int flags,
                  cos_handle* out)
+{
+    return build_impl(n, n_flavors, lattice, shifts, readout_envelope, 0u, flags, out);
+}
+
+int cos_build_orders(int n, int n_flavors, int lattice, const double* shifts, unsigned int order_mask, int flags,
+                     cos_handle* out)
+{
+    if (n >= 1 && n <= COS_MAX_N && (order_mask & ((2u << n) - 2u)) == 0u) {
+        if (out) *out = nullptr;
+        return fail(COS_EINVAL, "cos_build_orders: order_mask selects no order in [1, n]");
+    }
+    return build_impl(n, n_flavors, lattice, shifts, n, order_mask & ((2u << n) - 2u), flags, out);
+}
+
+static int build_impl(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope,
+                      unsigned int order_mask, int flags, cos_handle* out)
 {
     if (!out) return fail(COS_EINVAL, "cos_build: out is NULL");
     *out = nullptr;
@@ -84,7 +103,7 @@ int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int re
 
     cos_handle_s* h = new (std::nothrow) cos_handle_s();
     if (!h) return fail(COS_ENOMEM, "cos_build: out of host memory");
-    std::string err = compile_dag(n, n_flavors, nsub, shifts, readout_envelope == n, h->dag);
+    std::string err = compile_dag(n, n_flavors, nsub, shifts, readout_envelope == n, order_mask, h->dag);
     if (!err.empty()) { delete h; return fail(COS_ENOMEM, "cos_build: " + err); }
 
     const CompiledDag& D = h->dag;
@@ -194,6 +213,10 @@ int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev
     }
     double* slab[2] = {h->ws, h->ws + (size_t)D.max_layer_states * TILE * (size_t)tiles_chunk};
 
+    if (D.all_subsets && D.order_mask != (((2u << D.n) - 1u) & ~1u)) {     // partial readout set: other rows are zeros
+        cudaError_t e = cudaMemsetAsync(out_dev, 0, (size_t)D.n_out * (size_t)batch * sizeof(double), stream);
+        if (e != cudaSuccess) return cuda_fail(e, "cos_eval: clearing the output");
+    }
     if (h->profiling) ++h->profiled_evals;
     for (long long t0 = 0; t0 < tiles_total; t0 += tiles_chunk) {
         const uint32_t tiles = (uint32_t)((tiles_total - t0 < tiles_chunk) ? (tiles_total - t0) : tiles_chunk);
@@ -348,6 +371,7 @@ int cos_info(cos_handle h, int what, long long* value)
         case COS_INFO_N_STATES_UNPRUNED: *value = (long long)D.n_states_unpruned; break;
         case COS_INFO_WORKSPACE_BYTES: *value = (long long)h->ws_bytes; break;
         case COS_INFO_N_LAUNCHES: *value = h->n_launches; break;
+        case COS_INFO_ORDER_MASK: *value = (long long)D.order_mask; break;
         default: return fail(COS_EINVAL, "cos_info: unknown query");
     }
     return COS_OK;
@@ -393,6 +417,28 @@ void cos_tab_free(cos_tab tab)
     if (!tab) return;
     if (tab->T) cudaFree(tab->T);
     delete tab;
+}
+
+int cos_flux_weights(int n, unsigned int order_mask, const double* lambda_host, const double* C_dev,
+                     const double* Q_dev, long long batch, double* W_dev, double* Phi_dev, cos_stream stream)
+{
+    if (n < 1 || n > COS_MAX_N || batch < 0) return fail(COS_EINVAL, "cos_flux_weights: bad argument");
+    if (batch == 0) return COS_OK;
+    if (!lambda_host || !C_dev || !W_dev) return fail(COS_EINVAL, "cos_flux_weights: NULL pointer");
+    FluxArgs a;
+    a.n = n;
+    a.order_mask = order_mask ? (order_mask & ((2u << n) - 2u)) : ((2u << n) - 2u);
+    if (a.order_mask == 0u) return fail(COS_EINVAL, "cos_flux_weights: order_mask selects no order in [1, n]");
+    double b = 1.0;                                   // binom(n, k), exact in fp64 for n <= 12
+    for (int k = 0; k <= 12; ++k) {
+        a.lambda[k] = (k >= 1 && k <= n) ? lambda_host[k] : 0.0;
+        a.binom[k] = (k <= n) ? b : 1.0;
+        if (k < n) b = b * (double)(n - k) / (double)(k + 1);
+    }
+    a.C = C_dev; a.Q = Q_dev; a.W = W_dev; a.Phi = Phi_dev; a.batch = batch;
+    cudaError_t e = launch_flux(a, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "cos_flux_weights: launch");
+    return COS_OK;
 }
 
 int cos_measure_fp64_fma_peak(double* fma_per_s)

@@ -81,7 +81,8 @@ struct Builder {
 
 }  // namespace
 
-std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_subsets, CompiledDag& out)
+std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_subsets, uint32_t order_mask,
+                        CompiledDag& out)
 {
     if (n < 1 || n > 12) return "n must be in [1, 12]";
     if (nsub != 1 && nsub != 2) return "n_sub must be 1 or 2";
@@ -98,7 +99,16 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_s
         b.by_layer.assign(NL, {});
 
         // ---- initial states (Eq. 66; reading G8 for the rooted branches): (r, s) head = endpoint, m = (1,s) e_r
-        for (int r = 0; r < (all_subsets ? n : 1); ++r)
+        // requested subsets (Eq. 24): all-subset mode keeps S with |S| in the allowed orders U (order_mask bit |S|;
+        // 0 = every order); a subset of order k has root r = min S <= n - k, so larger roots are never started
+        if (all_subsets && order_mask == 0) order_mask = ((2u << n) - 1u) & ~1u;
+        int k_min = n;
+        if (all_subsets) { k_min = 1; while (k_min <= n && !((order_mask >> k_min) & 1u)) ++k_min; }
+        if (all_subsets && k_min > n) return "order_mask selects no order in [1, n]";
+        auto requested = [&](uint32_t S) {
+            return all_subsets ? (bool)((order_mask >> __builtin_popcount(S)) & 1u) : S == ((1u << n) - 1u);
+        };
+        for (int r = 0; r < (all_subsets ? n - k_min + 1 : 1); ++r)
             for (int s = 0; s < nsub; ++s) {
                 uint32_t id = b.get_mask((uint32_t)(1 + s) << (2 * r), 0);
                 int a = r * nsub + s;
@@ -139,7 +149,7 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_s
             for (uint32_t id : b.by_layer[l]) {
                 const uint32_t code = b.codes[id];
                 const int jm = b.jmin(code);
-                const bool readout = (jm < 0) && (all_subsets || b.full_set(code) == FULL);
+                const bool readout = (jm < 0) && requested(b.full_set(code));
                 bool fresh_ok = false;
                 if (jm >= 0 && l + 1 < NL) {
                     const int fa = jm * nsub + (Builder::cell(code, jm) - 1);
@@ -166,7 +176,7 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_s
         out = CompiledDag();
         out.n = n; out.nf = nf; out.nsub = nsub; out.d = d; out.nc = nc;
         out.n_blocks = sigma ? nf : 1;
-        out.uniform = (sigma == nullptr); out.all_subsets = all_subsets; out.has_shift = (sigma != nullptr);
+        out.uniform = (sigma == nullptr); out.all_subsets = all_subsets; out.order_mask = all_subsets ? order_mask : 0u; out.has_shift = (sigma != nullptr);
         out.kappa = sigma ? 1.0 : (double)nf;
         out.n_out = all_subsets ? (int)FULL : 1;
         for (int l = 0; l < nc && sigma; ++l) out.sigma[l] = sigma[l];
@@ -212,7 +222,7 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_s
                     fresh_did = b.index_of[code | (3u << (2 * jm))];
                     if (fresh_did >= 0 && ((b.alive[(size_t)fresh_did * d + fresh_a] >> fresh_a) & 1u)) flags |= FLAG_FRESH;
                 }
-                if (jm < 0 && (all_subsets || b.full_set(code) == FULL)) {
+                if (jm < 0 && requested(b.full_set(code))) {
                     flags |= FLAG_READOUT;
                     out_idx = all_subsets ? b.full_set(code) - 1u : 0u;
                 }

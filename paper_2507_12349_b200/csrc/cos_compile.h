@@ -42,6 +42,7 @@ struct LayerProgram {
 struct CompiledDag {
     int n = 0, nf = 0, nsub = 1, d = 0, nc = 1, n_blocks = 1, n_out = 1;
     bool uniform = true, all_subsets = false, has_shift = false;
+    uint32_t order_mask = 0;             // all-subset mode: requested orders (bit k <=> |S| = k)
     double sigma[4] = {0, 0, 0, 0};
     double kappa = 1.0;
     std::vector<LayerProgram> layers;    // 2n layers; layer l holds the transitions l -> l+1 and the readouts at l
@@ -51,6 +52,8 @@ struct CompiledDag {
 };
 
 // Returns "" on success, else an error message.  n in [1,12]; nsub in {1,2}; sigma == nullptr -> uniform.
-std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_subsets, CompiledDag& out);
+// order_mask (all_subsets only): bit k set <=> subsets of order k are requested outputs (0 = every order).
+std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_subsets, uint32_t order_mask,
+                        CompiledDag& out);
 
 }  // namespace cosb

@@ -442,6 +442,37 @@ cudaError_t launch_tabulate(const TabArgs& a, cudaStream_t stream)
 }
 
 // ------------------------------------------------------------------------------------------------------
+// Many-configuration heat-bath weights (Eq. 6-7): one thread per configuration, subsets in increasing
+// bitmask order, rounding order fixed (no contraction: products, one division and one addition per subset).
+__global__ void cos_flux_kernel(const FluxArgs a)
+{
+    const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= a.batch) return;
+    const uint32_t n_sub = (1u << a.n) - 1u;
+    double W = 0.0;
+    for (uint32_t S = 1; S <= n_sub; ++S) {
+        const int k = __popc(S);
+        const size_t idx = (size_t)(S - 1u) * (size_t)a.batch + (size_t)c;
+        if (!((a.order_mask >> k) & 1u)) {
+            if (a.Phi) a.Phi[idx] = 0.0;
+            continue;
+        }
+        double phi = __dmul_rn(a.lambda[k], __ldg(a.C + idx));
+        if (a.Q) phi = __dmul_rn(phi, __ldg(a.Q + idx));
+        if (a.Phi) a.Phi[idx] = phi;
+        W = __dadd_rn(W, __ddiv_rn(fabs(phi), a.binom[k]));
+    }
+    a.W[c] = W;
+}
+
+cudaError_t launch_flux(const FluxArgs& a, cudaStream_t stream)
+{
+    if (a.batch == 0) return cudaSuccess;
+    cos_flux_kernel<<<(unsigned)((a.batch + 127) / 128), 128, 0, stream>>>(a);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------
 __global__ void cos_fp64_peak_kernel(double* sink, int iters, double a0, double b0)
 {
     double acc[8];

@@ -45,6 +45,12 @@ struct TabArgs {
 };
 cudaError_t launch_tabulate(const TabArgs& a, cudaStream_t stream);
 
+struct FluxArgs {
+    int n; uint32_t order_mask; double lambda[13], binom[13];
+    const double* C; const double* Q; double* W; double* Phi; long long batch;
+};
+cudaError_t launch_flux(const FluxArgs& a, cudaStream_t stream);
+
 cudaError_t measure_fp64_fma(double* fma_per_s);
 
 }  // namespace cosb
