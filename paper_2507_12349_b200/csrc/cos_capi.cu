@@ -45,6 +45,8 @@ struct cos_handle_s {
     long long ws_limit = 64ll << 30;
     int masks_per_cta = 0;
     int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148, prefetch = 0, ring = 0, pdl = 1;
+    bool fused = false;                   // small DAG: every layer in one launch (cos_fused_kernel)
+    FusedLayer* fused_layers = nullptr;   // device array
     long long n_launches = 0;
     // profiling (cos_set_profiling): events[k*(NL+1) + l] brackets layer l of the k-th profiled chunk
     bool profiling = false;
@@ -150,6 +152,21 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
             if (e != cudaSuccess) { cos_free(h); return cuda_fail(e, "cos_build: uploading the layer program"); }
             h->program_bytes += wb + mb;
         }
+        // small DAGs (orders n <= 6) are launch-latency bound: walk all layers in one kernel
+        bool small = D.n_states <= 16384 && D.max_L <= 12 && env_int("COS_FUSED", 1) != 0;
+        for (const auto& P : D.layers) small = small && P.n_masks <= 2048;
+        if (small) {
+            e = configure_fused_kernels();
+            std::vector<FusedLayer> fl(D.layers.size());
+            for (size_t l = 0; l < D.layers.size(); ++l) {
+                fl[l].words = h->dl[l].words; fl[l].mask_off = h->dl[l].mask_off;
+                fl[l].n_masks = D.layers[l].n_masks; fl[l].n_states = D.layers[l].n_states;
+            }
+            if (e == cudaSuccess) e = cudaMalloc(&h->fused_layers, fl.size() * sizeof(FusedLayer));
+            if (e == cudaSuccess) e = cudaMemcpy(h->fused_layers, fl.data(), fl.size() * sizeof(FusedLayer), cudaMemcpyHostToDevice);
+            if (e != cudaSuccess) { cos_free(h); return cuda_fail(e, "cos_build: fused-path setup"); }
+            h->fused = true;
+        }
         h->on_device = true;
         // the host copy of the program is no longer needed
         for (auto& P : h->dag.layers) { std::vector<uint32_t>().swap(P.words); std::vector<uint32_t>().swap(P.mask_off); }
@@ -170,6 +187,7 @@ void cos_free(cos_handle h)
     if (!h) return;
     for (auto& l : h->dl) { if (l.words) cudaFree(l.words); if (l.mask_off) cudaFree(l.mask_off); }
     if (h->ws) cudaFree(h->ws);
+    if (h->fused_layers) cudaFree(h->fused_layers);
     for (cudaEvent_t e : h->events) cudaEventDestroy(e);
     if (h->st_sites) cudaFree(h->st_sites);
     if (h->st_tau) cudaFree(h->st_tau);
@@ -220,6 +238,17 @@ int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev
     if (h->profiling) ++h->profiled_evals;
     for (long long t0 = 0; t0 < tiles_total; t0 += tiles_chunk) {
         const uint32_t tiles = (uint32_t)((tiles_total - t0 < tiles_chunk) ? (tiles_total - t0) : tiles_chunk);
+        if (h->fused && !h->profiling) {
+            FusedArgs f;
+            f.layers = h->fused_layers; f.n_layers = NL; f.ws = h->ws; f.S_max = D.max_layer_states;
+            f.G = G_dev; f.batch = batch; f.b0 = t0 * TILE; f.out = out_dev; f.d = D.d; f.n_slots = D.n_blocks * D.d * D.d;
+            f.neg_kappa = -D.kappa;
+            for (int c = 0; c < 4; ++c) f.sigma[c] = D.sigma[c];
+            cudaError_t ef = launch_fused(f, (int)D.max_L, D.nc, D.has_shift, tiles, 8, stream);
+            if (ef != cudaSuccess) return cuda_fail(ef, "cos_eval: fused launch");
+            ++h->n_launches;
+            continue;
+        }
         cudaError_t e = launch_fill_ones(slab[0], (size_t)D.layers[0].n_states * TILE * tiles, stream);
         if (e != cudaSuccess) return cuda_fail(e, "cos_eval: fill launch");
         ++h->n_launches;

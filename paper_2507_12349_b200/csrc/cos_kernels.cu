@@ -51,7 +51,7 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 //   RING = 0 the L source values are loaded from global memory (xp);
 //   RING > 0 they were copied ahead of time into this warp's shared-memory ring (ring_lane, stream position o)
 // Inner loop per DAG edge: one integer add (address), one LDS.64, one DFMA.
-template <int L, int NC, bool SHIFT, int RING>
+template <int L, int NC, bool SHIFT, int RING, bool FUSED>
 __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, const double* __restrict__ xp,
                                          const uint32_t ring_lane, const uint32_t o,
                                          const int nJ, const int e_words, const bool need_close,
@@ -65,7 +65,7 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
         for (int k = 0; k < L; ++k) x[k] = lds64(ring_lane + (((o + (uint32_t)k) & (uint32_t)(RING - 1)) << 8));
     } else {
 #pragma unroll
-        for (int k = 0; k < L; ++k) x[k] = __ldcs(xp + (size_t)k * TILE);
+        for (int k = 0; k < L; ++k) x[k] = FUSED ? __ldcg(xp + (size_t)k * TILE) : __ldcs(xp + (size_t)k * TILE);
     }
     const uint32_t dstride = d * (TILE * 8u);
 #pragma unroll
@@ -108,51 +108,15 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
     }
 }
 
-template <int MAXL, int NC, bool SHIFT, int RING>
-__global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(const LayerArgs a)
+// All source blocks [m_begin, m_end) of one layer for one batch tile: the body shared by the per-layer kernel and the
+// fused small-DAG kernel.  s_next (shared) must be 0 and visible to the CTA on entry.
+template <int MAXL, int NC, bool SHIFT, int RING, bool FUSED>
+__device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t m_begin, const uint32_t m_end,
+                                             const uint32_t tile, unsigned int& s_next, const uint32_t gs_lane,
+                                             const uint32_t gd_lane, const uint32_t ring_lane, const int lane,
+                                             const bool valid, const long long b)
 {
-    extern __shared__ __align__(128) double Gs[];
-    __shared__ unsigned int s_next;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
-    const uint32_t tile = blockIdx.x;
     const int HDR = 3 + NC;
-
-    const uint32_t gs_lane = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)lane * 8u;
-    const uint32_t gd_lane = gs_lane + (uint32_t)a.n_slots * (TILE * 8u);
-    const uint32_t n_tab = (uint32_t)a.n_slots + (SHIFT ? (uint32_t)(NC * a.d) : 0u);
-    const uint32_t ring_lane = gs_lane + (n_tab + (uint32_t)warp * (uint32_t)(RING > 0 ? RING : 0)) * (TILE * 8u);
-
-    // Programmatic dependent launch: let the next layer's grid start (it only stages its table, which no layer
-    // writes) while this grid drains; this grid in turn touches the slabs only after the previous one has completed.
-    if (a.pdl) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
-    // ---- stage the tile's propagator table Gs[slot][lane] with asynchronous copies (all in flight at once)
-    const long long b = a.b0 + (long long)tile * TILE + lane;
-    const bool valid = b < a.batch;
-    if (threadIdx.x == 0) s_next = 0u;
-    for (int s = warp; s < a.n_slots; s += W) {
-        if (valid) cp_async8(gs_lane + (uint32_t)s * (TILE * 8u), a.G + (size_t)s * (size_t)a.batch + (size_t)b);
-        else Gs[s * TILE + lane] = 0.0;
-    }
-    cp_async_commit();
-    cp_async_wait<0>();
-    __syncthreads();
-    if (SHIFT) {
-        // continuation into the partner of the current endpoint (E2 with j = e) always comes with the
-        // counterterm one-cycle E3 at the same destination: fold c3*sigma_lam into the diagonal of the
-        // staged table (Eq. 49 / 72, 77) and keep the plain diagonal for the cycle-closing factor.
-        for (int q = warp; q < NC * a.d; q += W) {
-            const int lam = q / a.d, e = q - lam * a.d;
-            const double sh = lam == 0 ? a.shift[0] : lam == 1 ? a.shift[1] : lam == 2 ? a.shift[2] : a.shift[3];
-            const double g = Gs[((lam * a.d + e) * a.d + e) * TILE + lane];
-            Gs[(a.n_slots + q) * TILE + lane] = g;
-            Gs[((lam * a.d + e) * a.d + e) * TILE + lane] = g + sh;
-        }
-        __syncthreads();
-    }
-
-    if (a.pdl) asm volatile("griddepcontrol.wait;" ::: "memory");
-    const uint32_t m_begin = blockIdx.y * a.masks_per_cta;
-    const uint32_t m_end = min(a.n_masks, m_begin + a.masks_per_cta);
     const double* Xt = a.X + (size_t)tile * a.S_src * TILE + lane;
     const char* Xt0 = (const char*)(a.X + (size_t)tile * a.S_src * TILE);
     double* Yt = a.Y + (size_t)tile * a.S_dst * TILE + lane;
@@ -236,8 +200,9 @@ __global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(cons
 #define COS_ROW_CASE(LL)                                                                                        \
     case LL:                                                                                                    \
         if (LL <= MAXL)                                                                                         \
-            row_body<(LL <= MAXL ? LL : 1), NC, SHIFT, RING>(rw, rh, xp, ring_lane, o, nJ, e_words, need_close, \
-                                                             (uint32_t)a.d, gs_lane, gd_lane, Yt, close, sp);   \
+            row_body<(LL <= MAXL ? LL : 1), NC, SHIFT, RING, FUSED>(rw, rh, xp, ring_lane, o, nJ, e_words,     \
+                                                                    need_close, (uint32_t)a.d, gs_lane, gd_lane, \
+                                                                    Yt, close, sp);                              \
         break;
             switch (L) {
                 COS_ROW_CASE(1) COS_ROW_CASE(2) COS_ROW_CASE(3) COS_ROW_CASE(4) COS_ROW_CASE(5) COS_ROW_CASE(6)
@@ -263,6 +228,112 @@ __global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(cons
         mi = mi_n; off = off_n; hw = hw_n; rw = rw_n;
     }
     if (RING > 0) cp_async_wait<0>();
+}
+
+template <int MAXL, int NC, bool SHIFT, int RING>
+__global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(const LayerArgs a)
+{
+    extern __shared__ __align__(128) double Gs[];
+    __shared__ unsigned int s_next;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
+    const uint32_t tile = blockIdx.x;
+
+    const uint32_t gs_lane = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)lane * 8u;
+    const uint32_t gd_lane = gs_lane + (uint32_t)a.n_slots * (TILE * 8u);
+    const uint32_t n_tab = (uint32_t)a.n_slots + (SHIFT ? (uint32_t)(NC * a.d) : 0u);
+    const uint32_t ring_lane = gs_lane + (n_tab + (uint32_t)warp * (uint32_t)(RING > 0 ? RING : 0)) * (TILE * 8u);
+
+    // Programmatic dependent launch: let the next layer's grid start (it only stages its table, which no layer
+    // writes) while this grid drains; this grid in turn touches the slabs only after the previous one has completed.
+    if (a.pdl) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");
+    // ---- stage the tile's propagator table Gs[slot][lane] with asynchronous copies (all in flight at once)
+    const long long b = a.b0 + (long long)tile * TILE + lane;
+    const bool valid = b < a.batch;
+    if (threadIdx.x == 0) s_next = 0u;
+    for (int s = warp; s < a.n_slots; s += W) {
+        if (valid) cp_async8(gs_lane + (uint32_t)s * (TILE * 8u), a.G + (size_t)s * (size_t)a.batch + (size_t)b);
+        else Gs[s * TILE + lane] = 0.0;
+    }
+    cp_async_commit();
+    cp_async_wait<0>();
+    __syncthreads();
+    if (SHIFT) {
+        // continuation into the partner of the current endpoint (E2 with j = e) always comes with the
+        // counterterm one-cycle E3 at the same destination: fold c3*sigma_lam into the diagonal of the
+        // staged table (Eq. 49 / 72, 77) and keep the plain diagonal for the cycle-closing factor.
+        for (int q = warp; q < NC * a.d; q += W) {
+            const int lam = q / a.d, e = q - lam * a.d;
+            const double sh = lam == 0 ? a.shift[0] : lam == 1 ? a.shift[1] : lam == 2 ? a.shift[2] : a.shift[3];
+            const double g = Gs[((lam * a.d + e) * a.d + e) * TILE + lane];
+            Gs[(a.n_slots + q) * TILE + lane] = g;
+            Gs[((lam * a.d + e) * a.d + e) * TILE + lane] = g + sh;
+        }
+        __syncthreads();
+    }
+
+    if (a.pdl) asm volatile("griddepcontrol.wait;" ::: "memory");
+    const uint32_t m_begin = blockIdx.y * a.masks_per_cta;
+    const uint32_t m_end = min(a.n_masks, m_begin + a.masks_per_cta);
+    layer_blocks<MAXL, NC, SHIFT, RING, false>(a, m_begin, m_end, tile, s_next, gs_lane, gd_lane, ring_lane, lane, valid, b);
+}
+
+// ------------------------------------------------------------------------------------------------------
+// Fused small-DAG kernel: ONE launch walks every layer.  A batch tile's states are touched by one CTA only, so the
+// layers of a tile need nothing stronger than __syncthreads between them: grid = batch tiles, the CTA stages the table
+// once, writes the layer-0 states (Eq. 66) itself and ping-pongs between two slabs of S_max states per tile (L2-resident;
+// source rows are read with ld.global.cg so that no stale L1 line of the slab written two layers earlier is seen).
+// Used when every layer is small (launch latency, not bandwidth, decides: orders n <= 6).
+template <int MAXL, int NC, bool SHIFT>
+__global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedArgs f)
+{
+    extern __shared__ __align__(128) double Gs[];
+    __shared__ unsigned int s_next;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
+    const uint32_t tile = blockIdx.x;
+    const uint32_t gs_lane = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)lane * 8u;
+    const uint32_t gd_lane = gs_lane + (uint32_t)f.n_slots * (TILE * 8u);
+    const long long b = f.b0 + (long long)tile * TILE + lane;
+    const bool valid = b < f.batch;
+    if (threadIdx.x == 0) s_next = 0u;
+    for (int s = warp; s < f.n_slots; s += W) {
+        if (valid) cp_async8(gs_lane + (uint32_t)s * (TILE * 8u), f.G + (size_t)s * (size_t)f.batch + (size_t)b);
+        else Gs[s * TILE + lane] = 0.0;
+    }
+    cp_async_commit();
+    double* slab0 = f.ws + (size_t)tile * f.S_max * TILE;
+    double* slab1 = f.ws + ((size_t)gridDim.x + tile) * f.S_max * TILE;
+    for (uint32_t s = warp; s < f.layers[0].n_states; s += W) slab0[(size_t)s * TILE + lane] = 1.0;   // Eq. 66
+    cp_async_wait<0>();
+    __syncthreads();
+    if (SHIFT) {       // keep the plain diagonal (cycle closing); the shifted one is rewritten per layer below
+        for (int q = warp; q < NC * f.d; q += W) {
+            const int lam = q / f.d, e = q - lam * f.d;
+            Gs[(f.n_slots + q) * TILE + lane] = Gs[((lam * f.d + e) * f.d + e) * TILE + lane];
+        }
+        __syncthreads();
+    }
+    LayerArgs a;
+    a.G = f.G; a.batch = f.batch; a.b0 = f.b0; a.out = f.out; a.d = f.d; a.n_slots = f.n_slots;
+    a.neg_kappa = f.neg_kappa; a.prefetch = 0; a.pdl = 0; a.S_src = f.S_max; a.S_dst = f.S_max; a.masks_per_cta = 0;
+    for (int l = 0; l < f.n_layers; ++l) {
+        if (SHIFT && l <= 1) {               // c3 = -2 at layer 0, -1 afterwards (Eq. 72, 77)
+            for (int q = warp; q < NC * f.d; q += W) {
+                const int lam = q / f.d, e = q - lam * f.d;
+                const double sg = lam == 0 ? f.sigma[0] : lam == 1 ? f.sigma[1] : lam == 2 ? f.sigma[2] : f.sigma[3];
+                Gs[((lam * f.d + e) * f.d + e) * TILE + lane] = Gs[(f.n_slots + q) * TILE + lane] + (l == 0 ? -2.0 : -1.0) * sg;
+            }
+            __syncthreads();
+        }
+        const FusedLayer fl = f.layers[l];
+        a.words = fl.words; a.mask_off = fl.mask_off; a.n_masks = fl.n_masks;
+        a.X = (l & 1) ? slab1 : slab0; a.Y = (l & 1) ? slab0 : slab1;
+        // slabs are addressed per tile already: tile index 0 inside layer_blocks
+        layer_blocks<MAXL, NC, SHIFT, 0, true>(a, 0u, fl.n_masks, 0u, s_next, gs_lane, gd_lane, 0u, lane, valid, b);
+        __threadfence_block();
+        __syncthreads();
+        if (threadIdx.x == 0) s_next = 0u;
+        __syncthreads();
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -380,6 +451,58 @@ cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, int 
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
     return cudaLaunchKernelEx(&cfg, fn, a);
+}
+
+typedef void (*fused_fn)(const FusedArgs);
+template <int MAXL>
+static fused_fn pick_fused_nc(int nc, bool shift)
+{
+    if (!shift) {
+        switch (nc) {
+            case 1: return cos_fused_kernel<MAXL, 1, false>;
+            case 2: return cos_fused_kernel<MAXL, 2, false>;
+            case 3: return cos_fused_kernel<MAXL, 3, false>;
+            default: return cos_fused_kernel<MAXL, 4, false>;
+        }
+    }
+    switch (nc) {
+        case 1: return cos_fused_kernel<MAXL, 1, true>;
+        case 2: return cos_fused_kernel<MAXL, 2, true>;
+        case 3: return cos_fused_kernel<MAXL, 3, true>;
+        default: return cos_fused_kernel<MAXL, 4, true>;
+    }
+}
+static fused_fn pick_fused_fn(int max_L, int nc, bool shift)
+{
+    if (max_L <= 4) return pick_fused_nc<4>(nc, shift);
+    if (max_L <= 8) return pick_fused_nc<8>(nc, shift);
+    if (max_L <= 12) return pick_fused_nc<12>(nc, shift);
+    return nullptr;
+}
+
+cudaError_t configure_fused_kernels()
+{
+    static const int Ls[3] = {4, 8, 12};
+    for (int i = 0; i < 3; ++i)
+        for (int nc = 1; nc <= 4; ++nc)
+            for (int sh = 0; sh < 2; ++sh) {
+                cudaError_t e = cudaFuncSetAttribute((const void*)pick_fused_fn(Ls[i], nc, sh != 0),
+                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LAYER_SMEM_MAX);
+                if (e != cudaSuccess) return e;
+            }
+    return cudaSuccess;
+}
+
+cudaError_t launch_fused(const FusedArgs& f, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
+                         cudaStream_t stream)
+{
+    if (tiles == 0) return cudaSuccess;
+    fused_fn fn = pick_fused_fn(max_L, nc, shift);
+    if (!fn) return cudaErrorInvalidConfiguration;
+    if (warps_per_cta > MAX_WARPS) warps_per_cta = MAX_WARPS;
+    const size_t smem = layer_smem_bytes(f.n_slots, nc, f.d, shift, 0, 0);
+    fn<<<tiles, 32 * warps_per_cta, smem, stream>>>(f);
+    return cudaGetLastError();
 }
 
 // ------------------------------------------------------------------------------------------------------

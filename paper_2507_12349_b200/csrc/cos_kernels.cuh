@@ -37,6 +37,22 @@ size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift, int ring, int wa
 cudaError_t pick_layer_shape(int max_L, int nc, int d, int n_slots, bool shift, int want_ring, int* ring,
                              int* warps_per_cta, int* ctas_per_sm);
 
+// ---- fused small-DAG path: every layer in one launch (cos_fused_kernel)
+struct FusedLayer { const uint32_t* words; const uint32_t* mask_off; uint32_t n_masks, n_states; };
+struct FusedArgs {
+    const FusedLayer* layers;            // device array [n_layers]
+    int n_layers;
+    double* ws;                          // two slabs [2][tiles][S_max][32]
+    uint32_t S_max;
+    const double* G; long long batch, b0; double* out;
+    int d, n_slots;
+    double neg_kappa;
+    double sigma[4];
+};
+cudaError_t configure_fused_kernels();
+cudaError_t launch_fused(const FusedArgs& f, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
+                         cudaStream_t stream);
+
 cudaError_t launch_fill_ones(double* X, size_t n_doubles, cudaStream_t stream);
 
 struct TabArgs {

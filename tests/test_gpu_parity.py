@@ -381,3 +381,20 @@ def test_config3_reduced_batch(cos):
         Gc = np.ascontiguousarray(G[:, c].cpu().numpy().reshape(2, w.d, w.d))
         ref = oracle.connected_reference(Gc, w.n, 2, 2, w.sigmas, False, False, tier="o2a")[0]
         check(got[0, c], ref, M_lower_bound(Gc, w.n, 2, 2, False, n_assign=4, seed=c), ("cfg3", c))
+
+
+@pytest.mark.parametrize("n,nf,lattice,sb,all_subsets", [(4, 2, 0, False, False), (5, 3, 0, True, True),
+                                                          (3, 2, 1, True, True), (6, 3, 0, True, False)])
+def test_fused_and_layered_paths_agree(cos, n, nf, lattice, sb, all_subsets, monkeypatch):
+    """Small DAGs run in ONE launch (cos_fused_kernel); COS_FUSED=0 forces the per-layer kernels.  Both walk the same
+    program with the same arithmetic order, so the outputs must be bit-identical (and equal the oracle, tested above)."""
+    n_sub = 2 if lattice else 1
+    sig = [0.3, -0.2, 0.1][:nf] if sb else None
+    G = random_matrices(50 + n, nf if sb else 1, n * n_sub, 77, scale=0.5)
+    monkeypatch.setenv("COS_FUSED", "1")
+    a = gpu_eval(cos, G, n, nf, lattice, sig, all_subsets)
+    a_chunked = gpu_eval(cos, G, n, nf, lattice, sig, all_subsets, ws_limit=1)      # one tile per chunk
+    monkeypatch.setenv("COS_FUSED", "0")
+    b = gpu_eval(cos, G, n, nf, lattice, sig, all_subsets)
+    assert np.all(np.isfinite(a))
+    assert np.array_equal(a, b) and np.array_equal(a, a_chunked)
