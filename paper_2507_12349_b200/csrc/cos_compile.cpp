@@ -201,7 +201,7 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_s
                     b.row_base[(size_t)id * d + h] = (uint32_t)counter;
                     counter += (uint64_t)__builtin_popcount(a) * nc;
                 }
-            if (counter >= DIDX_DEFER) return "layer too large for the 26-bit destination index";
+            if (counter >= DIDX_DEAD) return "layer too large for the 24-bit destination index";
             out.layers[l].n_states = (uint32_t)counter;
             out.layers[l].n_masks = (uint32_t)ids.size();
         }
@@ -243,7 +243,9 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_s
                     P.mask_off.push_back(first);
                 }
                 P.words.push_back(n_rows | ((uint32_t)nJ << 16) | (flags << 24));
-                P.words.push_back(stride | (e_words << 8) | (fresh_a << 16));
+                // bits 24..: |S| - 1 of a readout block (the deferred multiplicity 2^(|S|-1), see cos_compile.h)
+                const uint32_t sexp = (flags & FLAG_READOUT) ? (uint32_t)__builtin_popcount(b.full_set(code)) - 1u : 0u;
+                P.words.push_back(stride | (e_words << 8) | (fresh_a << 16) | (sexp << 24));
                 P.words.push_back(out_idx);
                 for (int lam = 0; lam < nc; ++lam)
                     P.words.push_back((flags & FLAG_FRESH) ? b.state_index((uint32_t)fresh_did, (int)fresh_a, lam, (int)fresh_a)
@@ -255,34 +257,38 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool all_s
                     if (!a) continue;
                     const uint32_t L = (uint32_t)__builtin_popcount(a);
                     for (int lam = 0; lam < nc; ++lam) {
-                        const size_t w_begin = P.words.size();
                         P.words.push_back(b.row_base[(size_t)id * d + h] + (uint32_t)lam * L);
-                        const uint32_t kh = ((a >> h) & 1u) ? (uint32_t)__builtin_popcount(a & ((1u << h) - 1u)) : 0xFFu;
-                        P.words.push_back(L | ((uint32_t)h << 8) | ((uint32_t)lam << 16) | (kh << 24));
+                        const uint32_t kh = ((a >> h) & 1u) ? (uint32_t)__builtin_popcount(a & ((1u << h) - 1u)) : 31u;
+                        const size_t w_hdr = P.words.size();
+                        P.words.push_back(0u);           // w1, filled below
                         uint32_t packed[6] = {0, 0, 0, 0, 0, 0};
                         int k = 0;
                         for (int e = 0; e < d; ++e)      // byte = lam*d + e_a: row index of G_lam[e_a][.] in the staged table
                             if ((a >> e) & 1u) { packed[k / 4] |= (uint32_t)(lam * d + e) << (8 * (k % 4)); ++k; }
                         for (uint32_t w = 0; w < e_words; ++w) P.words.push_back(packed[w]);
-                        uint32_t alive_j = 0;
+                        // live destinations only (pruned ones are dropped), the merged E2/E4 destination last
+                        uint32_t n_live = 0, defer_word = 0, has_defer = 0;
                         for (int q = 0; q < nJ; ++q) {
-                            uint32_t didx = DIDX_DEAD;
                             const bool live = dest[q] >= 0 && ((b.alive[(size_t)dest[q] * d + h] >> J[q].j_a) & 1u);
-                            if (live) {
-                                ++alive_j;
-                                if ((flags & FLAG_FRESH) && (uint32_t)h == fresh_a && J[q].j_a == fresh_a) didx = DIDX_DEFER;
-                                else didx = b.state_index((uint32_t)dest[q], h, lam, J[q].j_a);
-                                if (J[q].mult2) P.e1 += L; else P.e2 += L;
+                            if (!live) continue;
+                            if (J[q].mult2) P.e1 += L; else P.e2 += L;
+                            if ((flags & FLAG_FRESH) && (uint32_t)h == fresh_a && J[q].j_a == fresh_a) {
+                                has_defer = 1; defer_word = (uint32_t)J[q].j_a << 24;
+                                continue;
                             }
-                            P.words.push_back(didx | ((uint32_t)J[q].j_a << 26) | ((uint32_t)J[q].mult2 << 31));
+                            P.words.push_back(b.state_index((uint32_t)dest[q], h, lam, J[q].j_a) | ((uint32_t)J[q].j_a << 24));
+                            ++n_live;
                         }
+                        if (has_defer) P.words.push_back(defer_word);
+                        for (uint32_t q = n_live + has_defer; q < (uint32_t)nJ; ++q) P.words.push_back(0u);
+                        P.words[w_hdr] = L | ((uint32_t)h << 5) | ((uint32_t)lam << 10) | (kh << 12) | (n_live << 17) | (has_defer << 22);
+                        const uint32_t alive_j = n_live + has_defer;
                         if (b.has_shift && l + 1 < NL)      // E3: states whose current interaction is singly occupied
                             for (int e = 0; e < d; ++e)
                                 if (((a >> e) & 1u)) { int c = Builder::cell(code, e / nsub); if (c == 1 || c == 2) P.e3 += 1; }
                         if (flags & FLAG_FRESH) P.e4 += (uint64_t)L * nc;
                         if (flags & FLAG_READOUT) P.readout_edges += L;
                         P.n_fma += (uint64_t)L * (alive_j + (need_close ? 1u : 0u));
-                        (void)w_begin;
                     }
                 }
                 P.n_rows += n_rows;

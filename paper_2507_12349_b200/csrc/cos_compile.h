@@ -17,19 +17,23 @@ namespace cosb {
 // block header (HDR_WORDS = 3 + nc words):
 //   w0 : n_rows[0:16) | nJ[16:24) | flags[24:32)        flags: bit0 FRESH (close-and-open target alive),
 //                                                               bit1 READOUT (terminal readout, Eq. 14-15)
-//   w1 : row_stride[0:8) | e_words[8:16) | fresh_a[16:24)
+//   w1 : row_stride[0:8) | e_words[8:16) | fresh_a[16:24) | (|S| - 1)[24:32) of a readout block
 //   w2 : out_idx (readout row of out_dev)
 //   w3..w3+nc-1 : destination state index (next layer) of the fresh-head state of colour lambda'
 // row (row_stride = 2 + e_words + nJ words):
 //   w0 : index of the row's first state in this layer's slab (row states are contiguous)
-//   w1 : L[0:8) | h_a[8:16) | lambda[16:24) | k_h[24:32)   k_h = position of the state with e_a == h_a in the
-//        row (0xFF: none); its cycle-closing factor G[h][h] must not carry the counterterm
+//   w1 : L[0:5) | h_a[5:10) | lambda[10:12) | k_h[12:17) | n_live[17:22) | defer[22]
+//        k_h = position of the state with e_a == h_a in the row (31: none); its cycle-closing factor G[h][h] must
+//        not carry the counterterm.  n_live = destinations that follow; defer = one more
+//        destination word after them whose value merges with the fresh-head state (coalesced E2/E4 pair)
 //   w2.. : lambda*d + e_a of the L states, one byte each (row of G_lambda[e_a][.] in the staged table)
-//   then nJ words: dj = didx[0:26) | j_a[26:31) | mult2[31]   (destination index in the next layer,
-//        destination endpoint, multiplicity 2 - m_j of Lemma 7 as a flag)
-static const uint32_t DIDX_MASK = 0x03FFFFFFu;
-static const uint32_t DIDX_DEAD = 0x03FFFFFFu;     // destination pruned (Eq. 23)
-static const uint32_t DIDX_DEFER = 0x03FFFFFEu;    // merges with the fresh-head state (coalesced E2/E4 pair)
+//   then n_live (+ defer) words: dj = didx[0:24) | j_a[24:29)  (destination index in the next layer, destination
+//        endpoint); pruned destinations (Eq. 23) are not listed; the row is padded to the block's common stride.
+// The multiplicity 2 - m_j = 2 of a continuation into an untouched interaction (Lemma 7) is NOT applied per edge:
+// every path into a state of mask m has taken exactly nz(m) - 1 such edges (nz = interactions with m_i >= 1; the root
+// enters with factor 1), so the slabs hold x / 2^(nz(m)-1) and a readout of subset S is scaled by 2^(|S|-1), exactly.
+static const uint32_t DIDX_MASK = 0x00FFFFFFu;
+static const uint32_t DIDX_DEAD = 0x00FFFFFFu;     // fresh-head destination pruned (block header only)
 static const uint32_t FLAG_FRESH = 1u, FLAG_READOUT = 2u;
 
 struct LayerProgram {

@@ -24,7 +24,7 @@ namespace cosb {
 static const int MAX_WARPS = 16;
 // CTA size bound per instantiation: the long-row kernels (honeycomb, d = 20) are shared-memory limited to one CTA
 // per SM, so they take 24 warps (<= 85 registers) instead of 16.
-__host__ __device__ constexpr int max_warps_of(int maxl) { return maxl == 20 ? 24 : MAX_WARPS; }
+__host__ __device__ constexpr int max_warps_of(int maxl) { return maxl == 20 ? 20 : MAX_WARPS; }
 
 __device__ __forceinline__ double lds64(uint32_t addr)
 {
@@ -73,10 +73,10 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
         const uint32_t ew = __shfl_sync(0xFFFFFFFFu, rw, 2 + (k >> 2));
         ra[k] = ((ew >> (8 * (k & 3))) & 0xFFu) * dstride + gs_lane;
     }
-    const int lam = (int)((rh >> 16) & 0xFFu);
+    const int lam = (int)((rh >> 10) & 3u);
     if (need_close) {                       // cycle-closing factor G_lam[e][h] (Eq. 12, 15), never shifted
-        const uint32_t h_a = (rh >> 8) & 0xFFu, hoff = h_a * (TILE * 8u);
-        const int kh = (int)(rh >> 24);
+        const uint32_t h_a = (rh >> 5) & 31u, hoff = h_a * (TILE * 8u);
+        const int kh = (int)((rh >> 12) & 31u);
         const uint32_t pd = gd_lane + ((uint32_t)lam * d + h_a) * (TILE * 8u);
         double c0 = 0.0, c1 = 0.0;
 #pragma unroll
@@ -87,23 +87,24 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
         }
         close += c0 + c1;
     }
-    for (int jj = 0; jj < nJ; ++jj) {
+    // destinations: n_live ordinary ones, then (defer) the one that merges with the fresh-head state.  No per-edge
+    // multiplicity (deferred to the readout, cos_compile.h), no pruned entries: SHFL, L x (LDS, DFMA), one store.
+    const int n_live = (int)((rh >> 17) & 31u), n_tot = n_live + (int)((rh >> 22) & 1u);
+    char* const Yb = (char*)Yt;
+    for (int jj = 0; jj < n_tot; ++jj) {
         const uint32_t dj = __shfl_sync(0xFFFFFFFFu, rw, 2 + e_words + jj);
-        const uint32_t didx = dj & DIDX_MASK;
-        if (didx == DIDX_DEAD) continue;
-        const uint32_t joff = (dj >> 18) & 0x1F00u;              // j_a * 256 bytes
+        const uint32_t joff = __byte_perm(dj, 0u, 0x4434u);      // j_a * 256 bytes (j_a is the top byte of dj)
         double acc0 = 0.0, acc1 = 0.0;
 #pragma unroll
         for (int k = 0; k < L; ++k) {
             if (k & 1) acc1 = fma(lds64(ra[k] + joff), x[k], acc1); else acc0 = fma(lds64(ra[k] + joff), x[k], acc0);
         }
-        double acc = acc0 + acc1;
-        if (dj >> 31) acc += acc;                                // multiplicity 2 - m_j (Lemma 7)
-        if (didx == DIDX_DEFER) {
+        const double acc = acc0 + acc1;
+        if (jj < n_live) {
+            __stcs((double*)(Yb + (size_t)(dj << 8)), acc);      // didx * 256 bytes: didx < 2^24, the shift drops j_a
+        } else {
 #pragma unroll
             for (int c = 0; c < NC; ++c) sp[c] = (c == lam) ? acc : sp[c];
-        } else {
-            __stcs(Yt + (size_t)didx * TILE, acc);
         }
     }
 }
@@ -174,7 +175,7 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
             uint32_t rw_next = 0u;
             if (r + 1 < n_rows) rw_next = __ldg(rp + (size_t)(r + 1) * stride + lane);
             const uint32_t base = __shfl_sync(0xFFFFFFFFu, rw, 0), rh = __shfl_sync(0xFFFFFFFFu, rw, 1);
-            const int L = (int)(rh & 0xFFu);
+            const int L = (int)(rh & 31u);
             const double* xp = Xt + (size_t)base * TILE;
             uint32_t o = 0;
             if (RING > 0) {
@@ -223,7 +224,9 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
         }
         if (flags & FLAG_READOUT) {          // terminal readout O_S (Eq. 15): one block per subset S
             const uint32_t out_idx = __shfl_sync(0xFFFFFFFFu, hw, 2);
-            if (valid) a.out[(size_t)out_idx * (size_t)a.batch + (size_t)b] = a.neg_kappa * close;
+            // 2^(|S|-1): the continuation multiplicities of Lemma 7, applied once per output (exact)
+            const double scale = (double)(1u << (__shfl_sync(0xFFFFFFFFu, hw, 1) >> 24));
+            if (valid) a.out[(size_t)out_idx * (size_t)a.batch + (size_t)b] = (a.neg_kappa * close) * scale;
         }
         mi = mi_n; off = off_n; hw = hw_n; rw = rw_n;
     }
