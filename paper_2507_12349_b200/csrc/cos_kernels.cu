@@ -24,7 +24,7 @@ namespace cosb {
 static const int MAX_WARPS = 16;
 // CTA size bound per instantiation: the long-row kernels (honeycomb, d = 20) are shared-memory limited to one CTA
 // per SM, so they take 24 warps (<= 85 registers) instead of 16.
-__host__ __device__ constexpr int max_warps_of(int maxl) { return maxl == 20 ? 20 : MAX_WARPS; }
+__host__ __device__ constexpr int max_warps_of(int maxl, int ring = 0) { return ring > 0 ? 24 : maxl == 20 ? 20 : MAX_WARPS; }
 
 __device__ __forceinline__ double lds64(uint32_t addr)
 {
@@ -41,6 +41,33 @@ __device__ __forceinline__ void cp_async8(uint32_t dst, const void* src)
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// ---- bulk (TMA) copies global -> shared, completion on an mbarrier (used by the source ring, RING > 0)
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n\t"
+        ".reg .pred P1;\n\t"
+        "COS_MBAR_WAIT:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
+        "@P1 bra COS_MBAR_DONE;\n\t"
+        "bra COS_MBAR_WAIT;\n\t"
+        "COS_MBAR_DONE:\n\t"
+        "}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
 
 // ------------------------------------------------------------------------------------------------------
 // One row of a block: L contiguous source states, nJ destinations.
@@ -91,9 +118,31 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
     // multiplicity (deferred to the readout, cos_compile.h), no pruned entries: SHFL, L x (LDS, DFMA), one store.
     const int n_live = (int)((rh >> 17) & 31u), n_tot = n_live + (int)((rh >> 22) & 1u);
     char* const Yb = (char*)Yt;
-    for (int jj = 0; jj < n_tot; ++jj) {
+    int jj = 0;
+    // two destinations at a time: four independent DFMA chains per warp hide the LDS -> DFMA latency
+    for (; jj + 1 < n_tot; jj += 2) {
+        const uint32_t dj0 = __shfl_sync(0xFFFFFFFFu, rw, 2 + e_words + jj);
+        const uint32_t dj1 = __shfl_sync(0xFFFFFFFFu, rw, 3 + e_words + jj);
+        const uint32_t joff0 = __byte_perm(dj0, 0u, 0x4434u), joff1 = __byte_perm(dj1, 0u, 0x4434u);   // j_a * 256 bytes
+        double a00 = 0.0, a01 = 0.0, a10 = 0.0, a11 = 0.0;
+#pragma unroll
+        for (int k = 0; k < L; ++k) {
+            const double g0 = lds64(ra[k] + joff0), g1 = lds64(ra[k] + joff1);
+            if (k & 1) { a01 = fma(g0, x[k], a01); a11 = fma(g1, x[k], a11); }
+            else { a00 = fma(g0, x[k], a00); a10 = fma(g1, x[k], a10); }
+        }
+        const double acc0 = a00 + a01, acc1 = a10 + a11;
+        __stcs((double*)(Yb + (size_t)(dj0 << 8)), acc0);        // didx * 256 bytes: didx < 2^24, the shift drops j_a
+        if (jj + 1 < n_live) {
+            __stcs((double*)(Yb + (size_t)(dj1 << 8)), acc1);
+        } else {
+#pragma unroll
+            for (int c = 0; c < NC; ++c) sp[c] = (c == lam) ? acc1 : sp[c];
+        }
+    }
+    if (jj < n_tot) {
         const uint32_t dj = __shfl_sync(0xFFFFFFFFu, rw, 2 + e_words + jj);
-        const uint32_t joff = __byte_perm(dj, 0u, 0x4434u);      // j_a * 256 bytes (j_a is the top byte of dj)
+        const uint32_t joff = __byte_perm(dj, 0u, 0x4434u);
         double acc0 = 0.0, acc1 = 0.0;
 #pragma unroll
         for (int k = 0; k < L; ++k) {
@@ -101,7 +150,7 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
         }
         const double acc = acc0 + acc1;
         if (jj < n_live) {
-            __stcs((double*)(Yb + (size_t)(dj << 8)), acc);      // didx * 256 bytes: didx < 2^24, the shift drops j_a
+            __stcs((double*)(Yb + (size_t)(dj << 8)), acc);
         } else {
 #pragma unroll
             for (int c = 0; c < NC; ++c) sp[c] = (c == lam) ? acc : sp[c];
@@ -114,8 +163,8 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
 template <int MAXL, int NC, bool SHIFT, int RING, bool FUSED>
 __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t m_begin, const uint32_t m_end,
                                              const uint32_t tile, unsigned int& s_next, const uint32_t gs_lane,
-                                             const uint32_t gd_lane, const uint32_t ring_lane, const int lane,
-                                             const bool valid, const long long b)
+                                             const uint32_t gd_lane, const uint32_t ring_lane, const uint32_t bar_addr,
+                                             const int lane, const bool valid, const long long b)
 {
     const int HDR = 3 + NC;
     const double* Xt = a.X + (size_t)tile * a.S_src * TILE + lane;
@@ -134,6 +183,7 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
     uint32_t off = 0, hw = 0, rw = 0;
     uint32_t s1 = 0, d0 = 0, d1 = 0, c1 = 0, front = 0;
     bool primed = false;
+    uint32_t t = 0;                      // ring copy group counter (one group per row step)
     if (mi < m_end) {
         const uint2 mt = __ldg(&mtab[mi]);
         off = mt.x;
@@ -184,14 +234,31 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
                 // (RING >= 2 * MAXL), so they have landed.
                 o = base - d0;
                 const uint32_t hi = min(o + (uint32_t)RING, s1 + c1);
-                while (front < hi) {
-                    const uint32_t g = front + (front < s1 ? d0 : d1);
-                    cp_async8(ring_lane + ((front & (uint32_t)(RING - 1)) << 8), Xt + (size_t)g * TILE);
-                    ++front;
+                __syncwarp();                   // every lane has consumed the ring slots that are about to be reused
+                if (lane == 0) {                // group t: contiguous slab ranges -> ring, at most four bulk copies
+                    const uint32_t bar = bar_addr + ((t & 1u) << 3);
+                    mbar_arrive_expect_tx(bar, (hi - front) * (uint32_t)(TILE * 8));
+                    uint32_t f = front;
+                    while (f < hi) {
+                        uint32_t end = hi;
+                        if (f < s1 && end > s1) end = s1;                              // block boundary
+                        const uint32_t wrap = (f | (uint32_t)(RING - 1)) + 1u;         // ring boundary
+                        if (end > wrap) end = wrap;
+                        const uint32_t g = f + (f < s1 ? d0 : d1);
+                        bulk_copy_g2s(ring_lane - (uint32_t)lane * 8u + ((f & (uint32_t)(RING - 1)) << 8),
+                                      Xt0 + (size_t)g * (TILE * 8), (end - f) * (uint32_t)(TILE * 8), bar);
+                        f = end;
+                    }
                 }
-                cp_async_commit();
-                if (primed) cp_async_wait<1>(); else cp_async_wait<0>();      // the very first row has no earlier step
+                // every step waits for the previous group (so each group is observed exactly once, in order); a row
+                // whose states were not all issued by then (the very first row, or one that did not fit the
+                // look-ahead) also waits for the group just issued
+                const bool covered = primed && o + (uint32_t)L <= front;
+                front = hi;
+                if (primed) mbar_wait(bar_addr + (((t - 1u) & 1u) << 3), ((t - 1u) >> 1) & 1u);
+                if (!covered) mbar_wait(bar_addr + ((t & 1u) << 3), (t >> 1) & 1u);
                 primed = true;
+                ++t;
             } else if (a.prefetch > 0) {     // L2 look-ahead: the L states `prefetch` states further down the slab
                 for (int q = lane; q < 2 * L; q += 32) {
                     const uint32_t st = base + (uint32_t)a.prefetch + (uint32_t)(q >> 1);
@@ -230,11 +297,11 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
         }
         mi = mi_n; off = off_n; hw = hw_n; rw = rw_n;
     }
-    if (RING > 0) cp_async_wait<0>();
+    if (RING > 0 && primed) mbar_wait(bar_addr + (((t - 1u) & 1u) << 3), ((t - 1u) >> 1) & 1u);   // nothing in flight at exit
 }
 
 template <int MAXL, int NC, bool SHIFT, int RING>
-__global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(const LayerArgs a)
+__global__ void __launch_bounds__(max_warps_of(MAXL, RING) * 32) cos_layer_kernel(const LayerArgs a)
 {
     extern __shared__ __align__(128) double Gs[];
     __shared__ unsigned int s_next;
@@ -245,6 +312,8 @@ __global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(cons
     const uint32_t gd_lane = gs_lane + (uint32_t)a.n_slots * (TILE * 8u);
     const uint32_t n_tab = (uint32_t)a.n_slots + (SHIFT ? (uint32_t)(NC * a.d) : 0u);
     const uint32_t ring_lane = gs_lane + (n_tab + (uint32_t)warp * (uint32_t)(RING > 0 ? RING : 0)) * (TILE * 8u);
+    __shared__ __align__(8) unsigned long long s_bar[2 * 24];
+    const uint32_t bar_addr = (uint32_t)__cvta_generic_to_shared(s_bar) + (uint32_t)warp * 16u;
 
     // Programmatic dependent launch: let the next layer's grid start (it only stages its table, which no layer
     // writes) while this grid drains; this grid in turn touches the slabs only after the previous one has completed.
@@ -253,6 +322,11 @@ __global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(cons
     const long long b = a.b0 + (long long)tile * TILE + lane;
     const bool valid = b < a.batch;
     if (threadIdx.x == 0) s_next = 0u;
+    if (RING > 0 && lane == 0) {
+        mbar_init(bar_addr, 1u);
+        mbar_init(bar_addr + 8u, 1u);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
     for (int s = warp; s < a.n_slots; s += W) {
         if (valid) cp_async8(gs_lane + (uint32_t)s * (TILE * 8u), a.G + (size_t)s * (size_t)a.batch + (size_t)b);
         else Gs[s * TILE + lane] = 0.0;
@@ -277,7 +351,8 @@ __global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(cons
     if (a.pdl) asm volatile("griddepcontrol.wait;" ::: "memory");
     const uint32_t m_begin = blockIdx.y * a.masks_per_cta;
     const uint32_t m_end = min(a.n_masks, m_begin + a.masks_per_cta);
-    layer_blocks<MAXL, NC, SHIFT, RING, false>(a, m_begin, m_end, tile, s_next, gs_lane, gd_lane, ring_lane, lane, valid, b);
+    layer_blocks<MAXL, NC, SHIFT, RING, false>(a, m_begin, m_end, tile, s_next, gs_lane, gd_lane, ring_lane, bar_addr, lane,
+                                               valid, b);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -331,7 +406,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
         a.words = fl.words; a.mask_off = fl.mask_off; a.n_masks = fl.n_masks;
         a.X = (l & 1) ? slab1 : slab0; a.Y = (l & 1) ? slab0 : slab1;
         // slabs are addressed per tile already: tile index 0 inside layer_blocks
-        layer_blocks<MAXL, NC, SHIFT, 0, true>(a, 0u, fl.n_masks, 0u, s_next, gs_lane, gd_lane, 0u, lane, valid, b);
+        layer_blocks<MAXL, NC, SHIFT, 0, true>(a, 0u, fl.n_masks, 0u, s_next, gs_lane, gd_lane, 0u, 0u, lane, valid, b);
         __threadfence_block();
         __syncthreads();
         if (threadIdx.x == 0) s_next = 0u;
@@ -407,9 +482,9 @@ cudaError_t pick_layer_shape(int max_L, int nc, int d, int n_slots, bool shift, 
                              int* warps_per_cta, int* ctas_per_sm)
 {
     static const int cand[8] = {4, 6, 8, 10, 12, 16, 20, 24};
-    const int max_w = max_warps_of(max_L <= 4 ? 4 : max_L <= 8 ? 8 : max_L <= 12 ? 12 : max_L <= 20 ? 20 : 24);
     for (int pass = 0; pass < 2; ++pass) {
         const int rg = (pass == 0) ? LAYER_RING : 0;
+        const int max_w = max_warps_of(max_L <= 4 ? 4 : max_L <= 8 ? 8 : max_L <= 12 ? 12 : max_L <= 20 ? 20 : 24, rg);
         if (pass == 0 && (want_ring == 0 || max_L > 12)) continue;
         layer_fn fn = pick_layer_fn(max_L, nc, shift, rg);
         if (!fn) continue;
@@ -434,7 +509,7 @@ cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, int 
 {
     if (a.n_masks == 0 || tiles == 0) return cudaSuccess;
     if (warps_per_cta < 1) warps_per_cta = 1;
-    const int max_w = max_warps_of(max_L <= 4 ? 4 : max_L <= 8 ? 8 : max_L <= 12 ? 12 : max_L <= 20 ? 20 : 24);
+    const int max_w = max_warps_of(max_L <= 4 ? 4 : max_L <= 8 ? 8 : max_L <= 12 ? 12 : max_L <= 20 ? 20 : 24, ring);
     if (warps_per_cta > max_w) warps_per_cta = max_w;
     const uint32_t chunks = (a.n_masks + a.masks_per_cta - 1) / a.masks_per_cta;
     if (chunks > 65535u) return cudaErrorInvalidConfiguration;

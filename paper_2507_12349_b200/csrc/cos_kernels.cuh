@@ -6,8 +6,8 @@
 namespace cosb {
 
 static const int TILE = 32;              // configurations per batch tile = one warp, lane = configuration
-static const int LAYER_RING = 32;        // states per warp of the shared-memory source ring (>= 2 * 12)
-static const size_t LAYER_SMEM_MAX = 227 * 1024 - 256;   // minus the static counter and the 128-byte alignment of the table
+static const int LAYER_RING = 16;        // states per warp of the shared-memory source ring (>= 12, power of two)
+static const size_t LAYER_SMEM_MAX = 227 * 1024 - 1024;   // minus the static counter and the 128-byte alignment of the table
 
 struct LayerArgs {
     const uint32_t* words;               // layer program (cos_compile.h)
