@@ -116,7 +116,7 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
     }
     h->warps_per_cta = 8;
     h->masks_per_cta = env_int("COS_MASKS_PER_CTA", 0);        // 0: chosen per layer in cos_eval
-    h->prefetch = env_int("COS_PREFETCH", 0);
+    h->prefetch = env_int("COS_PREFETCH", 8);
     h->pdl = env_int("COS_PDL", 1);
 
     if (!(flags & COS_BUILD_HOST_ONLY)) {
