@@ -69,6 +69,36 @@ __device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uin
                  ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
 
+// U ordinary destinations of a row at once (program words w0 .. w0+U-1 of the row record): U length-L dot products
+// against U columns of the staged table, 2U independent DFMA chains, U stores.
+#ifndef COS_DEST_WIDE
+#define COS_DEST_WIDE 4
+#endif
+template <int L, int U>
+__device__ __forceinline__ void dest_group(const uint32_t rw, const int w0, const uint32_t (&ra)[L], const double (&x)[L],
+                                           char* const Yb)
+{
+    uint32_t dj[U], joff[U];
+    double a0[U], a1[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        dj[u] = __shfl_sync(0xFFFFFFFFu, rw, w0 + u);
+        joff[u] = __byte_perm(dj[u], 0u, 0x4434u);              // j_a * 256 bytes (j_a is the top byte of dj)
+        a0[u] = 0.0; a1[u] = 0.0;
+    }
+#pragma unroll
+    for (int k = 0; k < L; ++k) {
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            const double g = lds64(ra[k] + joff[u]);
+            if (k & 1) a1[u] = fma(g, x[k], a1[u]); else a0[u] = fma(g, x[k], a0[u]);
+        }
+    }
+#pragma unroll
+    for (int u = 0; u < U; ++u)                                  // didx * 256 bytes: didx < 2^24, the shift drops j_a
+        __stcs((double*)(Yb + (size_t)(dj[u] << 8)), a0[u] + a1[u]);
+}
+
 // ------------------------------------------------------------------------------------------------------
 // One row of a block: L contiguous source states, nJ destinations.
 //   rw       this lane's word of the row record (lane k holds word k)
@@ -116,32 +146,18 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
     }
     // destinations: n_live ordinary ones, then (defer) the one that merges with the fresh-head state.  No per-edge
     // multiplicity (deferred to the readout, cos_compile.h), no pruned entries: SHFL, L x (LDS, DFMA), one store.
-    const int n_live = (int)((rh >> 17) & 31u), n_tot = n_live + (int)((rh >> 22) & 1u);
+    const int n_live = (int)((rh >> 17) & 31u);
     char* const Yb = (char*)Yt;
     int jj = 0;
-    // two destinations at a time: four independent DFMA chains per warp hide the LDS -> DFMA latency
-    for (; jj + 1 < n_tot; jj += 2) {
-        const uint32_t dj0 = __shfl_sync(0xFFFFFFFFu, rw, 2 + e_words + jj);
-        const uint32_t dj1 = __shfl_sync(0xFFFFFFFFu, rw, 3 + e_words + jj);
-        const uint32_t joff0 = __byte_perm(dj0, 0u, 0x4434u), joff1 = __byte_perm(dj1, 0u, 0x4434u);   // j_a * 256 bytes
-        double a00 = 0.0, a01 = 0.0, a10 = 0.0, a11 = 0.0;
-#pragma unroll
-        for (int k = 0; k < L; ++k) {
-            const double g0 = lds64(ra[k] + joff0), g1 = lds64(ra[k] + joff1);
-            if (k & 1) { a01 = fma(g0, x[k], a01); a11 = fma(g1, x[k], a11); }
-            else { a00 = fma(g0, x[k], a00); a10 = fma(g1, x[k], a10); }
-        }
-        const double acc0 = a00 + a01, acc1 = a10 + a11;
-        __stcs((double*)(Yb + (size_t)(dj0 << 8)), acc0);        // didx * 256 bytes: didx < 2^24, the shift drops j_a
-        if (jj + 1 < n_live) {
-            __stcs((double*)(Yb + (size_t)(dj1 << 8)), acc1);
-        } else {
-#pragma unroll
-            for (int c = 0; c < NC; ++c) sp[c] = (c == lam) ? acc1 : sp[c];
-        }
-    }
-    if (jj < n_tot) {
-        const uint32_t dj = __shfl_sync(0xFFFFFFFFu, rw, 2 + e_words + jj);
+    // COS_DEST_WIDE / two / one destination(s) at a time: 2 independent DFMA chains per destination hide the
+    // LDS -> DFMA latency at 20-24 resident warps
+#if COS_DEST_WIDE > 2
+    for (; jj + COS_DEST_WIDE <= n_live; jj += COS_DEST_WIDE) dest_group<L, COS_DEST_WIDE>(rw, 2 + e_words + jj, ra, x, Yb);
+#endif
+    for (; jj + 2 <= n_live; jj += 2) dest_group<L, 2>(rw, 2 + e_words + jj, ra, x, Yb);
+    if (jj < n_live) dest_group<L, 1>(rw, 2 + e_words + jj, ra, x, Yb);
+    if ((rh >> 22) & 1u) {                  // the destination that merges with the fresh-head state (E2/E4 pair)
+        const uint32_t dj = __shfl_sync(0xFFFFFFFFu, rw, 2 + e_words + n_live);
         const uint32_t joff = __byte_perm(dj, 0u, 0x4434u);
         double acc0 = 0.0, acc1 = 0.0;
 #pragma unroll
@@ -149,12 +165,8 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
             if (k & 1) acc1 = fma(lds64(ra[k] + joff), x[k], acc1); else acc0 = fma(lds64(ra[k] + joff), x[k], acc0);
         }
         const double acc = acc0 + acc1;
-        if (jj < n_live) {
-            __stcs((double*)(Yb + (size_t)(dj << 8)), acc);
-        } else {
 #pragma unroll
-            for (int c = 0; c < NC; ++c) sp[c] = (c == lam) ? acc : sp[c];
-        }
+        for (int c = 0; c < NC; ++c) sp[c] = (c == lam) ? acc : sp[c];
     }
 }
 
