@@ -34,7 +34,7 @@ METRIC = "connected_sum_configs_per_s"
 UNIT = "configs/s"
 # DRAM bytes (read + write) of the layer-kernel launches of ONE step, from a committed ncu capture; per workload at its
 # BASELINE batch.  None = not captured.
-NCU_DRAM_BYTES_PER_STEP = {"cfg4_square_sb3_n10": (231.650e9, 8192, "profiles/r01d_dram_traffic_step.md")}
+NCU_DRAM_BYTES_PER_STEP = {"cfg4_square_sb3_n10": (244.573e9, 8192, "profiles/r01e_dram_traffic_step.md")}
 DEFAULT_WORKLOAD = "cfg4"       # n = 10: the order BASELINE.json's target is quoted on
 
 
