@@ -369,15 +369,16 @@ def test_config5_full(cos):
         check(got[0, c], ref, Ms[c], ("cfg5", c))
 
 
-def test_config3_reduced_batch(cos):
-    """BASELINE config 3's DAG (honeycomb, two spins, opposite shifts, n = 10, 3.9e7 states) on a reduced
-    batch of 96 configurations; sampled configurations against sum over 2^10 sublattice assignments of O2a'."""
-    w = get_config(3).scaled(batch=96)
+def test_config3_full_sampled(cos):
+    """BASELINE config 3 at full size (honeycomb, two spins, opposite shifts, n = 10, 3.9e7 states, 16384 configurations;
+    the 64 GiB workspace budget makes cos_eval walk the batch in chunks of 17 tiles, as in bench.py); sampled
+    configurations against the sum over 2^10 sublattice assignments of O2a' (binary128)."""
+    w = get_config(3)
     table, v, G = _tabulated(cos, w)
     got, info = _eval_workload(cos, w, G)
     assert (info["n_states"], info["n_edges"], info["n_readout_edges"]) == (39320580, 422359128, 688)
     assert np.all(np.isfinite(got))
-    for c in (0, 95):
+    for c in (0, 8191, 16383):
         Gc = np.ascontiguousarray(G[:, c].cpu().numpy().reshape(2, w.d, w.d))
         ref = oracle.connected_reference(Gc, w.n, 2, 2, w.sigmas, False, False, tier="o2a")[0]
         check(got[0, c], ref, M_lower_bound(Gc, w.n, 2, 2, False, n_assign=4, seed=c), ("cfg3", c))
