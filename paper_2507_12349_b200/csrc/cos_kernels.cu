@@ -78,25 +78,34 @@ template <int L, int U>
 __device__ __forceinline__ void dest_group(const uint32_t rw, const int w0, const uint32_t (&ra)[L], const double (&x)[L],
                                            char* const Yb)
 {
-    uint32_t dj[U], joff[U];
-    double a0[U], a1[U];
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-        dj[u] = __shfl_sync(0xFFFFFFFFu, rw, w0 + u);
-        joff[u] = __byte_perm(dj[u], 0u, 0x4434u);              // j_a * 256 bytes (j_a is the top byte of dj)
-        a0[u] = 0.0; a1[u] = 0.0;
-    }
+    // (ptxas keeps the column offsets in vector registers here: one IMAD.IADD per LDS; only the single-destination
+    // loops get the LDS [R + UR] form)
+    const uint32_t dA = __shfl_sync(0xFFFFFFFFu, rw, w0);
+    const uint32_t dB = U > 1 ? __shfl_sync(0xFFFFFFFFu, rw, w0 + 1) : 0u;
+    const uint32_t dC = U > 2 ? __shfl_sync(0xFFFFFFFFu, rw, w0 + 2) : 0u;
+    const uint32_t dD = U > 3 ? __shfl_sync(0xFFFFFFFFu, rw, w0 + 3) : 0u;
+    const uint32_t jA = __byte_perm(dA, 0u, 0x4434u), jB = __byte_perm(dB, 0u, 0x4434u);   // j_a * 256 bytes
+    const uint32_t jC = __byte_perm(dC, 0u, 0x4434u), jD = __byte_perm(dD, 0u, 0x4434u);
+    double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0, c0 = 0.0, c1 = 0.0, d0 = 0.0, d1 = 0.0;
 #pragma unroll
     for (int k = 0; k < L; ++k) {
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            const double g = lds64(ra[k] + joff[u]);
-            if (k & 1) a1[u] = fma(g, x[k], a1[u]); else a0[u] = fma(g, x[k], a0[u]);
+        if (k & 1) {
+            a1 = fma(lds64(ra[k] + jA), x[k], a1);
+            if (U > 1) b1 = fma(lds64(ra[k] + jB), x[k], b1);
+            if (U > 2) c1 = fma(lds64(ra[k] + jC), x[k], c1);
+            if (U > 3) d1 = fma(lds64(ra[k] + jD), x[k], d1);
+        } else {
+            a0 = fma(lds64(ra[k] + jA), x[k], a0);
+            if (U > 1) b0 = fma(lds64(ra[k] + jB), x[k], b0);
+            if (U > 2) c0 = fma(lds64(ra[k] + jC), x[k], c0);
+            if (U > 3) d0 = fma(lds64(ra[k] + jD), x[k], d0);
         }
     }
-#pragma unroll
-    for (int u = 0; u < U; ++u)                                  // didx * 256 bytes: didx < 2^24, the shift drops j_a
-        __stcs((double*)(Yb + (size_t)(dj[u] << 8)), a0[u] + a1[u]);
+    // didx * 256 bytes: didx < 2^24, the shift drops j_a
+    __stcs((double*)(Yb + (size_t)(dA << 8)), a0 + a1);
+    if (U > 1) __stcs((double*)(Yb + (size_t)(dB << 8)), b0 + b1);
+    if (U > 2) __stcs((double*)(Yb + (size_t)(dC << 8)), c0 + c1);
+    if (U > 3) __stcs((double*)(Yb + (size_t)(dD << 8)), d0 + d1);
 }
 
 // ------------------------------------------------------------------------------------------------------
