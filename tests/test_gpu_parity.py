@@ -399,3 +399,25 @@ def test_fused_and_layered_paths_agree(cos, n, nf, lattice, sb, all_subsets, mon
     b = gpu_eval(cos, G, n, nf, lattice, sig, all_subsets)
     assert np.all(np.isfinite(a))
     assert np.array_equal(a, b) and np.array_equal(a, a_chunked)
+
+
+@pytest.mark.parametrize("n,nf,sb,all_subsets", [(8, 2, False, True), (7, 3, True, False)])
+def test_tma_ring_path_agrees(cos, n, nf, sb, all_subsets, monkeypatch):
+    """COS_RING=1 streams the source rows through a per-warp shared-memory ring with TMA bulk copies + mbarriers
+    (measured slower, off by default).  Same program, same arithmetic order: bit-identical to the default path."""
+    sig = [0.3, -0.2, 0.1][:nf] if sb else None
+    G = random_matrices(70 + n, nf if sb else 1, n, 101, scale=0.5, diag=-0.4)
+    monkeypatch.setenv("COS_RING", "0")
+    a = gpu_eval(cos, G, n, nf, 0, sig, all_subsets)
+    monkeypatch.setenv("COS_RING", "1")
+    b = gpu_eval(cos, G, n, nf, 0, sig, all_subsets)
+    assert np.all(np.isfinite(a)) and np.array_equal(a, b)
+    for c in (0, 100):
+        A = np.ascontiguousarray(G[..., c])
+        if sb:
+            ref = oracle.o2b_polynomial(A, sig)[-1:]
+            M = np.array([M_lower_bound(A, n, 1, nf, False)])
+        else:
+            ref = oracle.o2a_twospin(A[0], A[0])
+            M = oracle.o3_uniform(A[0], 2, 0.0, True, absolute=True)
+        check(a[:, c], ref, M, ("ring", n, c))
