@@ -135,7 +135,9 @@ void cos_tab_free(cos_tab tab);
  *   sites_host  host int32 [n][2][batch], tau_host host fp64 [n][batch] (layouts of cos_tabulate; pinned memory
  *               makes the copies asynchronous, pageable memory works too), out_host host fp64 [n_out][batch].
  * Copies the inputs to a device staging area owned by the handle (grown lazily), runs cos_tabulate and cos_eval on
- * `stream`, copies the result back and SYNCHRONISES the stream before returning.  n is the handle's order; the table
+ * `stream`, copies the result back and SYNCHRONISES the stream before returning.  Outputs of 16 MiB or more are
+ * produced in up to 8 batch slices whose columns are copied back on an internal second stream while the next slice
+ * is evaluated.  n is the handle's order; the table
  * must have the handle's number of propagator blocks and lattice.  Bytes moved per call:
  * H2D batch*n*(2*4+8), D2H batch*n_out*8. */
 int cos_eval_host(cos_handle h, cos_tab tab, const int* sites_host, const double* tau_host, long long batch,

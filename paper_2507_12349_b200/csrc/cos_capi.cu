@@ -56,6 +56,8 @@ struct cos_handle_s {
     // staging of cos_eval_host
     int* st_sites = nullptr; double* st_tau = nullptr; double* st_G = nullptr; double* st_out = nullptr;
     long long st_batch = 0;
+    cudaStream_t copy_stream = nullptr;   // D2H of finished output slices (cos_eval_host)
+    cudaEvent_t copy_events[8] = {};
 };
 
 struct cos_tab_s {
@@ -193,6 +195,10 @@ void cos_free(cos_handle h)
     if (h->st_tau) cudaFree(h->st_tau);
     if (h->st_G) cudaFree(h->st_G);
     if (h->st_out) cudaFree(h->st_out);
+    if (h->copy_stream) {
+        cudaStreamDestroy(h->copy_stream);
+        for (cudaEvent_t ev : h->copy_events) if (ev) cudaEventDestroy(ev);
+    }
     delete h;
 }
 
@@ -203,14 +209,11 @@ int cos_set_workspace_limit(cos_handle h, long long bytes)
     return COS_OK;
 }
 
-int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev, cos_stream stream_)
+// Layers + readouts for the batch tiles [tile_begin, tile_end) of a batch of `batch` configurations (G_dev / out_dev are
+// the whole-batch arrays).  clear: zero-fill the output rows of a partial readout set first (whole batch).
+static int eval_range(cos_handle h, const double* G_dev, long long batch, double* out_dev, long long tile_begin,
+                      long long tile_end, bool clear, cudaStream_t stream)
 {
-    if (!h) return fail(COS_EINVAL, "cos_eval: handle is NULL");
-    if (batch < 0) return fail(COS_EINVAL, "cos_eval: negative batch");
-    if (batch == 0) return COS_OK;
-    if (!G_dev || !out_dev) return fail(COS_EINVAL, "cos_eval: NULL device pointer");
-    if (!h->on_device) return fail(COS_ECUDA, "cos_eval: handle was built host-only / without a CUDA device (no CPU fallback)");
-    cudaStream_t stream = (cudaStream_t)stream_;
     const CompiledDag& D = h->dag;
     const int NL = (int)D.layers.size();
 
@@ -231,13 +234,12 @@ int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev
     }
     double* slab[2] = {h->ws, h->ws + (size_t)D.max_layer_states * TILE * (size_t)tiles_chunk};
 
-    if (D.all_subsets && D.order_mask != (((2u << D.n) - 1u) & ~1u)) {     // partial readout set: other rows are zeros
+    if (clear && D.all_subsets && D.order_mask != (((2u << D.n) - 1u) & ~1u)) {     // partial readout set: other rows are zeros
         cudaError_t e = cudaMemsetAsync(out_dev, 0, (size_t)D.n_out * (size_t)batch * sizeof(double), stream);
         if (e != cudaSuccess) return cuda_fail(e, "cos_eval: clearing the output");
     }
-    if (h->profiling) ++h->profiled_evals;
-    for (long long t0 = 0; t0 < tiles_total; t0 += tiles_chunk) {
-        const uint32_t tiles = (uint32_t)((tiles_total - t0 < tiles_chunk) ? (tiles_total - t0) : tiles_chunk);
+    for (long long t0 = tile_begin; t0 < tile_end; t0 += tiles_chunk) {
+        const uint32_t tiles = (uint32_t)((tile_end - t0 < tiles_chunk) ? (tile_end - t0) : tiles_chunk);
         if (h->fused && !h->profiling) {
             FusedArgs f;
             f.layers = h->fused_layers; f.n_layers = NL; f.ws = h->ws; f.S_max = D.max_layer_states;
@@ -303,6 +305,17 @@ int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev
     return COS_OK;
 }
 
+int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev, cos_stream stream_)
+{
+    if (!h) return fail(COS_EINVAL, "cos_eval: handle is NULL");
+    if (batch < 0) return fail(COS_EINVAL, "cos_eval: negative batch");
+    if (batch == 0) return COS_OK;
+    if (!G_dev || !out_dev) return fail(COS_EINVAL, "cos_eval: NULL device pointer");
+    if (!h->on_device) return fail(COS_ECUDA, "cos_eval: handle was built host-only / without a CUDA device (no CPU fallback)");
+    if (h->profiling) ++h->profiled_evals;
+    return eval_range(h, G_dev, batch, out_dev, 0, (batch + TILE - 1) / TILE, true, (cudaStream_t)stream_);
+}
+
 int cos_set_profiling(cos_handle h, int on)
 {
     if (!h) return fail(COS_EINVAL, "cos_set_profiling: handle is NULL");
@@ -365,9 +378,39 @@ int cos_eval_host(cos_handle h, cos_tab tab, const int* sites_host, const double
     int rc = cos_tabulate(tab, D.n, h->st_sites, h->st_tau, batch, h->st_G, stream_);
     if (rc != COS_OK) return rc;
     ++h->n_launches;
-    rc = cos_eval(h, h->st_G, batch, h->st_out, stream_);
-    if (rc != COS_OK) return rc;
-    e = cudaMemcpyAsync(out_host, h->st_out, b_out, cudaMemcpyDeviceToHost, stream);
+    if (h->profiling) ++h->profiled_evals;
+    // Large outputs (all-subset readouts): walk the batch in up to 8 slices and copy the output columns of slice i
+    // back on a second stream while slice i+1 is evaluated (one strided 2-D copy per slice).
+    const long long tiles_total = (batch + TILE - 1) / TILE;
+    long long n_slices = (long long)(b_out >> 23);                  // ~8 MiB of output per slice
+    if (n_slices > 8) n_slices = 8;
+    if (n_slices > tiles_total) n_slices = tiles_total;
+    if (n_slices <= 1 || env_int("COS_HOST_PIPELINE", 1) == 0) {
+        rc = eval_range(h, h->st_G, batch, h->st_out, 0, tiles_total, true, stream);
+        if (rc != COS_OK) return rc;
+        e = cudaMemcpyAsync(out_host, h->st_out, b_out, cudaMemcpyDeviceToHost, stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
+        if (e != cudaSuccess) return cuda_fail(e, "cos_eval_host: device-to-host copy");
+        return COS_OK;
+    }
+    if (!h->copy_stream) {
+        e = cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking);
+        for (int i = 0; i < 8 && e == cudaSuccess; ++i) e = cudaEventCreateWithFlags(&h->copy_events[i], cudaEventDisableTiming);
+        if (e != cudaSuccess) return cuda_fail(e, "cos_eval_host: copy stream");
+    }
+    for (long long i = 0; i < n_slices; ++i) {
+        const long long t_a = tiles_total * i / n_slices, t_b = tiles_total * (i + 1) / n_slices;
+        rc = eval_range(h, h->st_G, batch, h->st_out, t_a, t_b, i == 0, stream);
+        if (rc != COS_OK) return rc;
+        const size_t c0 = (size_t)t_a * TILE, c1 = (size_t)(t_b * TILE < batch ? t_b * TILE : batch);
+        e = cudaEventRecord(h->copy_events[i], stream);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(h->copy_stream, h->copy_events[i], 0);
+        if (e == cudaSuccess)
+            e = cudaMemcpy2DAsync(out_host + c0, B * sizeof(double), h->st_out + c0, B * sizeof(double),
+                                  (c1 - c0) * sizeof(double), (size_t)D.n_out, cudaMemcpyDeviceToHost, h->copy_stream);
+        if (e != cudaSuccess) return cuda_fail(e, "cos_eval_host: pipelined device-to-host copy");
+    }
+    e = cudaStreamSynchronize(h->copy_stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
     if (e != cudaSuccess) return cuda_fail(e, "cos_eval_host: device-to-host copy");
     return COS_OK;
