@@ -421,3 +421,31 @@ def test_tma_ring_path_agrees(cos, n, nf, sb, all_subsets, monkeypatch):
             ref = oracle.o2a_twospin(A[0], A[0])
             M = oracle.o3_uniform(A[0], 2, 0.0, True, absolute=True)
         check(a[:, c], ref, M, ("ring", n, c))
+
+
+def test_four_flavours_per_layer_kernels(cos):
+    """N_f = 4 (the largest colour count the state carries) at n = 7 -- beyond the fused small-DAG path -- against the
+    polynomial route Eq. 34-38 generalised to any N_f (reading G13) and against Algorithm 3 as printed."""
+    n, nf, B = 7, 4, 40
+    sig = [0.25, -0.1, 0.0, 0.3]
+    G = random_matrices(404, nf, n, B, scale=0.45, diag=-0.4)
+    got = gpu_eval(cos, G, n, nf, cos.COS_LATTICE_SQUARE, sig, False)
+    for c in (0, 17, 39):
+        A = np.ascontiguousarray(G[..., c])
+        M = oracle.o3_alg3(A, sig, absolute=True)
+        check(got[0, c], oracle.o2b_polynomial(A, sig)[-1], M, ("nf4 o2b", c))
+        check(got[0, c], oracle.o3_alg3(A, sig), M, ("nf4 o3", c))
+
+
+def test_honeycomb_uniform_long_rows(cos):
+    """Uniform CoS with the sublattice sum (Algorithm 2; Eq. 4, 55) at n = 7: d = 14 endpoints, rows of up
+    to 14 states (the MAXL = 20 kernels without shifts), against the sum over 2^7 assignments of the two-determinant
+    route."""
+    n, B = 7, 36
+    G = random_matrices(505, 1, 2 * n, B, scale=0.4, diag=-0.45)
+    got = gpu_eval(cos, G, n, 2, cos.COS_LATTICE_HONEYCOMB, None, False)
+    for c in (0, 35):
+        Gc = np.ascontiguousarray(G[..., c])
+        ref = oracle.connected_reference(Gc, n, 2, 2, None, True, False, tier="o2a")
+        M = oracle.connected_reference(Gc, n, 2, 2, None, True, False, tier="o3", absolute=True)
+        check(got[:, c], ref, M, ("honeycomb uniform", c))
