@@ -157,6 +157,34 @@ int cos_eval_host(cos_handle h, cos_tab tab, const int* sites_host, const double
 int cos_flux_weights(int n, unsigned int order_mask, const double* lambda_host, const double* C_dev,
                      const double* Q_dev, long long batch, double* W_dev, double* Phi_dev, cos_stream stream);
 
+/* ---- determinant-polynomial route on the device: PAPER.md:267-315 (Eq. 32-38); SURVEY.md 8(f).3 ---------------
+ * An independent second evaluator of the all-subset connected values ("an independent comparison with SB-CoS for
+ * non-uniform matrices and shifts"): principal minors d_a(S) = det A^(a)[S,S] (Eq. 34), full moments
+ * H(T) = sum_{S_a} prod_a d_a(S_a) prod_i L_i with the local tensor of Eq. 35 (a site of T carries a pair of flavours
+ * a < b with weight 2, or one flavour a with weight 2 sigma_a; reading G13 of DESIGN.md for two flavours), connected
+ * values C(T) = H(T) - sum_{S proper subset of T, min T in S} C(S) H(T \ S) (Eq. 38; proper subsets, reading G14).
+ * H has the physical convention of Eq. 83 (no shift-shift term), like cos_eval.  Square lattice (d = n) only.
+ *   n_flavors  2 or 3 (COS_EUNSUPPORTED otherwise).
+ *   n_blocks   n_flavors (one n x n matrix per flavour) or 1 (flavour-uniform: every flavour reads block 0; with
+ *              shifts = NULL this is the uniform CoS value with loop factor N_f, Eq. 33).
+ *   shifts     host, n_flavors shift-close weights sigma_a = alpha_a/U, or NULL for zero shifts.
+ *   precision  COS_DET_FP64: every step in fp64.  COS_DET_DD: every step (elimination, moments, Eq. 38) in
+ *              double-double arithmetic, ~106 significant bits, as the paper does for this route;
+ *              inputs are the caller's fp64 values, taken as exact; outputs are rounded to fp64 at the end.
+ *   G_dev      device fp64 [n_blocks][n][n][batch], the layout of cos_eval (read-only).
+ *   out_dev    device fp64 [2^n-1][batch], written: row bitmask(T)-1, the layout of an all-subset cos_eval.
+ *   work_dev   device scratch of at least cos_det_workspace_bytes(n, n_blocks, precision, batch) bytes, 16-byte aligned,
+ *              owned by the caller; work_bytes is its size (too small or misaligned: COS_EINVAL).
+ * Accuracy: Eq. 38 subtracts from H(T) every disconnected product of smaller moments, so the rounding error of the
+ * route scales with R(T) = the same recursion with every term positive on |A|, |sigma| (>= the DAG's M, which has
+ * only the connected terms): |error| ~ 1e-15 R in fp64, ~1e-30 R in double-double.  On physical propagators
+ * |C| / R falls from ~1e-8 (n = 6) to ~1e-22 (n = 10): fp64 is a cross-check up to n ~ 6, double-double to n ~ 11.
+ * Cost: 7^n (three flavours) or 4^n (two) terms per configuration.  Asynchronous on `stream`. */
+enum { COS_DET_FP64 = 0, COS_DET_DD = 1 };
+long long cos_det_workspace_bytes(int n, int n_blocks, int precision, long long batch);      /* -1 on bad arguments */
+int cos_det_eval(int n, int n_flavors, int n_blocks, const double* shifts, int precision, const double* G_dev,
+                 long long batch, double* out_dev, void* work_dev, long long work_bytes, cos_stream stream);
+
 /* ---- measurement helpers ------------------------------------------------------------------------------
  * cos_set_profiling(h, 1): every later cos_eval brackets each layer launch with CUDA events on its stream.
  * cos_get_layer_times synchronises on the recorded events, ADDS the elapsed milliseconds of layer l (summed over

@@ -267,6 +267,31 @@ static void cdet_recursion(int n, const xreal *a, xreal *c)
         }
 }
 
+/* Rounding-error scale of a floating-point evaluation of Eq. 53 / Eq. 38 itself (not of the connected value): the same
+ * recursion with every term taken positive, R(V) = a(V) + sum_S R(S) a(V \ S), on a >= 0 (the moments evaluated on
+ * |A|, |sigma|).  It contains the disconnected products that the recursion subtracts, so R >= |c|; it bounds what an
+ * fp64 evaluation of the determinant route can lose, and is used only as the tolerance scale of that route's tests
+ * (cos_o2b_polynomial with absolute = 2).                                                            */
+static void cdet_route_scale(int n, const xreal *a, xreal *c)
+{
+    uint32_t full = (1u << n), V;
+    int size;
+    c[0] = 0;
+    for (size = 1; size <= n; ++size)
+        for (V = 1; V < full; ++V) {
+            if (popc(V) != size) continue;
+            uint32_t anchor = V & (~V + 1u);
+            uint32_t rest = V ^ anchor, sub;
+            xreal acc = a[V];
+            for (sub = (rest - 1) & rest; ; sub = (sub - 1) & rest) {
+                if (rest == 0) break;
+                acc += c[anchor | sub] * a[V ^ (anchor | sub)];
+                if (sub == 0) break;
+            }
+            c[V] = acc;
+        }
+}
+
 /* O2a / O2a': two-spin Hubbard.  Full contraction sum at fixed vertices = product of two
  * determinants; the counterterm enters the TRUE diagonal of spin s with the
  * OPPOSITE spin's weight (Eq. 49); 2 endpoint assignments per contact vertex:
@@ -357,7 +382,8 @@ int cos_o2b_polynomial(int n, int nf, const double *A /*[nf][n][n]*/, const doub
         o2b_rec(&c, 0, 1);
         H[T] = c.acc;
     }
-    cdet_recursion(n, H, C);
+    if (absolute == 2) cdet_route_scale(n, H, C);
+    else cdet_recursion(n, H, C);
     for (T = 1; T < full; ++T) out[T - 1] = (double)C[T];
     free(d); free(H); free(C);
     return 0;

@@ -85,7 +85,9 @@ def o2a_twospin(A_up, A_dn, sig_up=0.0, sig_dn=0.0, absolute=False):
 
 def o2b_polynomial(A, sigma=None, absolute=False):
     """Flavour-polynomial route Eq. 34-38 on A[N_f][n][n]: all 2^n - 1 connected values (binary128 inside).
-    absolute=True: permanents of |A|, |sigma| -- a LOWER bound of the cancellation scale M (C file, O2 header)."""
+    absolute=True: permanents of |A|, |sigma| -- a LOWER bound of the cancellation scale M (C file, O2 header).
+    absolute=2: additionally every minus sign of Eq. 38 becomes a plus -- the rounding-error scale of evaluating the
+    ROUTE in floating point (it keeps the disconnected products Eq. 38 subtracts); tolerance scale of cos_det_eval."""
     A, pA = _c(A)
     nf, n, _ = A.shape
     s, ps = _sig(sigma)

@@ -14,6 +14,7 @@ _lib = None
 COS_OK, COS_EINVAL, COS_ENOMEM, COS_ECUDA, COS_EUNSUPPORTED = 0, 1, 2, 3, 4
 COS_LATTICE_SQUARE, COS_LATTICE_HONEYCOMB = 0, 1
 COS_BUILD_HOST_ONLY = 1
+COS_DET_FP64, COS_DET_DD = 0, 1
 
 INFO = {
     "n_layers": 0, "n_states": 1, "n_edges": 2, "n_readout_edges": 3, "n_out": 4, "max_layer_states": 5,
@@ -26,6 +27,7 @@ EXPORTS = [
     "cos_build", "cos_build_ex", "cos_eval", "cos_free", "cos_set_workspace_limit", "cos_info",
     "cos_last_error", "cos_tab_build", "cos_tabulate", "cos_tab_free", "cos_measure_fp64_fma_peak",
     "cos_eval_host", "cos_set_profiling", "cos_get_layer_times", "cos_build_orders", "cos_flux_weights",
+    "cos_det_workspace_bytes", "cos_det_eval",
 ]
 
 
@@ -79,6 +81,10 @@ def load_library():
     lib.cos_build_orders.argtypes = [ip, ip, ip, dp, ctypes.c_uint, ip, ctypes.POINTER(vp)]
     lib.cos_flux_weights.restype = ctypes.c_int
     lib.cos_flux_weights.argtypes = [ip, ctypes.c_uint, dp, vp, vp, ctypes.c_longlong, vp, vp, vp]
+    lib.cos_det_workspace_bytes.restype = ctypes.c_longlong
+    lib.cos_det_workspace_bytes.argtypes = [ip, ip, ip, ctypes.c_longlong]
+    lib.cos_det_eval.restype = ctypes.c_int
+    lib.cos_det_eval.argtypes = [ip, ip, ip, dp, ip, vp, ctypes.c_longlong, vp, vp, ctypes.c_longlong, vp]
     lib.cos_measure_fp64_fma_peak.restype = ctypes.c_int
     lib.cos_measure_fp64_fma_peak.argtypes = [dp]
     _lib = lib
@@ -127,6 +133,25 @@ def cos_flux_weights(n, order_mask, lambdas, C_dev, Q_dev, batch, W_dev, Phi_dev
         int(n), int(order_mask), ctypes.cast(lam, ctypes.POINTER(ctypes.c_double)), _dev_ptr(C_dev, "torch.float64"),
         None if Q_dev is None else _dev_ptr(Q_dev, "torch.float64"), int(batch), _dev_ptr(W_dev, "torch.float64"),
         None if Phi_dev is None else _dev_ptr(Phi_dev, "torch.float64"), _stream_ptr(stream)))
+
+
+def cos_det_workspace_bytes(n, n_blocks, precision, batch):
+    """Bytes of device scratch cos_det_eval needs (-1 on bad arguments)."""
+    return int(load_library().cos_det_workspace_bytes(int(n), int(n_blocks), int(precision), int(batch)))
+
+
+def cos_det_eval(n, n_flavors, n_blocks, shifts, precision, G_dev, batch, out_dev, work_dev, stream=None):
+    """Determinant-polynomial route (Eq. 34-38): all 2^n-1 connected values of every configuration.
+    precision: COS_DET_FP64 or COS_DET_DD (double-double).  G_dev: torch.float64 CUDA [n_blocks*n*n, batch];
+    out_dev: [2^n-1, batch]; work_dev: any contiguous CUDA tensor of at least
+    cos_det_workspace_bytes(n, n_blocks, precision, batch) bytes (torch allocations are suitably aligned)."""
+    keep, p = _shifts_arg(shifts)
+    if not work_dev.is_cuda or not work_dev.is_contiguous():
+        raise ValueError("work_dev must be a contiguous CUDA tensor")
+    _check(load_library().cos_det_eval(
+        int(n), int(n_flavors), int(n_blocks), p, int(precision), _dev_ptr(G_dev, "torch.float64"), int(batch),
+        _dev_ptr(out_dev, "torch.float64"), work_dev.data_ptr(), int(work_dev.numel() * work_dev.element_size()),
+        _stream_ptr(stream)))
 
 
 def cos_build(n, n_flavors, lattice, shifts, readout_envelope):

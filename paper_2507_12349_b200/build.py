@@ -12,7 +12,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libcos_b200.so")
-SOURCES = ["cos_capi.cu", "cos_kernels.cu", "cos_compile.cpp"]
+SOURCES = ["cos_capi.cu", "cos_kernels.cu", "cos_det.cu", "cos_compile.cpp"]
 HEADERS = ["cos_compile.h", "cos_kernels.cuh", os.path.join("..", "..", "include", "cos.h")]
 
 NVCC_FLAGS = [

@@ -513,6 +513,57 @@ int cos_flux_weights(int n, unsigned int order_mask, const double* lambda_host, 
     return COS_OK;
 }
 
+long long cos_det_workspace_bytes(int n, int n_blocks, int precision, long long batch)
+{
+    if (n < 1 || n > COS_MAX_N || n_blocks < 1 || n_blocks > 3 || batch < 0 || (precision != COS_DET_FP64 && precision != COS_DET_DD))
+        return -1;
+    const long long elem = precision == COS_DET_DD ? 16 : 8;
+    return elem * (n_blocks + 2) * (1ll << n) * batch + (long long)sizeof(uint32_t) * (1ll << n);
+}
+
+int cos_det_eval(int n, int n_flavors, int n_blocks, const double* shifts, int precision, const double* G_dev,
+                 long long batch, double* out_dev, void* work_dev, long long work_bytes, cos_stream stream)
+{
+    if (n < 1 || n > COS_MAX_N || batch < 0) return fail(COS_EINVAL, "cos_det_eval: bad n or batch");
+    if (precision != COS_DET_FP64 && precision != COS_DET_DD) return fail(COS_EINVAL, "cos_det_eval: bad precision");
+    if (n_flavors != 2 && n_flavors != 3)
+        return fail(COS_EUNSUPPORTED, "cos_det_eval: the local tensor of Eq. 35 is implemented for 2 or 3 flavours");
+    if (n_blocks != 1 && n_blocks != n_flavors) return fail(COS_EINVAL, "cos_det_eval: n_blocks must be 1 or n_flavors");
+    if (batch == 0) return COS_OK;
+    if (!G_dev || !out_dev || !work_dev) return fail(COS_EINVAL, "cos_det_eval: NULL pointer");
+    if (((size_t)work_dev & 15u) != 0) return fail(COS_EINVAL, "cos_det_eval: work_dev must be 16-byte aligned");
+    if (work_bytes < cos_det_workspace_bytes(n, n_blocks, precision, batch))
+        return fail(COS_EINVAL, "cos_det_eval: workspace smaller than cos_det_workspace_bytes");
+    if ((((1ll << n) - 1) * ((batch + 31) / 32)) > 0x7fffffffll)
+        return fail(COS_EUNSUPPORTED, "cos_det_eval: (2^n - 1) * ceil(batch / 32) exceeds the grid limit; split the batch");
+    DetArgs a;
+    a.n = n; a.n_blocks = n_blocks; a.three = n_flavors == 3; a.dd = precision == COS_DET_DD;
+    // kernel flavours 0, 1, 2; with two flavours the middle one is absent and caller flavour 1 takes slot 2
+    const int flav[3] = {0, 1, n_flavors - 1};
+    for (int f = 0; f < 3; ++f) {
+        a.blk[f] = n_blocks == 1 ? 0 : flav[f];
+        a.sigma[f] = shifts ? shifts[flav[f]] : 0.0;
+    }
+    uint32_t off = 0, b = 1;                          // level_off[k] = number of subsets larger than k
+    a.level_off[n] = 0;
+    for (int k = n; k >= 1; --k) {                    // b = binom(n, k)
+        off += b;
+        a.level_off[k - 1] = off;
+        b = b * (uint32_t)k / (uint32_t)(n - k + 1);
+    }
+    a.G = G_dev; a.batch = batch; a.out = out_dev;
+    // working-precision arrays first (16-byte elements need the alignment), the subset order behind them
+    const size_t elem = a.dd ? 16 : 8, plane = ((size_t)1 << n) * (size_t)batch * elem;
+    char* p = (char*)work_dev;
+    a.minors = p; p += plane * n_blocks;
+    a.H = p; p += plane;
+    a.C = p; p += plane;
+    a.order = (uint32_t*)p;
+    cudaError_t e = launch_det_route(a, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, "cos_det_eval: launch");
+    return COS_OK;
+}
+
 int cos_measure_fp64_fma_peak(double* fma_per_s)
 {
     if (!fma_per_s) return fail(COS_EINVAL, "cos_measure_fp64_fma_peak: NULL argument");

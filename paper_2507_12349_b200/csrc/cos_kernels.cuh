@@ -67,6 +67,23 @@ struct FluxArgs {
 };
 cudaError_t launch_flux(const FluxArgs& a, cudaStream_t stream);
 
+// ---- determinant-polynomial route (cos_det.cu; Eq. 34-38)
+#define COS_DET_MAX_N 12
+struct DetArgs {
+    int n, n_blocks, three;              // three = 1: flavours 0, 1, 2; 0: flavours 0 and 2 (the middle one absent)
+    int dd;                              // 1: double-double arithmetic (workspace elements are {hi, lo} pairs), 0: fp64
+    int blk[3];                          // propagator block of each flavour (all 0 when the matrices are flavour-uniform)
+    double sigma[3];                     // shift-close weights (sigma[1] unused with two flavours)
+    uint32_t level_off[COS_DET_MAX_N + 1];   // subsets of size k are order[level_off[k] .. level_off[k-1])
+    const double* G; long long batch;
+    uint32_t* order;                     // [2^n] subsets by decreasing size
+    void* minors;                        // [n_blocks][2^n][batch] elements of the working precision
+    void* H;                             // [2^n][batch]
+    void* C;                             // [2^n][batch] connected values in the working precision
+    double* out;                         // caller's output [2^n-1][batch], fp64
+};
+cudaError_t launch_det_route(const DetArgs& a, cudaStream_t stream);
+
 cudaError_t measure_fp64_fma(double* fma_per_s);
 
 }  // namespace cosb
