@@ -48,6 +48,11 @@ def parse_args():
     ap.add_argument("--batch", type=int, default=0, help="override the configuration count (0 = BASELINE's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--layers", action="store_true", help="print the per-layer table to stderr")
+    ap.add_argument("--route", default="dag", choices=["dag", "det"],
+                    help="dag: the hot path (default, the driver's contract); det: the determinant-polynomial route "
+                         "cos_det_eval (SURVEY 8(f).3) on the same workload, all 2^n-1 subsets, its own JSON line")
+    ap.add_argument("--precision", default="dd", choices=["fp64", "dd"], help="--route det: working precision")
+    ap.add_argument("--order", type=int, default=0, help="--route det: override the order n (0 = the workload's)")
     return ap.parse_args()
 
 
@@ -373,10 +378,80 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_det(args):
+    """Secondary workload (not the driver's line): tabulate -> cos_det_eval on a square-lattice workload; one step =
+    all 2^n-1 connected values of every configuration by Eq. 34-38.  ALU-bound: achieved = terms of Eq. 36 + Eq. 38 per
+    second against the measured fp64 FMA peak (one fp64 FMA per term in fp64; a double-double multiply-add is ~25 fp64
+    operations, so the dd fraction is reported against the same peak and is correspondingly small)."""
+    import torch
+    import paper_2507_12349_b200 as cos
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
+    torch.cuda.set_device(0)
+    dev = torch.device("cuda", 0)
+    cos.load_library()
+    w = workload_of(args)
+    if args.order:
+        w = w.scaled(n=args.order)
+    assert w.lattice == 0, "the determinant route is implemented for the square lattice (d = n)"
+    n, B, nf, nb = w.n, w.batch, w.n_flavors, w.n_blocks
+    prec = cos.COS_DET_DD if args.precision == "dd" else cos.COS_DET_FP64
+    table = table_for(w)
+    v = draw_vertices(w)
+    tab = cos.cos_tab_build(w.lattice, w.L, table.n_blocks, w.beta, w.n_tau, table.data)
+    sites, tau = torch.from_numpy(v["sites"]).to(dev), torch.from_numpy(v["tau"]).to(dev)
+    G = torch.empty((nb * n * n, B), dtype=torch.float64, device=dev)
+    out = torch.empty(((1 << n) - 1, B), dtype=torch.float64, device=dev)
+    work = torch.empty((cos.cos_det_workspace_bytes(n, nb, prec, B) + 7) // 8, dtype=torch.float64, device=dev)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        cos.cos_tabulate(tab, n, sites, tau, B, G, stream)
+        cos.cos_det_eval(n, nf, nb, w.sigmas, prec, G, B, out, work, stream)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    sampler.start()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ev0.record(stream)
+    for _ in range(args.steps):
+        step()
+    ev1.record(stream)
+    torch.cuda.synchronize()
+    clocks = sampler.stop()
+    ms = ev0.elapsed_time(ev1) / args.steps
+    assert bool(torch.isfinite(out).all())
+    # terms of Eq. 36 with a non-vanishing weight: per site of T one of the N_f(N_f-1)/2 flavour pairs or one of the
+    # flavours whose sigma is not zero (a zero sigma removes that choice from the loops) -> (1 + pairs + singles)^n - 1
+    n_single = sum(1 for x in (w.sigmas or ()) if x != 0.0)
+    terms36 = (1 + nf * (nf - 1) // 2 + n_single) ** n - 1
+    terms38 = (3 ** n - 1) // 2 - (2 ** n - 1)
+    fma_peak = cos.cos_measure_fp64_fma_peak()
+    achieved = (terms36 + terms38) * B / (ms * 1e-3)
+    line = {"metric": "det_route_configs_per_s", "value": B / (ms * 1e-3), "unit": UNIT, "n_gpus": 1,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if prec == 0 else "f64x2 (double-double)",
+            "data": "synthetic",
+            "config": config_dict(w, 1, {"route": "determinant-polynomial Eq. 34-38, all %d subsets" % ((1 << n) - 1),
+                                         "terms_eq36_per_config": terms36, "terms_eq36_all_sigma_nonzero": (1 + nf * (nf + 1) // 2) ** n - 1, "terms_eq38_per_config": terms38,
+                                         "workspace_bytes": work.numel() * 8,
+                                         "l2": "minors + moments per step: %.2f GB" % (work.numel() * 8 / 1e9)}),
+            "gpu_launches": 5 * args.steps, "clocks": clocks,
+            "roofline": {"bound": "alu", "kernel": "cos_det_moment_kernel", "achieved": achieved / 1e9,
+                         "peak": fma_peak / 1e9, "unit": "GFMA/s (terms of Eq. 36 + 38 vs fp64 FMA peak)",
+                         "frac": achieved / fma_peak, "traffic": None,
+                         "peak_source": "cos_measure_fp64_fma_peak (measured in this run)"}}
+    print(json.dumps(line), flush=True)
+    cos.cos_tab_free(tab)
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         run_reference(args)
+    elif args.route == "det":
+        run_det(args)
     else:
         run_ours(args)
 

@@ -47,12 +47,13 @@ __device__ __forceinline__ double r_round(double a) { return a; }
 __device__ __forceinline__ double r_fma(double a, double b, double acc) { return fma(a, b, acc); }
 __device__ __forceinline__ double r_scale2(double a, int e) { return ldexp(a, e); }
 
+// Addition with the low parts added in plain fp64 (11 operations instead of 20): the error is bounded by
+// ~2^-104 (|a| + |b|), not by 2^-104 |a + b| -- exactly the kind of bound this route needs, since its tolerance is
+// relative to the sum of absolute values R anyway (include/cos.h).
 __device__ __forceinline__ dd r_add(dd a, dd b)
 {
-    dd s = two_sum(a.hi, b.hi);
-    const dd t = two_sum(a.lo, b.lo);
-    s = quick_two_sum(s.hi, __dadd_rn(s.lo, t.hi));
-    return quick_two_sum(s.hi, __dadd_rn(s.lo, t.lo));
+    const dd s = two_sum(a.hi, b.hi);
+    return quick_two_sum(s.hi, __dadd_rn(s.lo, __dadd_rn(a.lo, b.lo)));
 }
 __device__ __forceinline__ dd r_mul(dd a, dd b)
 {
@@ -191,19 +192,23 @@ __global__ void __launch_bounds__(128) cos_det_minors_kernel(const DetArgs a)
 //   Y subset of U    : sites of S_1 outside S_0 ({12} or {1});   the rest U \ Y is {2}
 //   R_0 subset of F_0, R_1 subset of Y : the sites that take the pair with flavour 2; the others pay sigma_0 / sigma_1
 // term = d_0(S_0) d_1(X + Y) d_2((U \ Y) + R_0 + R_1) sigma_2^|U \ Y| sigma_0^|F_0 \ R_0| sigma_1^|Y \ R_1|, times 2^|T|.
-// The weights (powers of the caller's fp64 sigma, in the working precision) depend only on set sizes, are the same for
-// every configuration, and a vanishing one skips its loop.
+// The weights (powers of the caller's fp64 sigma, in the working precision, tabulated in shared memory) depend only on
+// set sizes and are the same for every configuration; sigma_a = 0 removes the "single a" choice from the loops.
 template <class R, bool THREE>
 __global__ void __launch_bounds__(256) cos_det_moment_kernel(const DetArgs a)
 {
-    __shared__ R pw[3][COS_DET_MAX_N + 1];
+    __shared__ R pw2[COS_DET_MAX_N + 1];                              // sigma_2^k
+    __shared__ R pw01[COS_DET_MAX_N + 1][COS_DET_MAX_N + 1];          // sigma_0^k0 sigma_1^k1
     __shared__ R red[8][32];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    if (threadIdx.x < 3 * (COS_DET_MAX_N + 1)) {
-        const int f = threadIdx.x / (COS_DET_MAX_N + 1), e = threadIdx.x % (COS_DET_MAX_N + 1);
-        R p = r_from<R>(1.0);
-        for (int i = 0; i < e; ++i) p = r_muld(p, a.sigma[f]);
-        pw[f][e] = p;
+    if (threadIdx.x < (COS_DET_MAX_N + 1) * (COS_DET_MAX_N + 1)) {
+        const int k0 = threadIdx.x / (COS_DET_MAX_N + 1), k1 = threadIdx.x % (COS_DET_MAX_N + 1);
+        R p = r_from<R>(1.0), q = r_from<R>(1.0);
+        for (int i = 0; i < k0; ++i) p = r_muld(p, a.sigma[0]);
+        for (int i = 0; i < k1; ++i) p = r_muld(p, a.sigma[1]);
+        for (int i = 0; i < k1; ++i) q = r_muld(q, a.sigma[2]);
+        pw01[k0][k1] = p;
+        if (k0 == 0) pw2[k1] = q;
     }
     __syncthreads();
     const uint32_t n_T = (1u << a.n) - 1u;                   // blockIdx.x = tile * n_T + rank: a tile's subsets are neighbours
@@ -216,6 +221,9 @@ __global__ void __launch_bounds__(256) cos_det_moment_kernel(const DetArgs a)
     const R* m1 = (const R*)a.minors + ((size_t)a.blk[1] << a.n) * B + c;
     const R* m2 = (const R*)a.minors + ((size_t)a.blk[2] << a.n) * B + c;
     const int kT = __popc(T);
+    // sigma_f = 0: no site may pay that counterterm, so the sites of that class are forced into the pair with flavour 2
+    // (sigma_0, sigma_1) or Y must be all of U (sigma_2)
+    const bool z0 = a.sigma[0] == 0.0, z1 = a.sigma[1] == 0.0, z2 = a.sigma[2] == 0.0;
     R acc = r_from<R>(0.0);
     for (uint32_t k = w; k < (1u << kT); k += 8) {
         const uint32_t S0 = deposit_bits(k, T), U = T & ~S0;
@@ -224,27 +232,39 @@ __global__ void __launch_bounds__(256) cos_det_moment_kernel(const DetArgs a)
             const uint32_t F0 = S0 & ~X;
             for (uint32_t Y = THREE ? U : 0u;; Y = (Y - 1) & U) {
                 const uint32_t base = U & ~Y;
-                const R w2 = pw[2][__popc(base)];
+                const R w2 = pw2[__popc(base)];
                 if (r_hi(w2) != 0.0) {
+                    // the sites of F0 and Y choose "pair with flavour 2" (in R) or "single" (weight sigma_0 / sigma_1):
+                    // one sub-mask loop over both classes; index of d_2 = fixed | R, weight sigma_0^|F0 \ R| sigma_1^|Y \ R|
+                    const uint32_t fr0 = z0 ? 0u : F0, fr1 = z1 ? 0u : Y, free_ = fr0 | fr1;
+                    const R* p2 = m2 + (size_t)(base | ((F0 | Y) & ~free_)) * B;
                     R inner = r_from<R>(0.0);
-                    for (uint32_t R0 = F0;; R0 = (R0 - 1) & F0) {
-                        const R w0 = pw[0][__popc(F0 & ~R0)];
-                        if (r_hi(w0) != 0.0) {
-                            const R* p2 = m2 + (size_t)(base | R0) * B;
-                            R in1 = r_from<R>(0.0);
-                            for (uint32_t R1 = Y;; R1 = (R1 - 1) & Y) {
-                                const R w1 = pw[1][__popc(Y & ~R1)];
-                                if (r_hi(w1) != 0.0) in1 = r_fma(w1, r_load(p2, (size_t)R1 * B), in1);
-                                if (R1 == 0u) break;
-                            }
-                            inner = r_fma(w0, in1, inner);
+                    if (__popc(free_) < 2) {
+                        for (uint32_t Rr = free_;; Rr = (Rr - 1) & free_) {
+                            inner = r_fma(pw01[__popc(fr0 & ~Rr)][__popc(fr1 & ~Rr)], r_load(p2, (size_t)Rr * B), inner);
+                            if (Rr == 0u) break;
                         }
-                        if (R0 == 0u) break;
+                    } else {
+                        // four sub-masks per iteration (the two lowest free sites in / out): four independent look-ups
+                        // in flight instead of one dependent load per term
+                        const uint32_t b0 = free_ & (0u - free_), f1 = free_ ^ b0, b1 = f1 & (0u - f1), rest = f1 ^ b1;
+                        const int a0 = (b0 & fr0) ? 1 : 0, a1 = (b1 & fr0) ? 1 : 0;     // class of b0 / b1: 1 = F0, 0 = Y
+                        for (uint32_t Rh = rest;; Rh = (Rh - 1) & rest) {
+                            const int k0 = __popc(fr0 & rest & ~Rh), k1 = __popc(fr1 & rest & ~Rh);
+                            const R* q = p2 + (size_t)Rh * B;
+                            const R v11 = r_load(q, (size_t)(b0 | b1) * B), v01 = r_load(q, (size_t)b1 * B);
+                            const R v10 = r_load(q, (size_t)b0 * B), v00 = r_load(q, 0);
+                            inner = r_fma(pw01[k0][k1], v11, inner);
+                            inner = r_fma(pw01[k0 + a0][k1 + 1 - a0], v01, inner);                  // b0 single
+                            inner = r_fma(pw01[k0 + a1][k1 + 1 - a1], v10, inner);                  // b1 single
+                            inner = r_fma(pw01[k0 + a0 + a1][k1 + 2 - a0 - a1], v00, inner);        // both single
+                            if (Rh == 0u) break;
+                        }
                     }
                     if (THREE) inner = r_mul(inner, r_load(m1, (size_t)(X | Y) * B));
                     accS0 = r_fma(w2, inner, accS0);
                 }
-                if (Y == 0u) break;
+                if (Y == 0u || (z2 && THREE)) break;
             }
             if (X == 0u) break;
         }

@@ -283,6 +283,63 @@ def test_o2_absolute_is_the_distinct_colour_part_of_M(n, nf):
     assert close(typed_connected_sum(A, s, nf, distinct_colours_only=True), typed_connected_sum(A, s, nf), scale=M)
 
 
+def _set_partitions(items):
+    if not items:
+        yield []
+        return
+    first, rest = items[0], items[1:]
+    for part in _set_partitions(rest):
+        for i in range(len(part)):
+            yield part[:i] + [[first] + part[i]] + part[i + 1:]
+        yield [[first]] + part
+
+
+@pytest.mark.parametrize("n,nf", [(2, 2), (3, 2), (3, 3), (4, 3)])
+def test_o2b_route_scale_is_the_unsigned_cumulant_formula(n, nf):
+    """O2b with absolute=2 (tolerance scale of the fp64 / double-double determinant route): Eq. 38 is the
+    moment-cumulant relation, whose closed form is C(T) = sum over set partitions pi of T of
+    (-1)^(|pi|-1) (|pi|-1)! prod_B H(B); with every term positive on |A|, |sigma| the scale must equal
+    sum_pi (|pi|-1)! prod_B Habs(B).  Habs(B) is written out from Eq. 35-36 with itertools permanents (no oracle code),
+    and the signed formula on numpy determinants pins Eq. 38 / reading G14 (proper subsets) once more."""
+    rng = np.random.default_rng(700 + 10 * n + nf)
+    A = rng.standard_normal((nf, n, n))
+    sig = rng.standard_normal(nf) * 0.5
+    options = [(a,) for a in range(nf)] + list(itertools.combinations(range(nf), 2))      # Eq. 35: one or two flavours
+
+    def minor(M, S, absolute):
+        if not S:
+            return 1.0
+        if absolute:
+            return sum(np.prod([abs(M[S[i], S[p[i]]]) for i in range(len(S))]) for p in itertools.permutations(range(len(S))))
+        return float(np.linalg.det(M[np.ix_(S, S)]))
+
+    def moment(B, absolute):
+        total = 0.0
+        for choice in itertools.product(options, repeat=len(B)):
+            w = 1.0
+            for o in choice:
+                s = sig[o[0]] if len(o) == 1 else 1.0
+                w *= 2.0 * (abs(s) if absolute else s)
+            for a in range(nf):
+                w *= minor(A[a], [B[i] for i in range(len(B)) if a in choice[i]], absolute)
+            total += w
+        return total
+
+    import math
+    R = oracle.o2b_polynomial(A, sig, absolute=2)
+    C = oracle.o2b_polynomial(A, sig)
+    for T in range(1, 1 << n):
+        verts = [i for i in range(n) if T >> i & 1]
+        scale = signed = 0.0
+        for part in _set_partitions(verts):
+            k = len(part)
+            scale += math.factorial(k - 1) * np.prod([moment(sorted(b), True) for b in part])
+            signed += (-1) ** (k - 1) * math.factorial(k - 1) * np.prod([moment(sorted(b), False) for b in part])
+        assert close(R[T - 1], scale, rtol=1e-10), (T, R[T - 1], scale)
+        assert close(C[T - 1], signed, scale=scale, rtol=1e-10), (T, C[T - 1], signed)
+        assert R[T - 1] >= oracle.o2b_polynomial(A, sig, absolute=True)[T - 1] * (1 - 1e-12) >= abs(C[T - 1]) * (1 - 1e-9)
+
+
 def test_determinant_route_precision_at_n10():
     """the determinant recursion needs more than fp64/x87 precision.  On benchmark-shaped
     propagators (diagonal -rho ~ -0.5, off-diagonal ~ 1e-2) at n = 10 the connected value is ~ 1e-28 while the
