@@ -283,7 +283,14 @@ static int eval_range(cos_handle h, const double* G_dev, long long batch, double
                     if (cap > 1024) cap = 1024;
                     cap = env_int("COS_MASKS_CAP", (int)cap);
                     if (mpc > cap) mpc = cap;
-                    if (mpc < 2 * h->warps_per_cta) mpc = 2 * h->warps_per_cta;
+                    // small layers (few blocks x few tiles): one wave of CTAs, so that every block finds a warp at once
+                    // (a block is walked by ONE warp, latency-bound), but never more than two blocks per warp
+                    long long floor_ = (P.n_masks * (long long)tiles + (long long)h->n_sm * h->ctas_per_sm - 1) /
+                                       ((long long)h->n_sm * h->ctas_per_sm);
+                    if (floor_ > 2 * h->warps_per_cta) floor_ = 2 * h->warps_per_cta;
+                    floor_ = env_int("COS_MASKS_FLOOR", (int)floor_);
+                    if (floor_ < 1) floor_ = 1;
+                    if (mpc < floor_) mpc = floor_;
                 }
                 while ((P.n_masks + mpc - 1) / mpc > 65535) mpc *= 2;
                 a.masks_per_cta = (uint32_t)mpc;
