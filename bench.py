@@ -392,21 +392,20 @@ def run_det(args):
     w = workload_of(args)
     if args.order:
         w = w.scaled(n=args.order)
-    assert w.lattice == 0, "the determinant route is implemented for the square lattice (d = n)"
     n, B, nf, nb = w.n, w.batch, w.n_flavors, w.n_blocks
     prec = cos.COS_DET_DD if args.precision == "dd" else cos.COS_DET_FP64
     table = table_for(w)
     v = draw_vertices(w)
     tab = cos.cos_tab_build(w.lattice, w.L, table.n_blocks, w.beta, w.n_tau, table.data)
     sites, tau = torch.from_numpy(v["sites"]).to(dev), torch.from_numpy(v["tau"]).to(dev)
-    G = torch.empty((nb * n * n, B), dtype=torch.float64, device=dev)
+    G = torch.empty((nb * w.d * w.d, B), dtype=torch.float64, device=dev)
     out = torch.empty(((1 << n) - 1, B), dtype=torch.float64, device=dev)
     work = torch.empty((cos.cos_det_workspace_bytes(n, nb, prec, B) + 7) // 8, dtype=torch.float64, device=dev)
     stream = torch.cuda.current_stream()
 
     def step():
         cos.cos_tabulate(tab, n, sites, tau, B, G, stream)
-        cos.cos_det_eval(n, nf, nb, w.sigmas, prec, G, B, out, work, stream)
+        cos.cos_det_eval(n, nf, nb, w.sigmas, prec, G, B, out, work, stream, lattice=w.lattice)
 
     for _ in range(max(args.warmup, 3)):
         step()
@@ -426,6 +425,8 @@ def run_det(args):
     # flavours whose sigma is not zero (a zero sigma removes that choice from the loops) -> (1 + pairs + singles)^n - 1
     n_single = sum(1 for x in (w.sigmas or ()) if x != 0.0)
     terms36 = (1 + nf * (nf - 1) // 2 + n_single) ** n - 1
+    n_assign = 2 ** n if w.lattice == 1 else 1          # honeycomb: every sublattice assignment is walked
+    terms36 *= n_assign
     terms38 = (3 ** n - 1) // 2 - (2 ** n - 1)
     fma_peak = cos.cos_measure_fp64_fma_peak()
     achieved = (terms36 + terms38) * B / (ms * 1e-3)
@@ -437,7 +438,7 @@ def run_det(args):
                                          "terms_eq36_per_config": terms36, "terms_eq36_all_sigma_nonzero": (1 + nf * (nf + 1) // 2) ** n - 1, "terms_eq38_per_config": terms38,
                                          "workspace_bytes": work.numel() * 8,
                                          "l2": "minors + moments per step: %.2f GB" % (work.numel() * 8 / 1e9)}),
-            "gpu_launches": 5 * args.steps, "clocks": clocks,
+            "gpu_launches": (3 + 2 * n_assign) * args.steps, "clocks": clocks,
             "roofline": {"bound": "alu", "kernel": "cos_det_moment_kernel", "achieved": achieved / 1e9,
                          "peak": fma_peak / 1e9, "unit": "GFMA/s (terms of Eq. 36 + 38 vs fp64 FMA peak)",
                          "frac": achieved / fma_peak, "traffic": None,

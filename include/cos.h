@@ -163,7 +163,11 @@ int cos_flux_weights(int n, unsigned int order_mask, const double* lambda_host, 
  * H(T) = sum_{S_a} prod_a d_a(S_a) prod_i L_i with the local tensor of Eq. 35 (a site of T carries a pair of flavours
  * a < b with weight 2, or one flavour a with weight 2 sigma_a; reading G13 of DESIGN.md for two flavours), connected
  * values C(T) = H(T) - sum_{S proper subset of T, min T in S} C(S) H(T \ S) (Eq. 38; proper subsets, reading G14).
- * H has the physical convention of Eq. 83 (no shift-shift term), like cos_eval.  Square lattice (d = n) only.
+ * H has the physical convention of Eq. 83 (no shift-shift term), like cos_eval.
+ *   lattice    COS_LATTICE_SQUARE (d = n), or COS_LATTICE_HONEYCOMB (d = 2n, endpoint a = 2i + s): the moments are
+ *              summed over the 2^|T| sublattice labels of the vertices of T before Eq. 38 (Eq. 54-55)
+ *              -- the sublattice-summed value the honeycomb DAG returns.  Implemented by walking all 2^n assignments
+ *              (2^n times the square-lattice cost; every H(T) is met 2^(n-|T|) times and that power of two divided out).
  *   n_flavors  2 or 3 (COS_EUNSUPPORTED otherwise).
  *   n_blocks   n_flavors (one n x n matrix per flavour) or 1 (flavour-uniform: every flavour reads block 0; with
  *              shifts = NULL this is the uniform CoS value with loop factor N_f, Eq. 33).
@@ -171,7 +175,7 @@ int cos_flux_weights(int n, unsigned int order_mask, const double* lambda_host, 
  *   precision  COS_DET_FP64: every step in fp64.  COS_DET_DD: every step (elimination, moments, Eq. 38) in
  *              double-double arithmetic, ~106 significant bits, as the paper does for this route;
  *              inputs are the caller's fp64 values, taken as exact; outputs are rounded to fp64 at the end.
- *   G_dev      device fp64 [n_blocks][n][n][batch], the layout of cos_eval (read-only).
+ *   G_dev      device fp64 [n_blocks][d][d][batch], the layout of cos_eval (read-only).
  *   out_dev    device fp64 [2^n-1][batch], written: row bitmask(T)-1, the layout of an all-subset cos_eval.
  *   work_dev   device scratch of at least cos_det_workspace_bytes(n, n_blocks, precision, batch) bytes, 16-byte aligned,
  *              owned by the caller; work_bytes is its size (too small or misaligned: COS_EINVAL).
@@ -182,8 +186,9 @@ int cos_flux_weights(int n, unsigned int order_mask, const double* lambda_host, 
  * Cost: 7^n (three flavours) or 4^n (two) terms per configuration.  Asynchronous on `stream`. */
 enum { COS_DET_FP64 = 0, COS_DET_DD = 1 };
 long long cos_det_workspace_bytes(int n, int n_blocks, int precision, long long batch);      /* -1 on bad arguments */
-int cos_det_eval(int n, int n_flavors, int n_blocks, const double* shifts, int precision, const double* G_dev,
-                 long long batch, double* out_dev, void* work_dev, long long work_bytes, cos_stream stream);
+int cos_det_eval(int n, int n_flavors, int n_blocks, int lattice, const double* shifts, int precision,
+                 const double* G_dev, long long batch, double* out_dev, void* work_dev, long long work_bytes,
+                 cos_stream stream);
 
 /* ---- measurement helpers ------------------------------------------------------------------------------
  * cos_set_profiling(h, 1): every later cos_eval brackets each layer launch with CUDA events on its stream.

@@ -84,7 +84,7 @@ def load_library():
     lib.cos_det_workspace_bytes.restype = ctypes.c_longlong
     lib.cos_det_workspace_bytes.argtypes = [ip, ip, ip, ctypes.c_longlong]
     lib.cos_det_eval.restype = ctypes.c_int
-    lib.cos_det_eval.argtypes = [ip, ip, ip, dp, ip, vp, ctypes.c_longlong, vp, vp, ctypes.c_longlong, vp]
+    lib.cos_det_eval.argtypes = [ip, ip, ip, ip, dp, ip, vp, ctypes.c_longlong, vp, vp, ctypes.c_longlong, vp]
     lib.cos_measure_fp64_fma_peak.restype = ctypes.c_int
     lib.cos_measure_fp64_fma_peak.argtypes = [dp]
     _lib = lib
@@ -140,16 +140,18 @@ def cos_det_workspace_bytes(n, n_blocks, precision, batch):
     return int(load_library().cos_det_workspace_bytes(int(n), int(n_blocks), int(precision), int(batch)))
 
 
-def cos_det_eval(n, n_flavors, n_blocks, shifts, precision, G_dev, batch, out_dev, work_dev, stream=None):
+def cos_det_eval(n, n_flavors, n_blocks, shifts, precision, G_dev, batch, out_dev, work_dev, stream=None,
+                 lattice=COS_LATTICE_SQUARE):
     """Determinant-polynomial route (Eq. 34-38): all 2^n-1 connected values of every configuration.
-    precision: COS_DET_FP64 or COS_DET_DD (double-double).  G_dev: torch.float64 CUDA [n_blocks*n*n, batch];
+    precision: COS_DET_FP64 or COS_DET_DD (double-double).  G_dev: torch.float64 CUDA [n_blocks*d*d, batch], d = n (square)
+    or 2n (lattice=COS_LATTICE_HONEYCOMB: sublattice-summed, Eq. 54-55);
     out_dev: [2^n-1, batch]; work_dev: any contiguous CUDA tensor of at least
     cos_det_workspace_bytes(n, n_blocks, precision, batch) bytes (torch allocations are suitably aligned)."""
     keep, p = _shifts_arg(shifts)
     if not work_dev.is_cuda or not work_dev.is_contiguous():
         raise ValueError("work_dev must be a contiguous CUDA tensor")
     _check(load_library().cos_det_eval(
-        int(n), int(n_flavors), int(n_blocks), p, int(precision), _dev_ptr(G_dev, "torch.float64"), int(batch),
+        int(n), int(n_flavors), int(n_blocks), int(lattice), p, int(precision), _dev_ptr(G_dev, "torch.float64"), int(batch),
         _dev_ptr(out_dev, "torch.float64"), work_dev.data_ptr(), int(work_dev.numel() * work_dev.element_size()),
         _stream_ptr(stream)))
 

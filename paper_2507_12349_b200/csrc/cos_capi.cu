@@ -528,10 +528,12 @@ long long cos_det_workspace_bytes(int n, int n_blocks, int precision, long long 
     return elem * (n_blocks + 2) * (1ll << n) * batch + (long long)sizeof(uint32_t) * (1ll << n);
 }
 
-int cos_det_eval(int n, int n_flavors, int n_blocks, const double* shifts, int precision, const double* G_dev,
-                 long long batch, double* out_dev, void* work_dev, long long work_bytes, cos_stream stream)
+int cos_det_eval(int n, int n_flavors, int n_blocks, int lattice, const double* shifts, int precision,
+                 const double* G_dev, long long batch, double* out_dev, void* work_dev, long long work_bytes,
+                 cos_stream stream)
 {
     if (n < 1 || n > COS_MAX_N || batch < 0) return fail(COS_EINVAL, "cos_det_eval: bad n or batch");
+    if (lattice != COS_LATTICE_SQUARE && lattice != COS_LATTICE_HONEYCOMB) return fail(COS_EINVAL, "cos_det_eval: bad lattice");
     if (precision != COS_DET_FP64 && precision != COS_DET_DD) return fail(COS_EINVAL, "cos_det_eval: bad precision");
     if (n_flavors != 2 && n_flavors != 3)
         return fail(COS_EUNSUPPORTED, "cos_det_eval: the local tensor of Eq. 35 is implemented for 2 or 3 flavours");
@@ -545,6 +547,7 @@ int cos_det_eval(int n, int n_flavors, int n_blocks, const double* shifts, int p
         return fail(COS_EUNSUPPORTED, "cos_det_eval: (2^n - 1) * ceil(batch / 32) exceeds the grid limit; split the batch");
     DetArgs a;
     a.n = n; a.n_blocks = n_blocks; a.three = n_flavors == 3; a.dd = precision == COS_DET_DD;
+    a.nsub = lattice == COS_LATTICE_HONEYCOMB ? 2 : 1; a.assign = 0; a.accumulate = 0;
     // kernel flavours 0, 1, 2; with two flavours the middle one is absent and caller flavour 1 takes slot 2
     const int flav[3] = {0, 1, n_flavors - 1};
     for (int f = 0; f < 3; ++f) {

@@ -151,9 +151,13 @@ __global__ void __launch_bounds__(128) cos_det_minors_kernel(const DetArgs a)
     for (int i = 0; i < n; ++i)
         if (S >> i & 1u) v[k++] = i;
     R M[COS_DET_MAX_N * COS_DET_MAX_N];
-    const double* A = a.G + (size_t)blk * n * n * a.batch + c;
+    // endpoint of vertex i under the current sublattice assignment: i * n_sub + s_i (include/cos.h); d = n * n_sub
+    const int d = n * a.nsub;
+    if (a.nsub == 2)
+        for (int r = 0; r < k; ++r) v[r] = 2 * v[r] + (int)(a.assign >> v[r] & 1u);
+    const double* A = a.G + (size_t)blk * d * d * a.batch + c;
     for (int r = 0; r < k; ++r)
-        for (int q = 0; q < k; ++q) M[r * k + q] = r_from<R>(A[(size_t)(v[r] * n + v[q]) * a.batch]);
+        for (int q = 0; q < k; ++q) M[r * k + q] = r_from<R>(A[(size_t)(v[r] * d + v[q]) * a.batch]);
     R det = r_from<R>(1.0);
     for (int p = 0; p < k; ++p) {
         int piv = p;
@@ -276,7 +280,11 @@ __global__ void __launch_bounds__(256) cos_det_moment_kernel(const DetArgs a)
         R s = red[0][lane];
 #pragma unroll
         for (int i = 1; i < 8; ++i) s = r_add(s, red[i][lane]);
-        r_store((R*)a.H, (size_t)T * B + c, r_scale2(s, kT));
+        // honeycomb: H^{(s)}(T) depends only on the labels of the sites of T, and all 2^n assignments are walked, so every
+        // value is met 2^(n - |T|) times: the exact power of two is divided out here (Eq. 54-55)
+        s = r_scale2(s, a.nsub == 2 ? 2 * kT - a.n : kT);
+        if (a.accumulate) s = r_add(s, r_load((const R*)a.H, (size_t)T * B + c));
+        r_store((R*)a.H, (size_t)T * B + c, s);
     }
 }
 
@@ -320,11 +328,18 @@ static cudaError_t launch_det_route_t(const DetArgs& a, cudaStream_t stream)
     const uint32_t tiles = (uint32_t)((a.batch + 31) / 32);
     cos_det_order_kernel<<<(n_sub + 255) / 256, 256, 0, stream>>>(a.n, a.order);
     const uint32_t n_minors = (uint32_t)a.n_blocks << a.n;
-    cos_det_minors_kernel<R><<<dim3(tiles, (n_minors + 3) / 4), dim3(32, 4), 0, stream>>>(a);
-    if (a.three)
-        cos_det_moment_kernel<R, true><<<(n_sub - 1) * tiles, 256, 0, stream>>>(a);
-    else
-        cos_det_moment_kernel<R, false><<<(n_sub - 1) * tiles, 256, 0, stream>>>(a);
+    // honeycomb (Eq. 54-55): the moments are summed over the sublattice labels of the vertices before Eq. 38 (the
+    // connected part of the summed moments is the sum of the connected parts: labels factorise over components)
+    DetArgs b = a;
+    for (uint32_t assign = 0; assign < (a.nsub == 2 ? n_sub : 1u); ++assign) {
+        b.assign = assign;
+        b.accumulate = assign > 0;
+        cos_det_minors_kernel<R><<<dim3(tiles, (n_minors + 3) / 4), dim3(32, 4), 0, stream>>>(b);
+        if (a.three)
+            cos_det_moment_kernel<R, true><<<(n_sub - 1) * tiles, 256, 0, stream>>>(b);
+        else
+            cos_det_moment_kernel<R, false><<<(n_sub - 1) * tiles, 256, 0, stream>>>(b);
+    }
     cos_det_connected_kernel<R><<<tiles, 256, 0, stream>>>(a);
     return cudaGetLastError();
 }

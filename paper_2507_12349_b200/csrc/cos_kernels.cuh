@@ -72,6 +72,9 @@ cudaError_t launch_flux(const FluxArgs& a, cudaStream_t stream);
 struct DetArgs {
     int n, n_blocks, three;              // three = 1: flavours 0, 1, 2; 0: flavours 0 and 2 (the middle one absent)
     int dd;                              // 1: double-double arithmetic (workspace elements are {hi, lo} pairs), 0: fp64
+    int nsub;                            // 1 square; 2 honeycomb: the launcher walks all 2^n sublattice assignments
+    uint32_t assign;                     // current assignment (bit i = sublattice of vertex i)
+    int accumulate;                      // moment kernel adds to H instead of overwriting it
     int blk[3];                          // propagator block of each flavour (all 0 when the matrices are flavour-uniform)
     double sigma[3];                     // shift-close weights (sigma[1] unused with two flavours)
     uint32_t level_off[COS_DET_MAX_N + 1];   // subsets of size k are order[level_off[k] .. level_off[k-1])

@@ -30,8 +30,8 @@ def cos():
     return cos_mod
 
 
-def det_eval(cos, G, n, nf, sigmas, prec=0):
-    """G: numpy [n_blocks][n][n][B] -> numpy [2^n-1][B] through cos_det_eval."""
+def det_eval(cos, G, n, nf, sigmas, prec=0, lattice=0):
+    """G: numpy [n_blocks][d][d][B] -> numpy [2^n-1][B] through cos_det_eval."""
     import torch
     B = G.shape[-1]
     nb = G.shape[0]
@@ -40,15 +40,15 @@ def det_eval(cos, G, n, nf, sigmas, prec=0):
     nbytes = cos.cos_det_workspace_bytes(n, nb, prec, B)
     assert nbytes > 0
     work = torch.empty((nbytes + 7) // 8, dtype=torch.float64, device="cuda")
-    cos.cos_det_eval(n, nf, nb, sigmas, prec, Gd, B, out, work)
+    cos.cos_det_eval(n, nf, nb, sigmas, prec, Gd, B, out, work, lattice=lattice)
     torch.cuda.synchronize()
     return out.cpu().numpy()
 
 
-def dag_eval(cos, G, n, nf, sigmas):
+def dag_eval(cos, G, n, nf, sigmas, lattice=0):
     import torch
     B = G.shape[-1]
-    h = cos.cos_build(n, nf, cos.COS_LATTICE_SQUARE, sigmas, n)
+    h = cos.cos_build(n, nf, lattice, sigmas, n)
     try:
         Gd = torch.from_numpy(np.ascontiguousarray(G.reshape(-1, B))).cuda()
         out = torch.full(((1 << n) - 1, B), float("nan"), dtype=torch.float64, device="cuda")
@@ -132,7 +132,7 @@ def _tabulated(cos, w):
     v = draw_vertices(w)
     tab = cos.cos_tab_build(w.lattice, w.L, table.n_blocks, w.beta, w.n_tau, table.data)
     try:
-        G = torch.empty((w.n_blocks * w.n * w.n, w.batch), dtype=torch.float64, device="cuda")
+        G = torch.empty((w.n_blocks * w.d * w.d, w.batch), dtype=torch.float64, device="cuda")
         cos.cos_tabulate(tab, w.n, torch.from_numpy(v["sites"]).cuda(), torch.from_numpy(v["tau"]).cuda(), w.batch, G)
         torch.cuda.synchronize()
     finally:
@@ -200,6 +200,77 @@ def test_det_route_config4_full(cos):
     assert np.median(rel) <= 1e-9 and np.max(rel) <= 1e-5, (np.median(rel), np.max(rel))
 
 
+# ------------------------------------------------------------------------------------------------ honeycomb (Eq. 54-55)
+@pytest.mark.parametrize("prec", PRECISIONS)
+@pytest.mark.parametrize("n,nf", [(1, 2), (2, 2), (2, 3), (3, 2), (3, 3), (4, 2)])
+def test_det_route_honeycomb_vs_bruteforce(cos, n, nf, prec):
+    """Sublattice-summed route (moments summed over the 2^|T| labels before Eq. 38) against the sum over assignments of
+    the brute-force connected sums O1 (Eq. 55), every subset; scale R = sum over assignments of the route's scale."""
+    B = 9 if n < 4 else 3
+    sig = [0.3, -0.3, 0.1][:nf]
+    G = random_matrices(9500 + 10 * n + nf, nf, 2 * n, B, scale=0.7)
+    got = det_eval(cos, G, n, nf, sig, prec, lattice=cos.COS_LATTICE_HONEYCOMB)
+    for c in range(B):
+        Gc = np.ascontiguousarray(G[..., c])
+        ref = oracle.connected_reference(Gc, n, 2, nf, sig, False, True, tier="o1")
+        R = oracle.connected_reference(Gc, n, 2, nf, sig, False, True, tier="o2b", absolute=2)
+        check(got[:, c], ref, R, ("honeycomb o1", n, nf, c), TOL[0])
+
+
+@pytest.mark.parametrize("prec", PRECISIONS)
+@pytest.mark.parametrize("n", [5, 6])
+def test_det_route_honeycomb_config3_shape_vs_dag(cos, n, prec):
+    """Config-3-shaped inputs (honeycomb, two spins, opposite shifts, tabulated 2x2 sublattice blocks) at reduced order:
+    the sublattice-summed determinant route vs the oracle (sum over assignments of O2b in binary128) on sampled
+    configurations, and in double-double vs the honeycomb DAG with all-subset readouts on every configuration."""
+    w = get_config(3).scaled(batch=65, n=n)
+    G = _tabulated(cos, w)
+    Gn = G.cpu().numpy().reshape(w.n_blocks, 2 * n, 2 * n, w.batch)
+    sig = list(w.sigmas)
+    got_det = det_eval(cos, Gn, n, 2, sig, prec, lattice=cos.COS_LATTICE_HONEYCOMB)
+    got_dag = dag_eval(cos, Gn, n, 2, sig, lattice=cos.COS_LATTICE_HONEYCOMB)
+    for c in (0, 64):
+        Gc = np.ascontiguousarray(Gn[..., c])
+        ref = oracle.connected_reference(Gc, n, 2, 2, sig, False, True, tier="o2b")
+        R = oracle.connected_reference(Gc, n, 2, 2, sig, False, True, tier="o2b", absolute=2)
+        M = oracle.connected_reference(Gc, n, 2, 2, sig, False, True, tier="o2b", absolute=True)
+        # the reference adds the 2^|T| per-assignment values in fp64, so it is itself only good to ~1e-16 M: the fp64 route
+        # is held to its own bound 1e-10 R, the double-double route to the DAG's (much smaller) 1e-10 M
+        check(got_det[:, c], ref, R if prec == 0 else M, ("honeycomb det", n, c), 1e-10)
+        check(got_dag[:, c], ref, M, ("honeycomb dag", n, c), 1e-10)
+    if prec == 1:
+        rel = np.abs(got_det - got_dag) / np.abs(got_dag)
+        assert np.max(rel) <= 1e-9, np.max(rel)
+
+
+def test_det_route_honeycomb_config3_n10_sampled(cos):
+    """BASELINE config 3 at its order (n = 10, honeycomb, 4.2e8-edge DAG) on its first 128 configurations: the
+    double-double sublattice-summed determinant route (1024 assignments) against the DAG's output on every one of them,
+    and against the oracle (sum over assignments of the two-determinant route O2a', binary128) on one."""
+    import torch
+    w = get_config(3).scaled(batch=128)
+    n = w.n
+    G = _tabulated(cos, w)
+    out = torch.full(((1 << n) - 1, w.batch), float("nan"), dtype=torch.float64, device="cuda")
+    work = torch.empty((cos.cos_det_workspace_bytes(n, 2, cos.COS_DET_DD, w.batch) + 7) // 8, dtype=torch.float64,
+                       device="cuda")
+    cos.cos_det_eval(n, 2, 2, w.sigmas, cos.COS_DET_DD, G, w.batch, out, work, lattice=cos.COS_LATTICE_HONEYCOMB)
+    h = cos.cos_build(n, 2, cos.COS_LATTICE_HONEYCOMB, w.sigmas, 0)
+    try:
+        dag = torch.empty((1, w.batch), dtype=torch.float64, device="cuda")
+        cos.cos_eval(h, G, w.batch, dag)
+        torch.cuda.synchronize()
+    finally:
+        cos.cos_free(h)
+    det_full, dag_full = out[-1].cpu().numpy(), dag[0].cpu().numpy()
+    assert np.all(np.isfinite(det_full))
+    rel = np.abs(det_full - dag_full) / np.abs(dag_full)
+    assert np.median(rel) <= 1e-8 and np.max(rel) <= 1e-4, (np.median(rel), np.max(rel))
+    Gc = np.ascontiguousarray(G[:, 5].cpu().numpy().reshape(2, 2 * n, 2 * n))
+    ref = oracle.connected_reference(Gc, n, 2, 2, w.sigmas, False, False, tier="o2a")[0]
+    assert abs(det_full[5] - ref) <= 1e-6 * abs(ref) and abs(dag_full[5] - ref) <= 1e-6 * abs(ref), (det_full[5], dag_full[5], ref)
+
+
 def test_det_route_edge_cases_and_errors(cos):
     import torch
     n, nf = 3, 3
@@ -223,6 +294,9 @@ def test_det_route_edge_cases_and_errors(cos):
     assert cos.cos_det_workspace_bytes(0, 1, 0, 4) == -1 and cos.cos_det_workspace_bytes(13, 1, 0, 4) == -1
     assert cos.cos_det_workspace_bytes(3, 1, 2, 4) == -1
     assert cos.cos_det_workspace_bytes(3, 3, 1, 4) > cos.cos_det_workspace_bytes(3, 3, 0, 4) > 0
+    with pytest.raises(cos.CosError) as e:
+        cos.cos_det_eval(n, 3, 3, None, 0, Gd, 4, out, work, lattice=2)
+    assert e.value.code == cos.COS_EINVAL
     for args, code in (((n, 4, 4, None, 0, Gd, 4, out, work), cos.COS_EUNSUPPORTED),
                        ((n, 3, 2, None, 0, Gd, 4, out, work), cos.COS_EINVAL),
                        ((n, 3, 3, None, 7, Gd, 4, out, work), cos.COS_EINVAL),
