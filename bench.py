@@ -218,7 +218,14 @@ def run_ours(args):
     assert torch.cuda.is_available(), "bench.py needs a CUDA device (no CPU fallback)"
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
-    if world > 1:
+    use_dist = world > 1 or bool(os.environ.get("COS_BENCH_FORCE_DIST"))     # the latter: exercise NCCL with one rank
+    json_out = sys.stdout
+    if use_dist:
+        # stdout carries the one JSON line and nothing else: NCCL prints its version banner to file descriptor 1 when the
+        # communicator is created, so fd 1 points at stderr from here on and the line goes to a duplicate of the real one
+        sys.stdout.flush()
+        json_out = os.fdopen(os.dup(1), "w")
+        os.dup2(2, 1)
         dist.init_process_group("nccl", device_id=dev)
     cos.load_library()
 
@@ -249,7 +256,7 @@ def run_ours(args):
 
     def barrier():
         torch.cuda.synchronize()
-        if world > 1:
+        if use_dist:
             dist.barrier()
         torch.cuda.synchronize()
 
@@ -369,11 +376,12 @@ def run_ours(args):
                 ms = layer_ms[l] / max(n_prof, 1)
                 gb = 8.0 * (s_in + s_out) * B / 1e9
                 sys.stderr.write("%3d %10d %10.4f %10.1f\n" % (l, s_in, ms, gb / (ms * 1e-3) if ms > 0 else 0.0))
-        print(json.dumps(line), flush=True)
+        json_out.write(json.dumps(line) + "\n")
+        json_out.flush()
 
     cos.cos_free(h)
     cos.cos_tab_free(tab)
-    if world > 1:
+    if use_dist:
         dist.barrier()
         dist.destroy_process_group()
 
