@@ -119,3 +119,24 @@ def test_sb_colour_scaling(cos):
     finally:
         cos.cos_free(hu)
         cos.cos_free(hs)
+
+
+def test_det_route_argument_checks_need_no_gpu(cos):
+    """cos_det_workspace_bytes is pure arithmetic; cos_det_eval validates its arguments before touching CUDA."""
+    lib = cos.load_library()
+    n, nb, B = 10, 3, 8192
+    assert cos.cos_det_workspace_bytes(n, nb, cos.COS_DET_FP64, B) == 8 * (nb + 2) * 2 ** n * B + 4 * 2 ** n
+    assert cos.cos_det_workspace_bytes(n, nb, cos.COS_DET_DD, B) == 16 * (nb + 2) * 2 ** n * B + 4 * 2 ** n
+    assert cos.cos_det_workspace_bytes(n, 4, 0, B) == -1 and cos.cos_det_workspace_bytes(n, nb, 0, -1) == -1
+    p = ctypes.c_void_p(256)
+    for args, code in (((0, 3, 3, 0, None, 0, p, 4, p, p, 1 << 30, None), cos.COS_EINVAL),            # n
+                       ((4, 5, 5, 0, None, 0, p, 4, p, p, 1 << 30, None), cos.COS_EUNSUPPORTED),      # flavours
+                       ((4, 3, 2, 0, None, 0, p, 4, p, p, 1 << 30, None), cos.COS_EINVAL),            # blocks
+                       ((4, 3, 3, 2, None, 0, p, 4, p, p, 1 << 30, None), cos.COS_EINVAL),            # lattice
+                       ((4, 3, 3, 0, None, 5, p, 4, p, p, 1 << 30, None), cos.COS_EINVAL),            # precision
+                       ((4, 3, 3, 0, None, 0, None, 4, p, p, 1 << 30, None), cos.COS_EINVAL),         # NULL input
+                       ((4, 3, 3, 0, None, 1, p, 4, p, ctypes.c_void_p(264), 1 << 30, None), cos.COS_EINVAL),   # alignment
+                       ((4, 3, 3, 0, None, 0, p, 4, p, p, 64, None), cos.COS_EINVAL)):                # workspace size
+        assert lib.cos_det_eval(*args) == code, args
+        assert cos.cos_last_error()
+    assert lib.cos_det_eval(4, 3, 3, 0, None, 0, p, 0, p, p, 0, None) == cos.COS_OK                  # batch 0: no-op
