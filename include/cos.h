@@ -182,7 +182,8 @@ int cos_flux_weights(int n, unsigned int order_mask, const double* lambda_host, 
  * Accuracy: Eq. 38 subtracts from H(T) every disconnected product of smaller moments, so the rounding error of the
  * route scales with R(T) = the same recursion with every term positive on |A|, |sigma| (>= the DAG's M, which has
  * only the connected terms): |error| ~ 1e-15 R in fp64, ~1e-30 R in double-double.  On physical propagators
- * |C| / R falls from ~1e-8 (n = 6) to ~1e-22 (n = 10): fp64 is a cross-check up to n ~ 6, double-double to n ~ 11.
+ * |C| / R falls from ~1e-8 (n = 6) to ~1e-22 (n = 10): fp64 is a cross-check up to n ~ 6, double-double to n ~ 10-11
+ * (at n = 12, beta = 8 it keeps ~5 digits of the full-order value).
  * Cost: 7^n (three flavours) or 4^n (two) terms per configuration.  Asynchronous on `stream`. */
 enum { COS_DET_FP64 = 0, COS_DET_DD = 1 };
 long long cos_det_workspace_bytes(int n, int n_blocks, int precision, long long batch);      /* -1 on bad arguments */

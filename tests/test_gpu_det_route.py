@@ -271,6 +271,69 @@ def test_det_route_honeycomb_config3_n10_sampled(cos):
     assert abs(det_full[5] - ref) <= 1e-6 * abs(ref) and abs(dag_full[5] - ref) <= 1e-6 * abs(ref), (det_full[5], dag_full[5], ref)
 
 
+def _dag_full(cos, w, G):
+    import torch
+    h = cos.cos_build(w.n, w.n_flavors, w.lattice, w.sigmas, w.n if w.all_subsets else 0)
+    try:
+        out = torch.empty((w.n_out, w.batch), dtype=torch.float64, device="cuda")
+        cos.cos_eval(h, G, w.batch, out)
+        torch.cuda.synchronize()
+        return out
+    finally:
+        cos.cos_free(h)
+
+
+def test_det_route_config2_full_every_output(cos):
+    """BASELINE config 2 at full size (n = 8, two spins, 65,536 configurations x 255 readouts): every output of the DAG
+    against the double-double determinant route (one flavour-uniform block, no shifts: H(T) = 2^|T| det(A[T])^2)."""
+    import torch
+    w = get_config(2)
+    G = _tabulated(cos, w)
+    dag = _dag_full(cos, w, G)
+    det = torch.empty_like(dag)
+    work = torch.empty((cos.cos_det_workspace_bytes(w.n, 1, cos.COS_DET_DD, w.batch) + 7) // 8, dtype=torch.float64,
+                       device="cuda")
+    cos.cos_det_eval(w.n, 2, 1, None, cos.COS_DET_DD, G, w.batch, det, work)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(det).all())
+    rel = ((det - dag).abs() / dag.abs()).cpu().numpy()
+    # the DAG's fp64 error is ~1e-15 M (the route's, in double-double, is far below), so the relative difference is
+    # ~1e-15 M / |C_S|: among 1.7e7 outputs a few cancel to |C_S| / M ~ 1e-9 (the element-wise 1e-10 M bound is checked
+    # against the oracle on sampled configurations in test_gpu_parity.py::test_config2_full_sampled)
+    assert np.median(rel) <= 1e-13 and np.quantile(rel, 0.9999) <= 1e-10 and np.max(rel) <= 1e-5, \
+        (np.median(rel), np.quantile(rel, 0.9999), np.max(rel))
+    A = np.ascontiguousarray(G[:, 77].cpu().numpy().reshape(w.n, w.n))
+    ref = oracle.o2a_twospin(A, A)
+    check(det[:, 77].cpu().numpy(), ref, oracle.o2b_polynomial(np.stack([A, A]), [0.0, 0.0], absolute=2), "cfg2 det", TOL[1])
+
+
+def test_det_route_config5_precision_limit(cos):
+    """BASELINE config 5 (n = 12, beta = 8, 64 configurations): where the determinant route stops being a cross-check.
+    The connected value is ~1e-27 of the route's scale R here, so even double-double (~1e-32 per operation) keeps only
+    ~5 digits (median) -- the reason the paper's determinant route needs extended precision and the DAG,
+    whose error scales with the connected M, does not.  Gross agreement only; the DAG itself is checked against the
+    binary128 oracle in test_gpu_parity.py::test_config5_full."""
+    import torch
+    w = get_config(5)
+    G = _tabulated(cos, w)
+    dag = _dag_full(cos, w, G)[0].cpu().numpy()
+    out = torch.empty(((1 << w.n) - 1, w.batch), dtype=torch.float64, device="cuda")
+    work = torch.empty((cos.cos_det_workspace_bytes(w.n, 1, cos.COS_DET_DD, w.batch) + 7) // 8, dtype=torch.float64,
+                       device="cuda")
+    cos.cos_det_eval(w.n, 2, 1, None, cos.COS_DET_DD, G, w.batch, out, work)
+    torch.cuda.synchronize()
+    det = out[-1].cpu().numpy()
+    assert np.all(np.isfinite(det))
+    rel = np.abs(det - dag) / np.abs(dag)
+    assert np.median(rel) <= 1e-3, (np.median(rel), np.max(rel))
+    # the lower orders of the same call are resolved: every subset of size <= 8 of configuration 9 against O2a (binary128)
+    A = np.ascontiguousarray(G[:, 9].cpu().numpy().reshape(w.n, w.n))
+    ref = oracle.o2a_twospin(A, A)
+    got = out[:, 9].cpu().numpy()
+    small = np.array([bin(T).count("1") <= 8 for T in range(1, 1 << w.n)])
+    assert np.max(np.abs(got[small] - ref[small]) / np.abs(ref[small])) <= 1e-6
+
+
 def test_det_route_edge_cases_and_errors(cos):
     import torch
     n, nf = 3, 3
