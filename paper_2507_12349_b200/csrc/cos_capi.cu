@@ -543,7 +543,7 @@ int cos_det_eval(int n, int n_flavors, int n_blocks, int lattice, const double* 
     if (((size_t)work_dev & 15u) != 0) return fail(COS_EINVAL, "cos_det_eval: work_dev must be 16-byte aligned");
     if (work_bytes < cos_det_workspace_bytes(n, n_blocks, precision, batch))
         return fail(COS_EINVAL, "cos_det_eval: workspace smaller than cos_det_workspace_bytes");
-    if ((((1ll << n) - 1) * ((batch + 31) / 32)) > 0x7fffffffll)
+    if (batch > 0x7fffffffll || (((1ll << n) - 1) * ((batch + 31) / 32)) > 0x7fffffffll)
         return fail(COS_EUNSUPPORTED, "cos_det_eval: (2^n - 1) * ceil(batch / 32) exceeds the grid limit; split the batch");
     DetArgs a;
     a.n = n; a.n_blocks = n_blocks; a.three = n_flavors == 3; a.dd = precision == COS_DET_DD;

@@ -107,6 +107,13 @@ __device__ __forceinline__ uint32_t deposit_bits(uint32_t k, uint32_t mask)
     return r;
 }
 
+__device__ __forceinline__ size_t wide_mul(uint32_t x, uint32_t y)      // 32 x 32 -> 64 bits, one instruction
+{
+    unsigned long long r;
+    asm("mul.wide.u32 %0, %1, %2;" : "=l"(r) : "r"(x), "r"(y));
+    return (size_t)r;
+}
+
 __device__ __forceinline__ uint32_t binom_u32(int p, int r)
 {
     if (r < 0 || r > p) return 0;
@@ -220,10 +227,10 @@ __global__ void __launch_bounds__(256) cos_det_moment_kernel(const DetArgs a)
     long long c = (long long)(blockIdx.x / n_T) * 32 + lane;
     const bool valid = c < a.batch;
     if (!valid) c = a.batch - 1;
-    const size_t B = (size_t)a.batch;
-    const R* m0 = (const R*)a.minors + ((size_t)a.blk[0] << a.n) * B + c;
-    const R* m1 = (const R*)a.minors + ((size_t)a.blk[1] << a.n) * B + c;
-    const R* m2 = (const R*)a.minors + ((size_t)a.blk[2] << a.n) * B + c;
+    const uint32_t B = (uint32_t)a.batch;                    // < 2^31 (checked by the C-ABI): subset x B is one IMAD.WIDE
+    const R* m0 = (const R*)a.minors + (size_t)((uint32_t)a.blk[0] << a.n) * B + c;
+    const R* m1 = (const R*)a.minors + (size_t)((uint32_t)a.blk[1] << a.n) * B + c;
+    const R* m2 = (const R*)a.minors + (size_t)((uint32_t)a.blk[2] << a.n) * B + c;
     const int kT = __popc(T);
     // sigma_f = 0: no site may pay that counterterm, so the sites of that class are forced into the pair with flavour 2
     // (sigma_0, sigma_1) or Y must be all of U (sigma_2)
@@ -241,11 +248,11 @@ __global__ void __launch_bounds__(256) cos_det_moment_kernel(const DetArgs a)
                     // the sites of F0 and Y choose "pair with flavour 2" (in R) or "single" (weight sigma_0 / sigma_1):
                     // one sub-mask loop over both classes; index of d_2 = fixed | R, weight sigma_0^|F0 \ R| sigma_1^|Y \ R|
                     const uint32_t fr0 = z0 ? 0u : F0, fr1 = z1 ? 0u : Y, free_ = fr0 | fr1;
-                    const R* p2 = m2 + (size_t)(base | ((F0 | Y) & ~free_)) * B;
+                    const R* p2 = m2 + wide_mul(base | ((F0 | Y) & ~free_), B);
                     R inner = r_from<R>(0.0);
                     if (__popc(free_) < 2) {
                         for (uint32_t Rr = free_;; Rr = (Rr - 1) & free_) {
-                            inner = r_fma(pw01[__popc(fr0 & ~Rr)][__popc(fr1 & ~Rr)], r_load(p2, (size_t)Rr * B), inner);
+                            inner = r_fma(pw01[__popc(fr0 & ~Rr)][__popc(fr1 & ~Rr)], r_load(p2, wide_mul(Rr, B)), inner);
                             if (Rr == 0u) break;
                         }
                     } else {
@@ -255,9 +262,9 @@ __global__ void __launch_bounds__(256) cos_det_moment_kernel(const DetArgs a)
                         const int a0 = (b0 & fr0) ? 1 : 0, a1 = (b1 & fr0) ? 1 : 0;     // class of b0 / b1: 1 = F0, 0 = Y
                         for (uint32_t Rh = rest;; Rh = (Rh - 1) & rest) {
                             const int k0 = __popc(fr0 & rest & ~Rh), k1 = __popc(fr1 & rest & ~Rh);
-                            const R* q = p2 + (size_t)Rh * B;
-                            const R v11 = r_load(q, (size_t)(b0 | b1) * B), v01 = r_load(q, (size_t)b1 * B);
-                            const R v10 = r_load(q, (size_t)b0 * B), v00 = r_load(q, 0);
+                            const R* q = p2 + wide_mul(Rh, B);
+                            const R v11 = r_load(q, wide_mul(b0 | b1, B)), v01 = r_load(q, wide_mul(b1, B));
+                            const R v10 = r_load(q, wide_mul(b0, B)), v00 = r_load(q, 0);
                             inner = r_fma(pw01[k0][k1], v11, inner);
                             inner = r_fma(pw01[k0 + a0][k1 + 1 - a0], v01, inner);                  // b0 single
                             inner = r_fma(pw01[k0 + a1][k1 + 1 - a1], v10, inner);                  // b1 single
@@ -265,14 +272,14 @@ __global__ void __launch_bounds__(256) cos_det_moment_kernel(const DetArgs a)
                             if (Rh == 0u) break;
                         }
                     }
-                    if (THREE) inner = r_mul(inner, r_load(m1, (size_t)(X | Y) * B));
+                    if (THREE) inner = r_mul(inner, r_load(m1, wide_mul(X | Y, B)));
                     accS0 = r_fma(w2, inner, accS0);
                 }
                 if (Y == 0u || (z2 && THREE)) break;
             }
             if (X == 0u) break;
         }
-        acc = r_fma(r_load(m0, (size_t)S0 * B), accS0, acc);
+        acc = r_fma(r_load(m0, wide_mul(S0, B)), accS0, acc);
     }
     red[w][lane] = acc;
     __syncthreads();
@@ -283,8 +290,8 @@ __global__ void __launch_bounds__(256) cos_det_moment_kernel(const DetArgs a)
         // honeycomb: H^{(s)}(T) depends only on the labels of the sites of T, and all 2^n assignments are walked, so every
         // value is met 2^(n - |T|) times: the exact power of two is divided out here (Eq. 54-55)
         s = r_scale2(s, a.nsub == 2 ? 2 * kT - a.n : kT);
-        if (a.accumulate) s = r_add(s, r_load((const R*)a.H, (size_t)T * B + c));
-        r_store((R*)a.H, (size_t)T * B + c, s);
+        if (a.accumulate) s = r_add(s, r_load((const R*)a.H, wide_mul(T, B) + c));
+        r_store((R*)a.H, wide_mul(T, B) + c, s);
     }
 }
 
