@@ -433,6 +433,11 @@ def run_det(args):
     # flavours whose sigma is not zero (a zero sigma removes that choice from the loops) -> (1 + pairs + singles)^n - 1
     n_single = sum(1 for x in (w.sigmas or ()) if x != 0.0)
     terms36 = (1 + nf * (nf - 1) // 2 + n_single) ** n - 1
+    sg = tuple(w.sigmas or (0.0,) * nf)
+    if nf == 3 and sg[1] == 0.0:
+        # sigma_1 = 0: the sums over d_1 and d_2 factorise (cos_det.cu): per (S_0, X) 2^|free F_0| + 2^|free U| terms
+        o0, oy = (2 if sg[0] != 0.0 else 1), (2 if sg[2] != 0.0 else 1)
+        terms36 = (3 + o0) ** n + (3 + oy) ** n - 2
     n_assign = 2 ** n if w.lattice == 1 else 1          # honeycomb: every sublattice assignment is walked
     terms36 *= n_assign
     terms38 = (3 ** n - 1) // 2 - (2 ** n - 1)

@@ -204,7 +204,8 @@ __global__ void __launch_bounds__(128) cos_det_minors_kernel(const DetArgs a)
 //   R_0 subset of F_0, R_1 subset of Y : the sites that take the pair with flavour 2; the others pay sigma_0 / sigma_1
 // term = d_0(S_0) d_1(X + Y) d_2((U \ Y) + R_0 + R_1) sigma_2^|U \ Y| sigma_0^|F_0 \ R_0| sigma_1^|Y \ R_1|, times 2^|T|.
 // The weights (powers of the caller's fp64 sigma, in the working precision, tabulated in shared memory) depend only on
-// set sizes and are the same for every configuration; sigma_a = 0 removes the "single a" choice from the loops.
+// set sizes and are the same for every configuration; sigma_a = 0 removes the "single a" choice from the loops, and
+// sigma_1 = 0 lets the sums over d_1 and d_2 factorise.
 template <class R, bool THREE>
 __global__ void __launch_bounds__(256) cos_det_moment_kernel(const DetArgs a)
 {
@@ -241,41 +242,61 @@ __global__ void __launch_bounds__(256) cos_det_moment_kernel(const DetArgs a)
         R accS0 = r_from<R>(0.0);
         for (uint32_t X = THREE ? S0 : 0u;; X = (X - 1) & S0) {
             const uint32_t F0 = S0 & ~X;
-            for (uint32_t Y = THREE ? U : 0u;; Y = (Y - 1) & U) {
-                const uint32_t base = U & ~Y;
-                const R w2 = pw2[__popc(base)];
-                if (r_hi(w2) != 0.0) {
-                    // the sites of F0 and Y choose "pair with flavour 2" (in R) or "single" (weight sigma_0 / sigma_1):
-                    // one sub-mask loop over both classes; index of d_2 = fixed | R, weight sigma_0^|F0 \ R| sigma_1^|Y \ R|
-                    const uint32_t fr0 = z0 ? 0u : F0, fr1 = z1 ? 0u : Y, free_ = fr0 | fr1;
-                    const R* p2 = m2 + wide_mul(base | ((F0 | Y) & ~free_), B);
-                    R inner = r_from<R>(0.0);
-                    if (__popc(free_) < 2) {
-                        for (uint32_t Rr = free_;; Rr = (Rr - 1) & free_) {
-                            inner = r_fma(pw01[__popc(fr0 & ~Rr)][__popc(fr1 & ~Rr)], r_load(p2, wide_mul(Rr, B)), inner);
-                            if (Rr == 0u) break;
-                        }
-                    } else {
-                        // four sub-masks per iteration (the two lowest free sites in / out): four independent look-ups
-                        // in flight instead of one dependent load per term
-                        const uint32_t b0 = free_ & (0u - free_), f1 = free_ ^ b0, b1 = f1 & (0u - f1), rest = f1 ^ b1;
-                        const int a0 = (b0 & fr0) ? 1 : 0, a1 = (b1 & fr0) ? 1 : 0;     // class of b0 / b1: 1 = F0, 0 = Y
-                        for (uint32_t Rh = rest;; Rh = (Rh - 1) & rest) {
-                            const int k0 = __popc(fr0 & rest & ~Rh), k1 = __popc(fr1 & rest & ~Rh);
-                            const R* q = p2 + wide_mul(Rh, B);
-                            const R v11 = r_load(q, wide_mul(b0 | b1, B)), v01 = r_load(q, wide_mul(b1, B));
-                            const R v10 = r_load(q, wide_mul(b0, B)), v00 = r_load(q, 0);
-                            inner = r_fma(pw01[k0][k1], v11, inner);
-                            inner = r_fma(pw01[k0 + a0][k1 + 1 - a0], v01, inner);                  // b0 single
-                            inner = r_fma(pw01[k0 + a1][k1 + 1 - a1], v10, inner);                  // b1 single
-                            inner = r_fma(pw01[k0 + a0 + a1][k1 + 2 - a0 - a1], v00, inner);        // both single
-                            if (Rh == 0u) break;
-                        }
+            // inner_sum(fixed, fr0, fr1) = sum over R subset of (fr0 | fr1) of sigma_0^|fr0 \ R| sigma_1^|fr1 \ R| d_2(fixed | R):
+            // the sites of fr0 (in F0) and fr1 (in Y) choose "pair with flavour 2" (in R) or "single" (weight sigma_0 /
+            // sigma_1); one sub-mask loop over both classes
+            auto inner_sum = [&](const uint32_t fixed, const uint32_t fr0, const uint32_t fr1) -> R {
+                const uint32_t free_ = fr0 | fr1;
+                const R* p2 = m2 + wide_mul(fixed, B);
+                R inner = r_from<R>(0.0);
+                if (__popc(free_) < 2) {
+                    for (uint32_t Rr = free_;; Rr = (Rr - 1) & free_) {
+                        inner = r_fma(pw01[__popc(fr0 & ~Rr)][__popc(fr1 & ~Rr)], r_load(p2, wide_mul(Rr, B)), inner);
+                        if (Rr == 0u) break;
                     }
-                    if (THREE) inner = r_mul(inner, r_load(m1, wide_mul(X | Y, B)));
-                    accS0 = r_fma(w2, inner, accS0);
+                } else {
+                    // four sub-masks per iteration (the two lowest free sites in / out): four independent look-ups
+                    // in flight instead of one dependent load per term
+                    const uint32_t b0 = free_ & (0u - free_), f1 = free_ ^ b0, b1 = f1 & (0u - f1), rest = f1 ^ b1;
+                    const int a0 = (b0 & fr0) ? 1 : 0, a1 = (b1 & fr0) ? 1 : 0;     // class of b0 / b1: 1 = F0, 0 = Y
+                    for (uint32_t Rh = rest;; Rh = (Rh - 1) & rest) {
+                        const int k0 = __popc(fr0 & rest & ~Rh), k1 = __popc(fr1 & rest & ~Rh);
+                        const R* q = p2 + wide_mul(Rh, B);
+                        const R v11 = r_load(q, wide_mul(b0 | b1, B)), v01 = r_load(q, wide_mul(b1, B));
+                        const R v10 = r_load(q, wide_mul(b0, B)), v00 = r_load(q, 0);
+                        inner = r_fma(pw01[k0][k1], v11, inner);
+                        inner = r_fma(pw01[k0 + a0][k1 + 1 - a0], v01, inner);                  // b0 single
+                        inner = r_fma(pw01[k0 + a1][k1 + 1 - a1], v10, inner);                  // b1 single
+                        inner = r_fma(pw01[k0 + a0 + a1][k1 + 2 - a0 - a1], v00, inner);        // both single
+                        if (Rh == 0u) break;
+                    }
                 }
-                if (Y == 0u || (z2 && THREE)) break;
+                return inner;
+            };
+            const uint32_t fr0 = z0 ? 0u : F0;
+            if (THREE && z1) {
+                // sigma_1 = 0: every site of Y pairs with flavour 2, so d_2 is taken at U | (forced part of F0) | R for every
+                // Y: the d_2 sum and the d_1 sum over Y factorise (2^|F0| + 2^|U| terms instead of their product)
+                const R inner = inner_sum(U | (F0 & ~fr0), fr0, 0u);
+                R sumY = r_from<R>(0.0);
+                for (uint32_t Y = U;; Y = (Y - 1) & U) {
+                    const R w2 = pw2[__popc(U & ~Y)];
+                    if (r_hi(w2) != 0.0) sumY = r_fma(w2, r_load(m1, wide_mul(X | Y, B)), sumY);
+                    if (Y == 0u || z2) break;
+                }
+                accS0 = r_fma(inner, sumY, accS0);
+            } else {
+                for (uint32_t Y = THREE ? U : 0u;; Y = (Y - 1) & U) {
+                    const uint32_t base = U & ~Y;
+                    const R w2 = pw2[__popc(base)];
+                    if (r_hi(w2) != 0.0) {
+                        const uint32_t fr1 = z1 ? 0u : Y;
+                        R inner = inner_sum(base | ((F0 | Y) & ~(fr0 | fr1)), fr0, fr1);
+                        if (THREE) inner = r_mul(inner, r_load(m1, wide_mul(X | Y, B)));
+                        accS0 = r_fma(w2, inner, accS0);
+                    }
+                    if (Y == 0u || (z2 && THREE)) break;
+                }
             }
             if (X == 0u) break;
         }
