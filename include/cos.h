@@ -38,8 +38,12 @@ typedef void*                cos_stream;     /* a cudaStream_t (0 / NULL = legac
 enum { COS_OK = 0, COS_EINVAL = 1, COS_ENOMEM = 2, COS_ECUDA = 3, COS_EUNSUPPORTED = 4 };
 enum { COS_LATTICE_SQUARE = 0, COS_LATTICE_HONEYCOMB = 1 };
 
-/* flags for cos_build_ex */
-enum { COS_BUILD_HOST_ONLY = 1 };            /* compile the DAG, do not touch CUDA (cos_eval then fails) */
+/* flags for cos_build_ex / cos_build_orders (bitwise or) */
+enum {
+    COS_BUILD_HOST_ONLY = 1,       /* compile the DAG, do not touch CUDA (cos_eval then fails) */
+    COS_BUILD_NO_FUSED = 2,        /* small DAGs: use the per-layer kernels instead of the single fused launch */
+    COS_BUILD_UNIFORM_SHIFT = 4    /* uniform CoS WITH a counterterm: shifts[0] = sigma = alpha/U (see cos_build) */
+};
 
 /* ---- (1) DAG compiler: PAPER.md:160-265 (canonical keys Eq. 17, 79-80; pruning Eq. 19-24) ----------
  * Enumerates the reachable states (occupancy mask m_i in {0,(1,s),2}, head, endpoint, colour), prunes
@@ -53,10 +57,17 @@ enum { COS_BUILD_HOST_ONLY = 1 };            /* compile the DAG, do not touch CU
  *                   non-NULL  -> SB-CoS: n_flavors blocks, shifts[lam] = sigma_lam = alpha_lam/U
  *                                (shift-close weight), n_flavors values; colour sums
  *                                replace N_f.  n_flavors <= COS_MAX_COLOURS.
+ *                   With COS_BUILD_UNIFORM_SHIFT (cos_build_ex): uniform CoS with a counterterm (PAPER.md:431,
+ *                   Eq. 33; reading G12 of DESIGN.md): one propagator block, factor N_f per closed loop, and
+ *                   the true one-cycle v -> v weighs A[v][v] + sigma/N_f with sigma = shifts[0] (one value).
  *   readout_envelope 0 -> one output per configuration, the full-order value C_{[n]};
  *                   n -> all 2^n-1 subset values (Eq. 5 with N = n); anything else: COS_EINVAL.
  *   out             receives the handle; the caller releases it with cos_free.
- * The values returned by cos_eval follow the physical convention of Eq. 83 (no shift-shift term).  */
+ * The values returned by cos_eval follow the physical convention of Eq. 83 (no shift-shift term).
+ * Structural limits (COS_EUNSUPPORTED, never COS_ENOMEM): n * n_sub <= 24; SB-CoS with more than COS_MAX_COLOURS
+ * flavours; a propagator tile (n_blocks * d * d + n_colours * d entries of 256 bytes) that exceeds the 226 KB of
+ * shared memory of one SM (e.g. honeycomb SB-CoS beyond n = 10 with two flavours); a layer of more than 2^32 - 2 states
+ * or a layer program of more than 2^32 words.  COS_ENOMEM is host or device memory exhaustion only.  */
 int cos_build(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope, cos_handle* out);
 int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope,
                  int flags, cos_handle* out);
@@ -77,16 +88,36 @@ int cos_build_orders(int n, int n_flavors, int lattice, const double* shifts, un
  *   out_dev  device, fp64, written: out_dev[k*batch + c]; k = 0 for readout_envelope = 0, otherwise
  *            k = bitmask(S)-1 with bit i <-> vertex i (2^n-1 rows).
  *   stream   CUDA stream the kernels are enqueued on.  The call is asynchronous: it returns after
- *            enqueueing (launch errors only).  The handle owns a workspace that is grown lazily (a
- *            synchronising cudaMalloc on first use / growth); one cos_eval in flight per handle.
+ *            enqueueing (launch errors only).  The handle owns the layer-slab workspace; one cos_eval in
+ *            flight per handle.  After cos_reserve(h, B) every cos_eval with batch <= B only enqueues
+ *            kernels (no allocation, no synchronisation: it can be captured into a CUDA graph); without
+ *            it the workspace is grown on demand by a synchronising cudaFree + cudaMalloc.
+ * The current CUDA device must be the one the handle was built on (COS_EINVAL otherwise).
  * Large batches are processed in chunks that fit the workspace budget (cos_set_workspace_limit). */
 int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev, cos_stream stream);
+
+/* Allocates the layer-slab workspace for batches of up to `batch` configurations now (synchronous), under the
+ * current workspace limit.  COS_ENOMEM when the device cannot hold it. */
+int cos_reserve(cos_handle h, long long batch);
 
 /* Releases host and device memory of the handle.  cos_free(NULL) is a no-op. */
 void cos_free(cos_handle h);
 
 /* Upper bound (bytes) for the layer-slab workspace of a handle; default 64 GiB. */
 int cos_set_workspace_limit(cos_handle h, long long bytes);
+
+/* Launch tuning of a handle.  These are the ONLY knobs; the library reads no environment variable.  Results do not
+ * depend on them (same arithmetic, same summation order).  Bad parameter or value: COS_EINVAL. */
+enum {
+    COS_TUNE_PREFETCH = 0,           /* L2 look-ahead of the layer kernel, in states (0 = off; default 32) */
+    COS_TUNE_WARPS_PER_CTA = 1,      /* 1..16; default: the CTA size with the most resident warps per SM */
+    COS_TUNE_BLOCKS_PER_CTA_CAP = 2, /* upper bound of occupancy-mask blocks per CTA (0 = default: one per staged table slot) */
+    COS_TUNE_PDL = 3,                /* programmatic dependent launch between layers (default 1) */
+    COS_TUNE_FUSED = 4,              /* small DAGs: 1 = one fused launch (default), 0 = per-layer kernels */
+    COS_TUNE_HOST_SLICES = 5,        /* cos_eval_host: at most this many output slices, 1..8 (default 8; 1 = no second stream) */
+    COS_TUNE_TILES_PER_CHUNK = 6     /* at most this many 32-configuration tiles per workspace chunk (0 = no bound) */
+};
+int cos_set_tuning(cos_handle h, int what, long long value);
 
 /* ---- introspection (SURVEY.md section 5 "metrics") ------------------------------------------------- */
 enum {
@@ -106,6 +137,11 @@ enum {
     COS_INFO_WORKSPACE_BYTES = 13,
     COS_INFO_N_LAUNCHES = 14,     /* kernels launched through this handle so far (cos_eval / cos_eval_host) */
     COS_INFO_ORDER_MASK = 15,     /* requested orders of an all-subset handle (0 for single-output handles) */
+    COS_INFO_N_GROUPS = 16,       /* group records: rows of one block and colour that share their factor loads (Eq. 29-31) */
+    COS_INFO_N_FACTOR_LOADS = 17, /* staged-factor loads per configuration the kernels execute (with sharing) */
+    COS_INFO_N_FACTOR_LOADS_UNSHARED = 18, /* ... one per DAG edge-evaluation, i.e. without Eq. 29-31 */
+    COS_INFO_DEVICE = 19,         /* CUDA device of the handle (-1: host-only) */
+    COS_INFO_FUSED = 20,          /* 1: cos_eval walks the DAG in one fused launch */
     COS_INFO_LAYER_STATES = 100,  /* + layer index */
     COS_INFO_LAYER_EDGES = 200,   /* + layer index: edges leaving that layer (readout edges included) */
     COS_INFO_LAYER_MASKS = 300    /* + layer index */

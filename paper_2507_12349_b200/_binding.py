@@ -13,13 +13,16 @@ _lib = None
 
 COS_OK, COS_EINVAL, COS_ENOMEM, COS_ECUDA, COS_EUNSUPPORTED = 0, 1, 2, 3, 4
 COS_LATTICE_SQUARE, COS_LATTICE_HONEYCOMB = 0, 1
-COS_BUILD_HOST_ONLY = 1
+COS_BUILD_HOST_ONLY, COS_BUILD_NO_FUSED, COS_BUILD_UNIFORM_SHIFT = 1, 2, 4
 COS_DET_FP64, COS_DET_DD = 0, 1
+TUNE = {"prefetch": 0, "warps_per_cta": 1, "blocks_per_cta_cap": 2, "pdl": 3, "fused": 4, "host_slices": 5,
+        "tiles_per_chunk": 6}
 
 INFO = {
     "n_layers": 0, "n_states": 1, "n_edges": 2, "n_readout_edges": 3, "n_out": 4, "max_layer_states": 5,
     "n_masks": 6, "n_rows": 7, "n_fma": 8, "program_bytes": 9, "d": 10, "n_blocks": 11,
     "n_states_unpruned": 12, "workspace_bytes": 13, "n_launches": 14, "order_mask": 15,
+    "n_groups": 16, "n_factor_loads": 17, "n_factor_loads_unshared": 18, "device": 19, "fused": 20,
     "layer_states": 100, "layer_edges": 200, "layer_masks": 300,
 }
 
@@ -27,7 +30,7 @@ EXPORTS = [
     "cos_build", "cos_build_ex", "cos_eval", "cos_free", "cos_set_workspace_limit", "cos_info",
     "cos_last_error", "cos_tab_build", "cos_tabulate", "cos_tab_free", "cos_measure_fp64_fma_peak",
     "cos_eval_host", "cos_set_profiling", "cos_get_layer_times", "cos_build_orders", "cos_flux_weights",
-    "cos_det_workspace_bytes", "cos_det_eval",
+    "cos_det_workspace_bytes", "cos_det_eval", "cos_reserve", "cos_set_tuning",
 ]
 
 
@@ -87,6 +90,10 @@ def load_library():
     lib.cos_det_eval.argtypes = [ip, ip, ip, ip, dp, ip, vp, ctypes.c_longlong, vp, vp, ctypes.c_longlong, vp]
     lib.cos_measure_fp64_fma_peak.restype = ctypes.c_int
     lib.cos_measure_fp64_fma_peak.argtypes = [dp]
+    lib.cos_reserve.restype = ctypes.c_int
+    lib.cos_reserve.argtypes = [vp, ctypes.c_longlong]
+    lib.cos_set_tuning.restype = ctypes.c_int
+    lib.cos_set_tuning.argtypes = [vp, ip, ctypes.c_longlong]
     _lib = lib
     return lib
 
@@ -108,7 +115,8 @@ def _shifts_arg(shifts):
 
 
 def cos_build_ex(n, n_flavors, lattice, shifts, readout_envelope, flags=0):
-    """-> opaque handle (int).  shifts: None (uniform CoS) or a sequence of n_flavors sigma values (SB-CoS)."""
+    """-> opaque handle (int).  shifts: None (uniform CoS), a sequence of n_flavors sigma values (SB-CoS), or one value
+    with COS_BUILD_UNIFORM_SHIFT in flags (uniform CoS with a counterterm)."""
     lib = load_library()
     keep, p = _shifts_arg(shifts)
     h = ctypes.c_void_p()
@@ -130,9 +138,12 @@ def cos_flux_weights(n, order_mask, lambdas, C_dev, Q_dev, batch, W_dev, Phi_dev
     C_dev / Q_dev / Phi_dev: torch.float64 CUDA tensors [2^n-1, batch] (Q_dev, Phi_dev may be None); W_dev: [batch]."""
     lam = (ctypes.c_double * (int(n) + 1))(*[float(x) for x in lambdas])
     _check(load_library().cos_flux_weights(
-        int(n), int(order_mask), ctypes.cast(lam, ctypes.POINTER(ctypes.c_double)), _dev_ptr(C_dev, "torch.float64"),
-        None if Q_dev is None else _dev_ptr(Q_dev, "torch.float64"), int(batch), _dev_ptr(W_dev, "torch.float64"),
-        None if Phi_dev is None else _dev_ptr(Phi_dev, "torch.float64"), _stream_ptr(stream)))
+        int(n), int(order_mask), ctypes.cast(lam, ctypes.POINTER(ctypes.c_double)),
+        _dev_ptr(C_dev, "torch.float64", ((1 << int(n)) - 1) * int(batch), "C_dev"),
+        None if Q_dev is None else _dev_ptr(Q_dev, "torch.float64", ((1 << int(n)) - 1) * int(batch), "Q_dev"), int(batch),
+        _dev_ptr(W_dev, "torch.float64", int(batch), "W_dev"),
+        None if Phi_dev is None else _dev_ptr(Phi_dev, "torch.float64", ((1 << int(n)) - 1) * int(batch), "Phi_dev"),
+        _stream_ptr(stream)))
 
 
 def cos_det_workspace_bytes(n, n_blocks, precision, batch):
@@ -150,10 +161,12 @@ def cos_det_eval(n, n_flavors, n_blocks, shifts, precision, G_dev, batch, out_de
     keep, p = _shifts_arg(shifts)
     if not work_dev.is_cuda or not work_dev.is_contiguous():
         raise ValueError("work_dev must be a contiguous CUDA tensor")
+    d = int(n) * (2 if int(lattice) == COS_LATTICE_HONEYCOMB else 1)
     _check(load_library().cos_det_eval(
-        int(n), int(n_flavors), int(n_blocks), int(lattice), p, int(precision), _dev_ptr(G_dev, "torch.float64"), int(batch),
-        _dev_ptr(out_dev, "torch.float64"), work_dev.data_ptr(), int(work_dev.numel() * work_dev.element_size()),
-        _stream_ptr(stream)))
+        int(n), int(n_flavors), int(n_blocks), int(lattice), p, int(precision),
+        _dev_ptr(G_dev, "torch.float64", int(n_blocks) * d * d * int(batch), "G_dev"), int(batch),
+        _dev_ptr(out_dev, "torch.float64", ((1 << int(n)) - 1) * int(batch), "out_dev"), work_dev.data_ptr(),
+        int(work_dev.numel() * work_dev.element_size()), _stream_ptr(stream)))
 
 
 def cos_build(n, n_flavors, lattice, shifts, readout_envelope):
@@ -167,18 +180,35 @@ def _stream_ptr(stream):
     return getattr(stream, "cuda_stream", stream)
 
 
-def _dev_ptr(t, dtype_name):
+def _dev_ptr(t, dtype_name, numel=0, what="tensor"):
+    """Data pointer of a contiguous CUDA tensor of the given dtype holding at least `numel` elements."""
     import torch
     if not (isinstance(t, torch.Tensor) and t.is_cuda and t.is_contiguous() and str(t.dtype) == dtype_name):
-        raise CosError(COS_EINVAL, "expected a contiguous CUDA tensor of dtype %s" % dtype_name)
+        raise CosError(COS_EINVAL, "%s: expected a contiguous CUDA tensor of dtype %s" % (what, dtype_name))
+    if t.numel() < numel:
+        raise CosError(COS_EINVAL, "%s: %d elements, the call needs %d" % (what, t.numel(), numel))
     return t.data_ptr()
 
 
 def cos_eval(handle, G_dev, batch, out_dev, stream=None):
     """G_dev: torch.float64 CUDA tensor [n_blocks*d*d, batch] (batch contiguous); out_dev: [n_out, batch]."""
     lib = load_library()
-    _check(lib.cos_eval(handle, _dev_ptr(G_dev, "torch.float64"), int(batch), _dev_ptr(out_dev, "torch.float64"),
+    B, d = int(batch), cos_info(handle, "d")
+    _check(lib.cos_eval(handle, _dev_ptr(G_dev, "torch.float64", cos_info(handle, "n_blocks") * d * d * B, "G_dev"), B,
+                        _dev_ptr(out_dev, "torch.float64", cos_info(handle, "n_out") * B, "out_dev"),
                         _stream_ptr(stream)))
+
+
+def cos_reserve(handle, batch):
+    """Allocate the layer-slab workspace for batches up to `batch` now, so that cos_eval only enqueues kernels."""
+    _check(load_library().cos_reserve(handle, int(batch)))
+
+
+def cos_set_tuning(handle, what, value):
+    """what: a key of TUNE ("prefetch", "warps_per_cta", "blocks_per_cta_cap", "pdl", "fused", "host_slices",
+    "tiles_per_chunk") or its integer code."""
+    code = TUNE[what] if isinstance(what, str) else int(what)
+    _check(load_library().cos_set_tuning(handle, code, int(value)))
 
 
 def cos_free(handle):
@@ -209,23 +239,32 @@ def cos_tab_build(lattice, L, n_blocks, beta, n_tau, table_host):
 
 
 def cos_tabulate(tab, n, sites_dev, tau_dev, batch, G_dev, stream=None):
-    _check(load_library().cos_tabulate(tab, int(n), _dev_ptr(sites_dev, "torch.int32"), _dev_ptr(tau_dev, "torch.float64"),
-                                       int(batch), _dev_ptr(G_dev, "torch.float64"), _stream_ptr(stream)))
+    """sites_dev int32 [n,2,batch], tau_dev fp64 [n,batch], G_dev fp64 [n_blocks*d*d, batch] (at least n*n*batch: the
+    library knows the table's block and sublattice counts, the binding checks the part it can)."""
+    n, B = int(n), int(batch)
+    _check(load_library().cos_tabulate(tab, n, _dev_ptr(sites_dev, "torch.int32", n * 2 * B, "sites_dev"),
+                                       _dev_ptr(tau_dev, "torch.float64", n * B, "tau_dev"), B,
+                                       _dev_ptr(G_dev, "torch.float64", n * n * B, "G_dev"), _stream_ptr(stream)))
 
 
-def _host_ptr(t, dtype_name):
+def _host_ptr(t, dtype_name, numel=0, what="tensor"):
     import torch
     if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.is_contiguous() and str(t.dtype) == dtype_name):
-        raise CosError(COS_EINVAL, "expected a contiguous host tensor of dtype %s" % dtype_name)
+        raise CosError(COS_EINVAL, "%s: expected a contiguous host tensor of dtype %s" % (what, dtype_name))
+    if t.numel() < numel:
+        raise CosError(COS_EINVAL, "%s: %d elements, the call needs %d" % (what, t.numel(), numel))
     return t.data_ptr()
 
 
 def cos_eval_host(handle, tab, sites_host, tau_host, batch, out_host, stream=None):
     """Host-buffer pipeline: sites_host int32 [n,2,batch], tau_host fp64 [n,batch], out_host fp64 [n_out,batch]
     (torch CPU tensors, ideally pinned).  Synchronises the stream before returning."""
-    _check(load_library().cos_eval_host(handle, tab, _host_ptr(sites_host, "torch.int32"),
-                                        _host_ptr(tau_host, "torch.float64"), int(batch),
-                                        _host_ptr(out_host, "torch.float64"), _stream_ptr(stream)))
+    B = int(batch)
+    n = cos_info(handle, "n_layers") // 2
+    _check(load_library().cos_eval_host(handle, tab, _host_ptr(sites_host, "torch.int32", n * 2 * B, "sites_host"),
+                                        _host_ptr(tau_host, "torch.float64", n * B, "tau_host"), B,
+                                        _host_ptr(out_host, "torch.float64", cos_info(handle, "n_out") * B, "out_host"),
+                                        _stream_ptr(stream)))
 
 
 def cos_set_profiling(handle, on):
@@ -254,7 +293,8 @@ def cos_measure_fp64_fma_peak():
 def dag_summary(handle):
     """Convenience: the cos_info counters as a dict (host data only)."""
     keys = ["n_layers", "n_states", "n_edges", "n_readout_edges", "n_out", "max_layer_states", "n_masks",
-            "n_rows", "n_fma", "program_bytes", "d", "n_blocks", "n_states_unpruned", "order_mask"]
+            "n_rows", "n_fma", "program_bytes", "d", "n_blocks", "n_states_unpruned", "order_mask", "n_groups",
+            "n_factor_loads", "n_factor_loads_unshared"]
     out = {k: cos_info(handle, k) for k in keys}
     nl = out["n_layers"]
     out["layer_states"] = [cos_info(handle, "layer_states", l) for l in range(nl)]

@@ -25,12 +25,8 @@ int cuda_fail(cudaError_t e, const char* what)
 
 struct DeviceLayer { uint32_t* words = nullptr; uint32_t* mask_off = nullptr; };
 
-int env_int(const char* name, int dflt)
-{
-    const char* s = getenv(name);
-    if (!s || !*s) return dflt;
-    return atoi(s);
-}
+// compile_dag reports structural limits with this prefix; everything else it returns is an out-of-memory condition
+bool is_unsupported(const std::string& err) { return err.compare(0, 12, "unsupported:") == 0; }
 
 }  // namespace
 
@@ -43,9 +39,15 @@ struct cos_handle_s {
     double* ws = nullptr;                 // two ping-pong layer slabs
     size_t ws_bytes = 0;
     long long ws_limit = 64ll << 30;
-    int masks_per_cta = 0;
-    int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148, prefetch = 0, ring = 0, pdl = 1;
-    bool fused = false;                   // small DAG: every layer in one launch (cos_fused_kernel)
+    // launch shape and tuning (cos_set_tuning); nothing here is read from the environment
+    int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148;
+    int prefetch = 32;                    // L2 look-ahead distance in states
+    int blocks_per_cta_cap = 0;           // 0: one block per staged table slot (64 .. 1024)
+    int pdl = 1;                          // programmatic dependent launch between layers
+    int host_slices = 8;                  // cos_eval_host: at most this many output slices (1: no second stream)
+    long long tiles_per_chunk = 0;        // 0: as many batch tiles per workspace chunk as the limit allows
+    bool fused_ok = false;                // small DAG: every layer can run in one launch (cos_fused_kernel)
+    bool fused = false;                   // ... and does
     FusedLayer* fused_layers = nullptr;   // device array
     long long n_launches = 0;
     // profiling (cos_set_profiling): events[k*(NL+1) + l] brackets layer l of the k-th profiled chunk
@@ -100,26 +102,27 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
         return fail(COS_EINVAL, "cos_build: unknown lattice");
     if (readout_envelope != 0 && readout_envelope != n)
         return fail(COS_EINVAL, "cos_build: readout_envelope must be 0 or n");
-    if (shifts && n_flavors > COS_MAX_COLOURS)
+    const bool uniform_shift = (flags & COS_BUILD_UNIFORM_SHIFT) != 0;
+    if (uniform_shift && !shifts) return fail(COS_EINVAL, "cos_build: COS_BUILD_UNIFORM_SHIFT needs shifts[0]");
+    if (shifts && !uniform_shift && n_flavors > COS_MAX_COLOURS)
         return fail(COS_EUNSUPPORTED, "cos_build: SB-CoS supports at most 4 flavours");
     const int nsub = lattice == COS_LATTICE_HONEYCOMB ? 2 : 1;
     if (n * nsub > 24) return fail(COS_EUNSUPPORTED, "cos_build: n * n_sub must be <= 24");
 
     cos_handle_s* h = new (std::nothrow) cos_handle_s();
     if (!h) return fail(COS_ENOMEM, "cos_build: out of host memory");
-    std::string err = compile_dag(n, n_flavors, nsub, shifts, readout_envelope == n, order_mask, h->dag);
-    if (!err.empty()) { delete h; return fail(COS_ENOMEM, "cos_build: " + err); }
+    std::string err = compile_dag(n, n_flavors, nsub, shifts, uniform_shift, readout_envelope == n, order_mask, h->dag);
+    if (!err.empty()) {
+        delete h;
+        return fail(is_unsupported(err) ? COS_EUNSUPPORTED : COS_ENOMEM, "cos_build: " + err);
+    }
 
     const CompiledDag& D = h->dag;
-    const size_t smem = layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d, D.has_shift, 0, 0);
+    const size_t smem = layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d);
     if (smem > LAYER_SMEM_MAX) {
         delete h;
         return fail(COS_EUNSUPPORTED, "cos_build: propagator tile does not fit the 227 KB shared memory of one SM");
     }
-    h->warps_per_cta = 8;
-    h->masks_per_cta = env_int("COS_MASKS_PER_CTA", 0);        // 0: chosen per layer in cos_eval
-    h->prefetch = env_int("COS_PREFETCH", 8);
-    h->pdl = env_int("COS_PDL", 1);
 
     if (!(flags & COS_BUILD_HOST_ONLY)) {
         int ndev = 0;
@@ -131,16 +134,9 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
         cudaGetDevice(&h->device);
         e = configure_layer_kernels();
         if (e != cudaSuccess) { delete h; return cuda_fail(e, "cos_build: cudaFuncSetAttribute"); }
-        // launch shape: the CTA size that keeps the most warps resident per SM for this instantiation
-        e = pick_layer_shape((int)D.max_L, D.nc, D.d, D.n_blocks * D.d * D.d, D.has_shift, env_int("COS_RING", 0),
-                             &h->ring, &h->warps_per_cta, &h->ctas_per_sm);
+        // launch shape: the CTA size that keeps the most warps resident per SM
+        e = pick_layer_shape(D.nc, D.d, D.n_blocks * D.d * D.d, &h->warps_per_cta, &h->ctas_per_sm);
         if (e != cudaSuccess) { delete h; return cuda_fail(e, "cos_build: occupancy query"); }
-        {   // experiment override; the ring must still fit
-            const int w = env_int("COS_WARPS_PER_CTA", h->warps_per_cta);
-            if (w >= 1 && w <= 24 &&
-                layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d, D.has_shift, h->ring, w) <= LAYER_SMEM_MAX)
-                h->warps_per_cta = w;
-        }
         cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
         h->dl.resize(D.layers.size());
         for (size_t l = 0; l < D.layers.size(); ++l) {
@@ -155,19 +151,19 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
             h->program_bytes += wb + mb;
         }
         // small DAGs (orders n <= 6) are launch-latency bound: walk all layers in one kernel
-        bool small = D.n_states <= 16384 && D.max_L <= 12 && env_int("COS_FUSED", 1) != 0;
+        bool small = D.n_states <= 16384;
         for (const auto& P : D.layers) small = small && P.n_masks <= 2048;
         if (small) {
-            e = configure_fused_kernels();
             std::vector<FusedLayer> fl(D.layers.size());
             for (size_t l = 0; l < D.layers.size(); ++l) {
                 fl[l].words = h->dl[l].words; fl[l].mask_off = h->dl[l].mask_off;
                 fl[l].n_masks = D.layers[l].n_masks; fl[l].n_states = D.layers[l].n_states;
             }
-            if (e == cudaSuccess) e = cudaMalloc(&h->fused_layers, fl.size() * sizeof(FusedLayer));
+            e = cudaMalloc(&h->fused_layers, fl.size() * sizeof(FusedLayer));
             if (e == cudaSuccess) e = cudaMemcpy(h->fused_layers, fl.data(), fl.size() * sizeof(FusedLayer), cudaMemcpyHostToDevice);
             if (e != cudaSuccess) { cos_free(h); return cuda_fail(e, "cos_build: fused-path setup"); }
-            h->fused = true;
+            h->fused_ok = true;
+            h->fused = !(flags & COS_BUILD_NO_FUSED);
         }
         h->on_device = true;
         // the host copy of the program is no longer needed
@@ -209,6 +205,85 @@ int cos_set_workspace_limit(cos_handle h, long long bytes)
     return COS_OK;
 }
 
+// The handle's device must be the current one: its program, workspace and the caller's pointers live there.
+static int check_device(cos_handle h, const char* who)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, who);
+    if (dev != h->device)
+        return fail(COS_EINVAL, std::string(who) + ": the current CUDA device is not the one the handle was built on");
+    return COS_OK;
+}
+
+// Batch tiles per workspace chunk for a batch of `batch` configurations, and the bytes that chunk needs.
+static long long chunk_tiles(cos_handle h, long long batch, size_t* bytes)
+{
+    const CompiledDag& D = h->dag;
+    const long long tiles_total = (batch + TILE - 1) / TILE;
+    const size_t tile_bytes = (size_t)D.max_layer_states * TILE * sizeof(double) * 2;
+    long long tiles_chunk = (long long)((size_t)h->ws_limit / tile_bytes);
+    if (tiles_chunk < 1) tiles_chunk = 1;
+    if (tiles_chunk > tiles_total) tiles_chunk = tiles_total;
+    if (h->tiles_per_chunk > 0 && tiles_chunk > h->tiles_per_chunk) tiles_chunk = h->tiles_per_chunk;
+    *bytes = tile_bytes * (size_t)tiles_chunk;
+    return tiles_chunk;
+}
+
+static int grow_workspace(cos_handle h, size_t need, const char* who)
+{
+    if (need <= h->ws_bytes) return COS_OK;
+    if (h->ws) { cudaFree(h->ws); h->ws = nullptr; h->ws_bytes = 0; }
+    cudaError_t e = cudaMalloc(&h->ws, need);
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, who); }
+    h->ws_bytes = need;
+    return COS_OK;
+}
+
+int cos_reserve(cos_handle h, long long batch)
+{
+    if (!h || batch < 0) return fail(COS_EINVAL, "cos_reserve: bad argument");
+    if (!h->on_device) return fail(COS_ECUDA, "cos_reserve: handle was built host-only (no CPU fallback)");
+    int rc = check_device(h, "cos_reserve");
+    if (rc != COS_OK || batch == 0) return rc;
+    size_t need = 0;
+    chunk_tiles(h, batch, &need);
+    return grow_workspace(h, need, "cos_reserve: workspace allocation");
+}
+
+int cos_set_tuning(cos_handle h, int what, long long value)
+{
+    if (!h) return fail(COS_EINVAL, "cos_set_tuning: handle is NULL");
+    switch (what) {
+        case COS_TUNE_PREFETCH:
+            if (value < 0 || value > 4096) return fail(COS_EINVAL, "cos_set_tuning: prefetch distance must be in [0, 4096]");
+            h->prefetch = (int)value; break;
+        case COS_TUNE_WARPS_PER_CTA:
+            if (value < 1 || value > 16) return fail(COS_EINVAL, "cos_set_tuning: warps per CTA must be in [1, 16]");
+            h->warps_per_cta = (int)value;
+            if (h->on_device) {       // resident CTAs per SM for the new shape (sizes the grid waves)
+                const CompiledDag& D = h->dag;
+                int c = 0;
+                if (layer_ctas_per_sm(D.nc, D.d, D.n_blocks * D.d * D.d, (int)value, &c) == cudaSuccess && c > 0) h->ctas_per_sm = c;
+                else cudaGetLastError();
+            }
+            break;
+        case COS_TUNE_BLOCKS_PER_CTA_CAP:
+            if (value < 0 || value > 65535) return fail(COS_EINVAL, "cos_set_tuning: blocks-per-CTA cap must be in [0, 65535]");
+            h->blocks_per_cta_cap = (int)value; break;
+        case COS_TUNE_PDL: h->pdl = value != 0; break;
+        case COS_TUNE_FUSED: h->fused = h->fused_ok && value != 0; break;
+        case COS_TUNE_HOST_SLICES:
+            if (value < 1 || value > 8) return fail(COS_EINVAL, "cos_set_tuning: host slices must be in [1, 8]");
+            h->host_slices = (int)value; break;
+        case COS_TUNE_TILES_PER_CHUNK:
+            if (value < 0) return fail(COS_EINVAL, "cos_set_tuning: tiles per chunk must be >= 0");
+            h->tiles_per_chunk = value; break;
+        default: return fail(COS_EINVAL, "cos_set_tuning: unknown parameter");
+    }
+    return COS_OK;
+}
+
 // Layers + readouts for the batch tiles [tile_begin, tile_end) of a batch of `batch` configurations (G_dev / out_dev are
 // the whole-batch arrays).  clear: zero-fill the output rows of a partial readout set first (whole batch).
 static int eval_range(cos_handle h, const double* G_dev, long long batch, double* out_dev, long long tile_begin,
@@ -218,35 +293,28 @@ static int eval_range(cos_handle h, const double* G_dev, long long batch, double
     const int NL = (int)D.layers.size();
 
     // ---- batch chunking against the workspace budget: two slabs of max_layer_states x 32 doubles per tile
-    const long long tiles_total = (batch + TILE - 1) / TILE;
-    const size_t tile_bytes = (size_t)D.max_layer_states * TILE * sizeof(double) * 2;
-    long long tiles_chunk = (long long)((size_t)h->ws_limit / tile_bytes);
-    if (tiles_chunk < 1) tiles_chunk = 1;
-    if (tiles_chunk > tiles_total) tiles_chunk = tiles_total;
-    const int max_tiles_env = env_int("COS_TILES_PER_CHUNK", 0);
-    if (max_tiles_env > 0 && tiles_chunk > max_tiles_env) tiles_chunk = max_tiles_env;
-    const size_t need = tile_bytes * (size_t)tiles_chunk;
-    if (need > h->ws_bytes) {
-        if (h->ws) { cudaFree(h->ws); h->ws = nullptr; h->ws_bytes = 0; }
-        cudaError_t e = cudaMalloc(&h->ws, need);
-        if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, "cos_eval: workspace allocation"); }
-        h->ws_bytes = need;
-    }
+    size_t need = 0;
+    const long long tiles_chunk = chunk_tiles(h, batch, &need);
+    // (cos_reserve hoists this allocation out of the call; growing here synchronises the device)
+    int rc = grow_workspace(h, need, "cos_eval: workspace allocation");
+    if (rc != COS_OK) return rc;
     double* slab[2] = {h->ws, h->ws + (size_t)D.max_layer_states * TILE * (size_t)tiles_chunk};
 
     if (clear && D.all_subsets && D.order_mask != (((2u << D.n) - 1u) & ~1u)) {     // partial readout set: other rows are zeros
         cudaError_t e = cudaMemsetAsync(out_dev, 0, (size_t)D.n_out * (size_t)batch * sizeof(double), stream);
         if (e != cudaSuccess) return cuda_fail(e, "cos_eval: clearing the output");
     }
+    const int n_slots = D.n_blocks * D.d * D.d;
     for (long long t0 = tile_begin; t0 < tile_end; t0 += tiles_chunk) {
         const uint32_t tiles = (uint32_t)((tile_end - t0 < tiles_chunk) ? (tile_end - t0) : tiles_chunk);
         if (h->fused && !h->profiling) {
             FusedArgs f;
             f.layers = h->fused_layers; f.n_layers = NL; f.ws = h->ws; f.S_max = D.max_layer_states;
-            f.G = G_dev; f.batch = batch; f.b0 = t0 * TILE; f.out = out_dev; f.d = D.d; f.n_slots = D.n_blocks * D.d * D.d;
+            f.G = G_dev; f.batch = batch; f.b0 = t0 * TILE; f.out = out_dev; f.d = D.d; f.nc = D.nc; f.n_slots = n_slots;
+            f.has_shift = D.has_shift ? 1 : 0;
             f.neg_kappa = -D.kappa;
             for (int c = 0; c < 4; ++c) f.sigma[c] = D.sigma[c];
-            cudaError_t ef = launch_fused(f, (int)D.max_L, D.nc, D.has_shift, tiles, 8, stream);
+            cudaError_t ef = launch_fused(f, tiles, 8, stream);
             if (ef != cudaSuccess) return cuda_fail(ef, "cos_eval: fused launch");
             ++h->n_launches;
             continue;
@@ -273,25 +341,21 @@ static int eval_range(cos_handle h, const double* G_dev, long long batch, double
             a.words = h->dl[l].words; a.mask_off = h->dl[l].mask_off;
             a.n_masks = P.n_masks;
             {   // blocks per CTA: amortise the table staging but keep >= 4 waves of CTAs on the GPU
-                long long mpc = h->masks_per_cta;
-                if (mpc <= 0) {
-                    mpc = (long long)P.n_masks * tiles / ((long long)h->n_sm * h->ctas_per_sm * 4);
-                    // staging the table costs one 256-byte line per slot and CTA; a block moves ~30 lines each way:
-                    // about one block per staged slot keeps the staging share at a few percent
-                    long long cap = D.n_blocks * D.d * D.d + (D.has_shift ? D.nc * D.d : 0);
-                    if (cap < 64) cap = 64;
-                    if (cap > 1024) cap = 1024;
-                    cap = env_int("COS_MASKS_CAP", (int)cap);
-                    if (mpc > cap) mpc = cap;
-                    // small layers (few blocks x few tiles): one wave of CTAs, so that every block finds a warp at once
-                    // (a block is walked by ONE warp, latency-bound), but never more than two blocks per warp
-                    long long floor_ = (P.n_masks * (long long)tiles + (long long)h->n_sm * h->ctas_per_sm - 1) /
-                                       ((long long)h->n_sm * h->ctas_per_sm);
-                    if (floor_ > 2 * h->warps_per_cta) floor_ = 2 * h->warps_per_cta;
-                    floor_ = env_int("COS_MASKS_FLOOR", (int)floor_);
-                    if (floor_ < 1) floor_ = 1;
-                    if (mpc < floor_) mpc = floor_;
-                }
+                const long long resident = (long long)h->n_sm * h->ctas_per_sm;
+                long long mpc = (long long)P.n_masks * tiles / (resident * 4);
+                // staging the table costs one 256-byte line per slot and CTA; a block moves ~30 lines each way:
+                // about one block per staged slot keeps the staging share at a few percent
+                long long cap = n_slots + D.nc * D.d;
+                if (cap < 64) cap = 64;
+                if (cap > 1024) cap = 1024;
+                if (h->blocks_per_cta_cap > 0) cap = h->blocks_per_cta_cap;
+                if (mpc > cap) mpc = cap;
+                // small layers (few blocks x few tiles): one wave of CTAs, so that every block finds a warp at once
+                // (a block is walked by ONE warp, latency-bound), but never more than two blocks per warp
+                long long floor_ = (P.n_masks * (long long)tiles + resident - 1) / resident;
+                if (floor_ > 2 * h->warps_per_cta) floor_ = 2 * h->warps_per_cta;
+                if (floor_ < 1) floor_ = 1;
+                if (mpc < floor_) mpc = floor_;
                 while ((P.n_masks + mpc - 1) / mpc > 65535) mpc *= 2;
                 a.masks_per_cta = (uint32_t)mpc;
             }
@@ -300,10 +364,10 @@ static int eval_range(cos_handle h, const double* G_dev, long long batch, double
             a.X = slab[l & 1]; a.Y = slab[(l + 1) & 1];
             a.S_src = P.n_states; a.S_dst = (l + 1 < NL) ? D.layers[l + 1].n_states : 0;
             a.G = G_dev; a.batch = batch; a.b0 = t0 * TILE; a.out = out_dev;
-            a.d = D.d; a.n_slots = D.n_blocks * D.d * D.d;
+            a.d = D.d; a.nc = D.nc; a.n_slots = n_slots; a.has_shift = D.has_shift ? 1 : 0;
             a.neg_kappa = -D.kappa;
             for (int c = 0; c < 4; ++c) a.shift[c] = (l == 0 ? -2.0 : -1.0) * D.sigma[c];
-            e = launch_layer(a, (int)D.max_L, D.nc, D.has_shift, h->ring, tiles, h->warps_per_cta, stream);
+            e = launch_layer(a, tiles, h->warps_per_cta, stream);
             if (e != cudaSuccess) return cuda_fail(e, "cos_eval: layer launch");
             if (P.n_masks) ++h->n_launches;
             if (ev) cudaEventRecord(ev[l + 1], stream);
@@ -319,6 +383,8 @@ int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev
     if (batch == 0) return COS_OK;
     if (!G_dev || !out_dev) return fail(COS_EINVAL, "cos_eval: NULL device pointer");
     if (!h->on_device) return fail(COS_ECUDA, "cos_eval: handle was built host-only / without a CUDA device (no CPU fallback)");
+    int rc = check_device(h, "cos_eval");
+    if (rc != COS_OK) return rc;
     if (h->profiling) ++h->profiled_evals;
     return eval_range(h, G_dev, batch, out_dev, 0, (batch + TILE - 1) / TILE, true, (cudaStream_t)stream_);
 }
@@ -359,6 +425,10 @@ int cos_eval_host(cos_handle h, cos_tab tab, const int* sites_host, const double
     if (batch == 0) return COS_OK;
     if (!sites_host || !tau_host || !out_host) return fail(COS_EINVAL, "cos_eval_host: NULL host pointer");
     if (!h->on_device) return fail(COS_ECUDA, "cos_eval_host: handle was built host-only (no CPU fallback)");
+    {
+        const int rcd = check_device(h, "cos_eval_host");
+        if (rcd != COS_OK) return rcd;
+    }
     const CompiledDag& D = h->dag;
     if (tab->n_blocks != D.n_blocks || tab->nsub != D.nsub)
         return fail(COS_EINVAL, "cos_eval_host: table blocks / lattice do not match the handle");
@@ -390,9 +460,9 @@ int cos_eval_host(cos_handle h, cos_tab tab, const int* sites_host, const double
     // back on a second stream while slice i+1 is evaluated (one strided 2-D copy per slice).
     const long long tiles_total = (batch + TILE - 1) / TILE;
     long long n_slices = (long long)(b_out >> 23);                  // ~8 MiB of output per slice
-    if (n_slices > 8) n_slices = 8;
+    if (n_slices > h->host_slices) n_slices = h->host_slices;
     if (n_slices > tiles_total) n_slices = tiles_total;
-    if (n_slices <= 1 || env_int("COS_HOST_PIPELINE", 1) == 0) {
+    if (n_slices <= 1) {
         rc = eval_range(h, h->st_G, batch, h->st_out, 0, tiles_total, true, stream);
         if (rc != COS_OK) return rc;
         e = cudaMemcpyAsync(out_host, h->st_out, b_out, cudaMemcpyDeviceToHost, stream);
@@ -451,6 +521,11 @@ int cos_info(cos_handle h, int what, long long* value)
         case COS_INFO_WORKSPACE_BYTES: *value = (long long)h->ws_bytes; break;
         case COS_INFO_N_LAUNCHES: *value = h->n_launches; break;
         case COS_INFO_ORDER_MASK: *value = (long long)D.order_mask; break;
+        case COS_INFO_N_GROUPS: *value = (long long)D.n_groups; break;
+        case COS_INFO_N_FACTOR_LOADS: *value = (long long)D.n_factor_loads; break;
+        case COS_INFO_N_FACTOR_LOADS_UNSHARED: *value = (long long)D.n_factor_loads_unshared; break;
+        case COS_INFO_DEVICE: *value = h->device; break;
+        case COS_INFO_FUSED: *value = h->fused ? 1 : 0; break;
         default: return fail(COS_EINVAL, "cos_info: unknown query");
     }
     return COS_OK;

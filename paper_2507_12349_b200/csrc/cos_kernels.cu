@@ -2,29 +2,28 @@
 //
 //  cos_layer_kernel   north_star (3)+(4): one layer step x_t += c_e L[x_s] (Eq. 16) for every
 //                     state of the next layer, plus the terminal readouts of this layer (Eq. 14-15).
+//  cos_fused_kernel   the same for small DAGs: every layer in one launch.
 //  cos_tabulate_kernel north_star (2): propagator lookup with linear tau-interpolation (Eq. 32).
 //  cos_fill_kernel    layer-0 initial states <- 1 (Eq. 66).
 //  fp64 FMA peak probe for the roofline report.
 //
-// Work decomposition of the layer kernel (DESIGN.md section 4):
+// Work decomposition of the layer kernel (DESIGN.md section 4-5):
 //   lane  = configuration (32 per batch tile, the contiguous dimension of every array),
-//   warp  = one occupancy-mask block at a time: all rows (head, colour) of the block,
+//   warp  = one occupancy-mask block at a time: all group records of the block,
 //   CTA   = `masks_per_cta` blocks x one batch tile; the tile's propagator table G (all blocks, d x d,
 //           32 configurations) is staged once in shared memory.
-// For one row the L source values are loaded ONCE into registers (contiguous states, coalesced
-// 256-byte lines), every continuation destination is a length-L dot product against a column of
-// G in shared memory (1 LDS.64 + 1 DFMA per DAG edge), and the cycle-closing sum of the whole block is
-// accumulated in a register.  Every destination state is written exactly once: no atomics, no
-// second pass, HBM traffic = one read + one write per state.
+// A group record is up to 4 rows (heads) of one colour of the block.  The continuation factor G_lambda[e][j] does not
+// depend on the head, so the record is a small product  Y[head][j] = sum_e X[head][e] * G_lambda[e][j]  per
+// configuration: for every source endpoint e the TJ factors are loaded ONCE from shared memory and applied to the TH
+// source values (factor-application sharing, Eq. 29-31), TH x TJ accumulators live in registers, and every
+// source state is read from HBM exactly once, just in time (one step ahead).  Every destination state is written exactly
+// once: no atomics, no second pass, HBM traffic = one read + one write per state.
 #include "cos_kernels.cuh"
 #include "cos_compile.h"
 
 namespace cosb {
 
-static const int MAX_WARPS = 16;
-// CTA size bound per instantiation: the long-row kernels (honeycomb, d = 20) are shared-memory limited to one CTA
-// per SM, so they take 24 warps (<= 85 registers) instead of 16.
-__host__ __device__ constexpr int max_warps_of(int maxl, int ring = 0) { return ring > 0 ? 24 : maxl == 20 ? 20 : MAX_WARPS; }
+static const int MAX_WARPS = 16;         // 128 registers per thread
 
 __device__ __forceinline__ double lds64(uint32_t addr)
 {
@@ -33,6 +32,7 @@ __device__ __forceinline__ double lds64(uint32_t addr)
     return v;
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
 // asynchronous 8-byte global -> shared copy (LDGSTS): no register staging, completion by commit / wait groups
 __device__ __forceinline__ void cp_async8(uint32_t dst, const void* src)
 {
@@ -42,287 +42,237 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// ---- bulk (TMA) copies global -> shared, completion on an mbarrier (used by the source ring, RING > 0)
-__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n\t"
-        ".reg .pred P1;\n\t"
-        "COS_MBAR_WAIT:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n\t"
-        "@P1 bra COS_MBAR_DONE;\n\t"
-        "bra COS_MBAR_WAIT;\n\t"
-        "COS_MBAR_DONE:\n\t"
-        "}" ::"r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void bulk_copy_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
-                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
-}
+// What a warp needs to walk the records of one batch tile.
+struct TileCtx {
+    const char* Xl;                      // source slab of the tile + lane * 8
+    char* Yl;                            // destination slab of the tile + lane * 8
+    uint32_t gs_lane;                    // shared-memory byte address of Gs[0][lane]
+    uint32_t gd_lane;                    // ... of the plain diagonal Gd[0][lane]
+    uint32_t d, dstride;                 // table dimension, d * 256 bytes (one table row of 32 configurations)
+    uint32_t S_src;                      // states of the source layer
+    int prefetch;                        // L2 look-ahead distance in states (0: off)
+    int lane;
+};
 
-// U ordinary destinations of a row at once (program words w0 .. w0+U-1 of the row record): U length-L dot products
-// against U columns of the staged table, 2U independent DFMA chains, U stores.
-#ifndef COS_DEST_WIDE
-#define COS_DEST_WIDE 4
-#endif
-template <int L, int U>
-__device__ __forceinline__ void dest_group(const uint32_t rw, const int w0, const uint32_t (&ra)[L], const double (&x)[L],
-                                           char* const Yb)
+// The source values of endpoint e for the TH heads of a record (0 where a head has no such state).
+template <int TH, bool FUSED>
+__device__ __forceinline__ void load_x(const uint32_t e, double (&x)[TH], uint32_t (&idx)[TH], const uint32_t (&al)[TH],
+                                       const char* __restrict__ Xl)
 {
-    // (ptxas keeps the column offsets in vector registers here: one IMAD.IADD per LDS; only the single-destination
-    // loops get the LDS [R + UR] form)
-    const uint32_t dA = __shfl_sync(0xFFFFFFFFu, rw, w0);
-    const uint32_t dB = U > 1 ? __shfl_sync(0xFFFFFFFFu, rw, w0 + 1) : 0u;
-    const uint32_t dC = U > 2 ? __shfl_sync(0xFFFFFFFFu, rw, w0 + 2) : 0u;
-    const uint32_t dD = U > 3 ? __shfl_sync(0xFFFFFFFFu, rw, w0 + 3) : 0u;
-    const uint32_t jA = __byte_perm(dA, 0u, 0x4434u), jB = __byte_perm(dB, 0u, 0x4434u);   // j_a * 256 bytes
-    const uint32_t jC = __byte_perm(dC, 0u, 0x4434u), jD = __byte_perm(dD, 0u, 0x4434u);
-    double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0, c0 = 0.0, c1 = 0.0, d0 = 0.0, d1 = 0.0;
 #pragma unroll
-    for (int k = 0; k < L; ++k) {
-        if (k & 1) {
-            a1 = fma(lds64(ra[k] + jA), x[k], a1);
-            if (U > 1) b1 = fma(lds64(ra[k] + jB), x[k], b1);
-            if (U > 2) c1 = fma(lds64(ra[k] + jC), x[k], c1);
-            if (U > 3) d1 = fma(lds64(ra[k] + jD), x[k], d1);
-        } else {
-            a0 = fma(lds64(ra[k] + jA), x[k], a0);
-            if (U > 1) b0 = fma(lds64(ra[k] + jB), x[k], b0);
-            if (U > 2) c0 = fma(lds64(ra[k] + jC), x[k], c0);
-            if (U > 3) d0 = fma(lds64(ra[k] + jD), x[k], d0);
+    for (int t = 0; t < TH; ++t) {
+        x[t] = 0.0;
+        if ((al[t] >> e) & 1u) {
+            const double* p = (const double*)(Xl + ((size_t)idx[t] << 8));
+            x[t] = FUSED ? __ldcg(p) : __ldcs(p);
+            ++idx[t];
         }
     }
-    // didx * 256 bytes: didx < 2^24, the shift drops j_a
-    __stcs((double*)(Yb + (size_t)(dA << 8)), a0 + a1);
-    if (U > 1) __stcs((double*)(Yb + (size_t)(dB << 8)), b0 + b1);
-    if (U > 2) __stcs((double*)(Yb + (size_t)(dC << 8)), c0 + c1);
-    if (U > 3) __stcs((double*)(Yb + (size_t)(dD << 8)), d0 + d1);
+}
+
+// One source endpoint e of a record: TJ factor loads, TH x TJ FMAs; the cycle-closing factor G_lambda[e][h] (Eq. 12, 15)
+// is per head and never carries the counterterm (plain diagonal Gd when e == h).
+template <int TH, int TJ>
+__device__ __forceinline__ void apply_e(const uint32_t e, const double (&x)[TH], double (&acc)[TH][TJ > 0 ? TJ : 1],
+                                        double (&cl)[TH], const uint32_t (&joff)[TJ > 0 ? TJ : 1],
+                                        const uint32_t (&hoff)[TH], const uint32_t (&al)[TH], const uint32_t row0,
+                                        const uint32_t dstride, const uint32_t gdl, const bool do_close)
+{
+    const uint32_t ra = row0 + e * dstride;
+    double g[TJ > 0 ? TJ : 1];
+#pragma unroll
+    for (int q = 0; q < TJ; ++q) g[q] = lds64(ra + joff[q]);
+#pragma unroll
+    for (int q = 0; q < TJ; ++q)
+#pragma unroll
+        for (int t = 0; t < TH; ++t) acc[t][q] = fma(g[q], x[t], acc[t][q]);
+    if (do_close) {
+#pragma unroll
+        for (int t = 0; t < TH; ++t)
+            if ((al[t] >> e) & 1u) {
+                const uint32_t p = hoff[t] + ((hoff[t] == (e << 8)) ? gdl : ra);
+                cl[t] = fma(lds64(p), x[t], cl[t]);
+            }
+    }
 }
 
 // ------------------------------------------------------------------------------------------------------
-// One row of a block: L contiguous source states, nJ destinations.
-//   rw       this lane's word of the row record (lane k holds word k)
-//   gs_lane  shared-memory byte address of Gs[0][lane]; row (lambda, e) of the table starts at
-//            gs_lane + (lambda*d + e) * dstride, entry j at + j*256 (dstride = d*256 bytes)
-//   gd_lane  shared-memory byte address of the plain diagonal Gd[0][lane] (SHIFT only)
-//   RING = 0 the L source values are loaded from global memory (xp);
-//   RING > 0 they were copied ahead of time into this warp's shared-memory ring (ring_lane, stream position o)
-// Inner loop per DAG edge: one integer add (address), one LDS.64, one DFMA.
-template <int L, int NC, bool SHIFT, int RING, bool FUSED>
-__device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, const double* __restrict__ xp,
-                                         const uint32_t ring_lane, const uint32_t o,
-                                         const int nJ, const int e_words, const bool need_close,
-                                         const uint32_t d, const uint32_t gs_lane, const uint32_t gd_lane,
-                                         double* __restrict__ Yt, double& close, double (&sp)[NC])
+// One group record (cos_compile.h): TH heads x TJ destination endpoints of one colour.
+template <int TH, int TJ, bool FUSED>
+__device__ __forceinline__ void group_body(const uint4* __restrict__ rec, const uint4 q0, const TileCtx& c,
+                                           double& close, double (&sp)[4])
 {
-    double x[L];
-    uint32_t ra[L];
-    if (RING > 0) {
+    constexpr int TJ1 = TJ > 0 ? TJ : 1;
+    const uint32_t g0 = q0.x, lam = (g0 >> 8) & 3u;
+    const bool do_close = (g0 >> 10) & 1u;
+    uint32_t idx[TH], al[TH], hoff[TH];
 #pragma unroll
-        for (int k = 0; k < L; ++k) x[k] = lds64(ring_lane + (((o + (uint32_t)k) & (uint32_t)(RING - 1)) << 8));
-    } else {
-#pragma unroll
-        for (int k = 0; k < L; ++k) x[k] = FUSED ? __ldcg(xp + (size_t)k * TILE) : __ldcs(xp + (size_t)k * TILE);
+    for (int t = 0; t < TH; ++t) {
+        const uint4 qh = __ldg(rec + 1 + t);
+        idx[t] = qh.x; al[t] = qh.y; hoff[t] = qh.z << 8;
     }
-    const uint32_t dstride = d * (TILE * 8u);
+    if (c.prefetch > 0) {                // L2 look-ahead: the states `prefetch` states further down the slab
+        uint32_t cnt = 0;
 #pragma unroll
-    for (int k = 0; k < L; ++k) {
-        const uint32_t ew = __shfl_sync(0xFFFFFFFFu, rw, 2 + (k >> 2));
-        ra[k] = ((ew >> (8 * (k & 3))) & 0xFFu) * dstride + gs_lane;
-    }
-    const int lam = (int)((rh >> 10) & 3u);
-    if (need_close) {                       // cycle-closing factor G_lam[e][h] (Eq. 12, 15), never shifted
-        const uint32_t h_a = (rh >> 5) & 31u, hoff = h_a * (TILE * 8u);
-        const int kh = (int)((rh >> 12) & 31u);
-        const uint32_t pd = gd_lane + ((uint32_t)lam * d + h_a) * (TILE * 8u);
-        double c0 = 0.0, c1 = 0.0;
-#pragma unroll
-        for (int k = 0; k < L; ++k) {
-            uint32_t p = ra[k] + hoff;
-            if (SHIFT) p = (k == kh) ? pd : p;
-            if (k & 1) c1 = fma(lds64(p), x[k], c1); else c0 = fma(lds64(p), x[k], c0);
+        for (int t = 0; t < TH; ++t) cnt += (uint32_t)__popc(al[t]);
+        const char* X0 = c.Xl - c.lane * 8;
+        for (uint32_t q = (uint32_t)c.lane; q < 2u * cnt; q += 32u) {
+            const uint32_t st = q0.w + (uint32_t)c.prefetch + (q >> 1);
+            if (st < c.S_src) prefetch_l2(X0 + ((size_t)st << 8) + (size_t)(q & 1u) * 128);
         }
-        close += c0 + c1;
     }
-    // destinations: n_live ordinary ones, then (defer) the one that merges with the fresh-head state.  No per-edge
-    // multiplicity (deferred to the readout, cos_compile.h), no pruned entries: SHFL, L x (LDS, DFMA), one store.
-    const int n_live = (int)((rh >> 17) & 31u);
-    char* const Yb = (char*)Yt;
-    int jj = 0;
-    // COS_DEST_WIDE / two / one destination(s) at a time: 2 independent DFMA chains per destination hide the
-    // LDS -> DFMA latency at 20-24 resident warps
-#if COS_DEST_WIDE > 2
-    for (; jj + COS_DEST_WIDE <= n_live; jj += COS_DEST_WIDE) dest_group<L, COS_DEST_WIDE>(rw, 2 + e_words + jj, ra, x, Yb);
-#endif
-    for (; jj + 2 <= n_live; jj += 2) dest_group<L, 2>(rw, 2 + e_words + jj, ra, x, Yb);
-    if (jj < n_live) dest_group<L, 1>(rw, 2 + e_words + jj, ra, x, Yb);
-    if ((rh >> 22) & 1u) {                  // the destination that merges with the fresh-head state (E2/E4 pair)
-        const uint32_t dj = __shfl_sync(0xFFFFFFFFu, rw, 2 + e_words + n_live);
-        const uint32_t joff = __byte_perm(dj, 0u, 0x4434u);
-        double acc0 = 0.0, acc1 = 0.0;
+    uint32_t joff[TJ1];
+    {
+        uint32_t jm = q0.z;
 #pragma unroll
-        for (int k = 0; k < L; ++k) {
-            if (k & 1) acc1 = fma(lds64(ra[k] + joff), x[k], acc1); else acc0 = fma(lds64(ra[k] + joff), x[k], acc0);
+        for (int q = 0; q < TJ; ++q) { joff[q] = (uint32_t)(__ffs((int)jm) - 1) << 8; jm &= jm - 1u; }
+    }
+    const uint32_t row0 = c.gs_lane + lam * c.d * c.dstride;
+    const uint32_t gdl = c.gd_lane + ((lam * c.d) << 8);
+    double acc[TH][TJ1], cl[TH];
+#pragma unroll
+    for (int t = 0; t < TH; ++t) {
+        cl[t] = 0.0;
+#pragma unroll
+        for (int q = 0; q < TJ1; ++q) acc[t][q] = 0.0;
+    }
+    // source endpoints in increasing order, the loads of the next one issued before the FMAs of the current one
+    uint32_t em = q0.y;
+    double xa[TH], xb[TH];
+    uint32_t e0 = (uint32_t)(__ffs((int)em) - 1), e1;
+    em &= em - 1u;
+    load_x<TH, FUSED>(e0, xa, idx, al, c.Xl);
+    for (;;) {
+        e1 = 32u;
+        if (em) { e1 = (uint32_t)(__ffs((int)em) - 1); em &= em - 1u; load_x<TH, FUSED>(e1, xb, idx, al, c.Xl); }
+        apply_e<TH, TJ>(e0, xa, acc, cl, joff, hoff, al, row0, c.dstride, gdl, do_close);
+        if (e1 == 32u) break;
+        e0 = 32u;
+        if (em) { e0 = (uint32_t)(__ffs((int)em) - 1); em &= em - 1u; load_x<TH, FUSED>(e0, xa, idx, al, c.Xl); }
+        apply_e<TH, TJ>(e1, xb, acc, cl, joff, hoff, al, row0, c.dstride, gdl, do_close);
+        if (e0 == 32u) break;
+    }
+    // destinations: one store per live (head, endpoint); the one that merges with the fresh-head state is kept
+    if (TJ > 0) {
+        const uint4* dw = rec + 1 + TH;
+        double spv = 0.0;
+        bool has_sp = false;
+#pragma unroll
+        for (int i = 0; i < (TH * TJ + 3) / 4; ++i) {
+            const uint4 w4 = __ldg(dw + i);
+#pragma unroll
+            for (int k = 0; k < 4; ++k) {
+                const int f = 4 * i + k;
+                if (f < TH * TJ) {
+                    const uint32_t w = k == 0 ? w4.x : k == 1 ? w4.y : k == 2 ? w4.z : w4.w;
+                    const double v = acc[f / TJ1][f % TJ1];
+                    if (w < DIDX_DEFER) {
+                        double* y = (double*)(c.Yl + ((size_t)w << 8));
+                        if (FUSED) *y = v; else __stcs(y, v);
+                    } else if (w == DIDX_DEFER) { spv = v; has_sp = true; }
+                }
+            }
         }
-        const double acc = acc0 + acc1;
 #pragma unroll
-        for (int c = 0; c < NC; ++c) sp[c] = (c == lam) ? acc : sp[c];
+        for (int k = 0; k < 4; ++k) sp[k] = (has_sp && (uint32_t)k == lam) ? spv : sp[k];
+    }
+    if (do_close) {
+        double s = cl[0];
+#pragma unroll
+        for (int t = 1; t < TH; ++t) s += cl[t];
+        close += s;
     }
 }
 
 // All source blocks [m_begin, m_end) of one layer for one batch tile: the body shared by the per-layer kernel and the
 // fused small-DAG kernel.  s_next (shared) must be 0 and visible to the CTA on entry.
-template <int MAXL, int NC, bool SHIFT, int RING, bool FUSED>
+template <bool FUSED>
 __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t m_begin, const uint32_t m_end,
                                              const uint32_t tile, unsigned int& s_next, const uint32_t gs_lane,
-                                             const uint32_t gd_lane, const uint32_t ring_lane, const uint32_t bar_addr,
-                                             const int lane, const bool valid, const long long b)
+                                             const uint32_t gd_lane, const int lane, const bool valid, const long long b)
 {
-    const int HDR = 3 + NC;
-    const double* Xt = a.X + (size_t)tile * a.S_src * TILE + lane;
-    const char* Xt0 = (const char*)(a.X + (size_t)tile * a.S_src * TILE);
-    double* Yt = a.Y + (size_t)tile * a.S_dst * TILE + lane;
+    TileCtx c;
+    c.Xl = (const char*)(a.X + (size_t)tile * a.S_src * TILE + lane);
+    c.Yl = (char*)(a.Y + (size_t)tile * a.S_dst * TILE + lane);
+    c.gs_lane = gs_lane; c.gd_lane = gd_lane; c.d = (uint32_t)a.d; c.dstride = (uint32_t)a.d * (TILE * 8u);
+    c.S_src = a.S_src; c.prefetch = a.prefetch; c.lane = lane;
     const uint2* mtab = (const uint2*)a.mask_off;
 
-    // Blocks are handed to warps dynamically (block sizes vary).  A warp always knows its current AND its next
-    // block: the next block's program window is fetched early, and (RING > 0) the source states of both are
-    // streamed, in slab order, through the warp's shared-memory ring up to RING states ahead of the row in work.
-    //   stream coordinate = running count of the source states of the blocks this warp has taken;
-    //   current block: coordinates [s0, s1), slab index = coordinate + d0;  next block: [s1, s1 + c1), + d1.
+    // Blocks are handed to warps dynamically (block sizes vary).  A warp always knows its current AND its next block:
+    // the next block's header is fetched while the current block is processed.
     uint32_t mi = 0;
     if (lane == 0) mi = atomicAdd(&s_next, 1u);
     mi = __shfl_sync(0xFFFFFFFFu, mi, 0) + m_begin;
-    uint32_t off = 0, hw = 0, rw = 0;
-    uint32_t s1 = 0, d0 = 0, d1 = 0, c1 = 0, front = 0;
-    bool primed = false;
-    uint32_t t = 0;                      // ring copy group counter (one group per row step)
+    const uint4* bp = nullptr;
+    uint4 h0 = make_uint4(0u, 0u, 0u, 0u);
     if (mi < m_end) {
-        const uint2 mt = __ldg(&mtab[mi]);
-        off = mt.x;
-        hw = __ldg(a.words + off + lane);
-        rw = __ldg(a.words + off + HDR + lane);
-        if (RING > 0) { d1 = mt.y; c1 = __ldg(&mtab[mi + 1].y) - mt.y; }     // becomes the current block below
+        bp = (const uint4*)(a.words + __ldg(&mtab[mi]).x);
+        h0 = __ldg(bp);
     }
     while (mi < m_end) {
         uint32_t mi_n = 0;
         if (lane == 0) mi_n = atomicAdd(&s_next, 1u);
         mi_n = __shfl_sync(0xFFFFFFFFu, mi_n, 0) + m_begin;
-        uint32_t off_n = 0, hw_n = 0, rw_n = 0;
-        if (RING > 0) { d0 = d1; s1 += c1; c1 = 0; }                        // next -> current
+        const uint4* bp_n = nullptr;
+        uint4 h0_n = make_uint4(0u, 0u, 0u, 0u);
         if (mi_n < m_end) {
-            const uint2 mt = __ldg(&mtab[mi_n]);
-            off_n = mt.x;
-            hw_n = __ldg(a.words + off_n + lane);
-            rw_n = __ldg(a.words + off_n + HDR + lane);
-            if (RING > 0) { c1 = __ldg(&mtab[mi_n + 1].y) - mt.y; d1 = mt.y - s1; }
-            if (RING == 0 && a.prefetch < 0) {
-                const uint32_t first = mt.y, lines = (__ldg(&mtab[mi_n + 1].y) - first) * 2u;   // 128-byte lines
-                const char* p0 = Xt0 + (size_t)first * (TILE * 8);
-                for (uint32_t i = lane; i < lines; i += 32) prefetch_l2(p0 + (size_t)i * 128);
-            }
+            bp_n = (const uint4*)(a.words + __ldg(&mtab[mi_n]).x);
+            h0_n = __ldg(bp_n);
         }
-
-        const uint32_t w0 = __shfl_sync(0xFFFFFFFFu, hw, 0), w1 = __shfl_sync(0xFFFFFFFFu, hw, 1);
-        const int n_rows = (int)(w0 & 0xFFFFu), nJ = (int)((w0 >> 16) & 0xFFu);
-        const uint32_t flags = w0 >> 24;
-        const int stride = (int)(w1 & 0xFFu), e_words = (int)((w1 >> 8) & 0xFFu);
-        const bool need_close = flags != 0u;
+        const int n_groups = (int)(h0.x & 0xFFFFu);
+        const uint32_t flags = h0.x >> 24;
         double close = 0.0;
-        double sp[NC];
-#pragma unroll
-        for (int c = 0; c < NC; ++c) sp[c] = 0.0;
+        double sp[4] = {0.0, 0.0, 0.0, 0.0};
 
-        const uint32_t* rp = a.words + off + HDR;
-        for (int r = 0; r < n_rows; ++r) {
-            uint32_t rw_next = 0u;
-            if (r + 1 < n_rows) rw_next = __ldg(rp + (size_t)(r + 1) * stride + lane);
-            const uint32_t base = __shfl_sync(0xFFFFFFFFu, rw, 0), rh = __shfl_sync(0xFFFFFFFFu, rw, 1);
-            const int L = (int)(rh & 31u);
-            const double* xp = Xt + (size_t)base * TILE;
-            uint32_t o = 0;
-            if (RING > 0) {
-                // top the ring up to RING states past the start of this row (never past the next block), then
-                // wait for everything but the copies just issued: this row's states were issued a row earlier
-                // (RING >= 2 * MAXL), so they have landed.
-                o = base - d0;
-                const uint32_t hi = min(o + (uint32_t)RING, s1 + c1);
-                __syncwarp();                   // every lane has consumed the ring slots that are about to be reused
-                if (lane == 0) {                // group t: contiguous slab ranges -> ring, at most four bulk copies
-                    const uint32_t bar = bar_addr + ((t & 1u) << 3);
-                    mbar_arrive_expect_tx(bar, (hi - front) * (uint32_t)(TILE * 8));
-                    uint32_t f = front;
-                    while (f < hi) {
-                        uint32_t end = hi;
-                        if (f < s1 && end > s1) end = s1;                              // block boundary
-                        const uint32_t wrap = (f | (uint32_t)(RING - 1)) + 1u;         // ring boundary
-                        if (end > wrap) end = wrap;
-                        const uint32_t g = f + (f < s1 ? d0 : d1);
-                        bulk_copy_g2s(ring_lane - (uint32_t)lane * 8u + ((f & (uint32_t)(RING - 1)) << 8),
-                                      Xt0 + (size_t)g * (TILE * 8), (end - f) * (uint32_t)(TILE * 8), bar);
-                        f = end;
-                    }
-                }
-                // every step waits for the previous group (so each group is observed exactly once, in order); a row
-                // whose states were not all issued by then (the very first row, or one that did not fit the
-                // look-ahead) also waits for the group just issued
-                const bool covered = primed && o + (uint32_t)L <= front;
-                front = hi;
-                if (primed) mbar_wait(bar_addr + (((t - 1u) & 1u) << 3), ((t - 1u) >> 1) & 1u);
-                if (!covered) mbar_wait(bar_addr + ((t & 1u) << 3), (t >> 1) & 1u);
-                primed = true;
-                ++t;
-            } else if (a.prefetch > 0) {     // L2 look-ahead: the L states `prefetch` states further down the slab
-                for (int q = lane; q < 2 * L; q += 32) {
-                    const uint32_t st = base + (uint32_t)a.prefetch + (uint32_t)(q >> 1);
-                    if (st < a.S_src) prefetch_l2(Xt0 + (size_t)st * (TILE * 8) + (size_t)(q & 1) * 128);
-                }
+        const uint4* rec = bp + 2;
+        uint4 q0 = n_groups > 0 ? __ldg(rec) : make_uint4(0u, 0u, 0u, 0u);
+        for (int g = 0; g < n_groups; ++g) {
+            const uint4* rec_n = rec + (q0.x >> 24);
+            uint4 q0_n = make_uint4(0u, 0u, 0u, 0u);
+            if (g + 1 < n_groups) {
+                q0_n = __ldg(rec_n);
+                prefetch_l1((const char*)rec_n + 128);
             }
-#define COS_ROW_CASE(LL)                                                                                        \
-    case LL:                                                                                                    \
-        if (LL <= MAXL)                                                                                         \
-            row_body<(LL <= MAXL ? LL : 1), NC, SHIFT, RING, FUSED>(rw, rh, xp, ring_lane, o, nJ, e_words,     \
-                                                                    need_close, (uint32_t)a.d, gs_lane, gd_lane, \
-                                                                    Yt, close, sp);                              \
-        break;
-            switch (L) {
-                COS_ROW_CASE(1) COS_ROW_CASE(2) COS_ROW_CASE(3) COS_ROW_CASE(4) COS_ROW_CASE(5) COS_ROW_CASE(6)
-                COS_ROW_CASE(7) COS_ROW_CASE(8) COS_ROW_CASE(9) COS_ROW_CASE(10) COS_ROW_CASE(11) COS_ROW_CASE(12)
-                COS_ROW_CASE(13) COS_ROW_CASE(14) COS_ROW_CASE(15) COS_ROW_CASE(16) COS_ROW_CASE(17) COS_ROW_CASE(18)
-                COS_ROW_CASE(19) COS_ROW_CASE(20) COS_ROW_CASE(21) COS_ROW_CASE(22) COS_ROW_CASE(23) COS_ROW_CASE(24)
+#define COS_GROUP_CASE(TH_, TJ_) \
+    case ((TH_) | ((TJ_) << 3)): group_body<TH_, TJ_, FUSED>(rec, q0, c, close, sp); break;
+            switch (q0.x & 0xFFu) {
+                COS_GROUP_CASE(1, 0) COS_GROUP_CASE(1, 1) COS_GROUP_CASE(1, 2) COS_GROUP_CASE(1, 3) COS_GROUP_CASE(1, 4)
+                COS_GROUP_CASE(1, 5) COS_GROUP_CASE(1, 6) COS_GROUP_CASE(1, 7) COS_GROUP_CASE(1, 8) COS_GROUP_CASE(1, 9)
+                COS_GROUP_CASE(1, 10) COS_GROUP_CASE(1, 11) COS_GROUP_CASE(1, 12)
+                COS_GROUP_CASE(2, 0) COS_GROUP_CASE(2, 1) COS_GROUP_CASE(2, 2) COS_GROUP_CASE(2, 3) COS_GROUP_CASE(2, 4)
+                COS_GROUP_CASE(2, 5) COS_GROUP_CASE(2, 6) COS_GROUP_CASE(2, 7) COS_GROUP_CASE(2, 8) COS_GROUP_CASE(2, 9)
+                COS_GROUP_CASE(2, 10) COS_GROUP_CASE(2, 11) COS_GROUP_CASE(2, 12)
+                COS_GROUP_CASE(3, 0) COS_GROUP_CASE(3, 1) COS_GROUP_CASE(3, 2) COS_GROUP_CASE(3, 3) COS_GROUP_CASE(3, 4)
+                COS_GROUP_CASE(3, 5) COS_GROUP_CASE(3, 6) COS_GROUP_CASE(3, 7) COS_GROUP_CASE(3, 8)
+                COS_GROUP_CASE(4, 0) COS_GROUP_CASE(4, 1) COS_GROUP_CASE(4, 2) COS_GROUP_CASE(4, 3) COS_GROUP_CASE(4, 4)
+                COS_GROUP_CASE(4, 5) COS_GROUP_CASE(4, 6)
                 default: break;
             }
-#undef COS_ROW_CASE
-            rw = rw_next;
+#undef COS_GROUP_CASE
+            rec = rec_n; q0 = q0_n;
         }
         if (flags & FLAG_FRESH) {            // close-and-open: fresh head of every colour (Eq. 12, 70-71)
+            const uint4 fd = __ldg(bp + 1);
 #pragma unroll
-            for (int c = 0; c < NC; ++c) {
-                const uint32_t didx = __shfl_sync(0xFFFFFFFFu, hw, 3 + c);
-                __stcs(Yt + (size_t)didx * TILE, fma(a.neg_kappa, close, sp[c]));
+            for (int k = 0; k < 4; ++k) {
+                const uint32_t didx = k == 0 ? fd.x : k == 1 ? fd.y : k == 2 ? fd.z : fd.w;
+                if (didx != DIDX_DEAD) {
+                    double* y = (double*)(c.Yl + ((size_t)didx << 8));
+                    const double v = fma(a.neg_kappa, close, sp[k]);
+                    if (FUSED) *y = v; else __stcs(y, v);
+                }
             }
         }
         if (flags & FLAG_READOUT) {          // terminal readout O_S (Eq. 15): one block per subset S
-            const uint32_t out_idx = __shfl_sync(0xFFFFFFFFu, hw, 2);
             // 2^(|S|-1): the continuation multiplicities of Lemma 7, applied once per output (exact)
-            const double scale = (double)(1u << (__shfl_sync(0xFFFFFFFFu, hw, 1) >> 24));
-            if (valid) a.out[(size_t)out_idx * (size_t)a.batch + (size_t)b] = (a.neg_kappa * close) * scale;
+            const double scale = (double)(1u << h0.y);
+            if (valid) a.out[(size_t)h0.z * (size_t)a.batch + (size_t)b] = (a.neg_kappa * close) * scale;
         }
-        mi = mi_n; off = off_n; hw = hw_n; rw = rw_n;
+        mi = mi_n; bp = bp_n; h0 = h0_n;
     }
-    if (RING > 0 && primed) mbar_wait(bar_addr + (((t - 1u) & 1u) << 3), ((t - 1u) >> 1) & 1u);   // nothing in flight at exit
 }
 
-template <int MAXL, int NC, bool SHIFT, int RING>
-__global__ void __launch_bounds__(max_warps_of(MAXL, RING) * 32) cos_layer_kernel(const LayerArgs a)
+__global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerArgs a)
 {
     extern __shared__ __align__(128) double Gs[];
     __shared__ unsigned int s_next;
@@ -331,10 +281,6 @@ __global__ void __launch_bounds__(max_warps_of(MAXL, RING) * 32) cos_layer_kerne
 
     const uint32_t gs_lane = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)lane * 8u;
     const uint32_t gd_lane = gs_lane + (uint32_t)a.n_slots * (TILE * 8u);
-    const uint32_t n_tab = (uint32_t)a.n_slots + (SHIFT ? (uint32_t)(NC * a.d) : 0u);
-    const uint32_t ring_lane = gs_lane + (n_tab + (uint32_t)warp * (uint32_t)(RING > 0 ? RING : 0)) * (TILE * 8u);
-    __shared__ __align__(8) unsigned long long s_bar[2 * 24];
-    const uint32_t bar_addr = (uint32_t)__cvta_generic_to_shared(s_bar) + (uint32_t)warp * 16u;
 
     // Programmatic dependent launch: let the next layer's grid start (it only stages its table, which no layer
     // writes) while this grid drains; this grid in turn touches the slabs only after the previous one has completed.
@@ -343,11 +289,6 @@ __global__ void __launch_bounds__(max_warps_of(MAXL, RING) * 32) cos_layer_kerne
     const long long b = a.b0 + (long long)tile * TILE + lane;
     const bool valid = b < a.batch;
     if (threadIdx.x == 0) s_next = 0u;
-    if (RING > 0 && lane == 0) {
-        mbar_init(bar_addr, 1u);
-        mbar_init(bar_addr + 8u, 1u);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
     for (int s = warp; s < a.n_slots; s += W) {
         if (valid) cp_async8(gs_lane + (uint32_t)s * (TILE * 8u), a.G + (size_t)s * (size_t)a.batch + (size_t)b);
         else Gs[s * TILE + lane] = 0.0;
@@ -355,25 +296,22 @@ __global__ void __launch_bounds__(max_warps_of(MAXL, RING) * 32) cos_layer_kerne
     cp_async_commit();
     cp_async_wait<0>();
     __syncthreads();
-    if (SHIFT) {
-        // continuation into the partner of the current endpoint (E2 with j = e) always comes with the
-        // counterterm one-cycle E3 at the same destination: fold c3*sigma_lam into the diagonal of the
-        // staged table (Eq. 49 / 72, 77) and keep the plain diagonal for the cycle-closing factor.
-        for (int q = warp; q < NC * a.d; q += W) {
-            const int lam = q / a.d, e = q - lam * a.d;
-            const double sh = lam == 0 ? a.shift[0] : lam == 1 ? a.shift[1] : lam == 2 ? a.shift[2] : a.shift[3];
-            const double g = Gs[((lam * a.d + e) * a.d + e) * TILE + lane];
-            Gs[(a.n_slots + q) * TILE + lane] = g;
-            Gs[((lam * a.d + e) * a.d + e) * TILE + lane] = g + sh;
-        }
-        __syncthreads();
+    // continuation into the partner of the current endpoint (E2 with j = e) always comes with the counterterm one-cycle
+    // E3 at the same destination: fold c3*sigma_lam into the diagonal of the staged table (Eq. 49 / 72, 77) and keep
+    // the plain diagonal Gd for the cycle-closing factor (no shifts: Gd is a copy of the diagonal).
+    for (int q = warp; q < a.nc * a.d; q += W) {
+        const int lam = q / a.d, e = q - lam * a.d;
+        const double sh = lam == 0 ? a.shift[0] : lam == 1 ? a.shift[1] : lam == 2 ? a.shift[2] : a.shift[3];
+        const double g = Gs[((lam * a.d + e) * a.d + e) * TILE + lane];
+        Gs[(a.n_slots + q) * TILE + lane] = g;
+        if (a.has_shift) Gs[((lam * a.d + e) * a.d + e) * TILE + lane] = g + sh;
     }
+    __syncthreads();
 
     if (a.pdl) asm volatile("griddepcontrol.wait;" ::: "memory");
     const uint32_t m_begin = blockIdx.y * a.masks_per_cta;
     const uint32_t m_end = min(a.n_masks, m_begin + a.masks_per_cta);
-    layer_blocks<MAXL, NC, SHIFT, RING, false>(a, m_begin, m_end, tile, s_next, gs_lane, gd_lane, ring_lane, bar_addr, lane,
-                                               valid, b);
+    layer_blocks<false>(a, m_begin, m_end, tile, s_next, gs_lane, gd_lane, lane, valid, b);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -382,7 +320,6 @@ __global__ void __launch_bounds__(max_warps_of(MAXL, RING) * 32) cos_layer_kerne
 // once, writes the layer-0 states (Eq. 66) itself and ping-pongs between two slabs of S_max states per tile (L2-resident;
 // source rows are read with ld.global.cg so that no stale L1 line of the slab written two layers earlier is seen).
 // Used when every layer is small (launch latency, not bandwidth, decides: orders n <= 6).
-template <int MAXL, int NC, bool SHIFT>
 __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedArgs f)
 {
     extern __shared__ __align__(128) double Gs[];
@@ -404,19 +341,19 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
     for (uint32_t s = warp; s < f.layers[0].n_states; s += W) slab0[(size_t)s * TILE + lane] = 1.0;   // Eq. 66
     cp_async_wait<0>();
     __syncthreads();
-    if (SHIFT) {       // keep the plain diagonal (cycle closing); the shifted one is rewritten per layer below
-        for (int q = warp; q < NC * f.d; q += W) {
-            const int lam = q / f.d, e = q - lam * f.d;
-            Gs[(f.n_slots + q) * TILE + lane] = Gs[((lam * f.d + e) * f.d + e) * TILE + lane];
-        }
-        __syncthreads();
+    // keep the plain diagonal (cycle closing); the shifted one is rewritten per layer below
+    for (int q = warp; q < f.nc * f.d; q += W) {
+        const int lam = q / f.d, e = q - lam * f.d;
+        Gs[(f.n_slots + q) * TILE + lane] = Gs[((lam * f.d + e) * f.d + e) * TILE + lane];
     }
+    __syncthreads();
     LayerArgs a;
-    a.G = f.G; a.batch = f.batch; a.b0 = f.b0; a.out = f.out; a.d = f.d; a.n_slots = f.n_slots;
+    a.G = f.G; a.batch = f.batch; a.b0 = f.b0; a.out = f.out; a.d = f.d; a.nc = f.nc; a.n_slots = f.n_slots;
+    a.has_shift = f.has_shift;
     a.neg_kappa = f.neg_kappa; a.prefetch = 0; a.pdl = 0; a.S_src = f.S_max; a.S_dst = f.S_max; a.masks_per_cta = 0;
     for (int l = 0; l < f.n_layers; ++l) {
-        if (SHIFT && l <= 1) {               // c3 = -2 at layer 0, -1 afterwards (Eq. 72, 77)
-            for (int q = warp; q < NC * f.d; q += W) {
+        if (f.has_shift && l <= 1) {         // c3 = -2 at layer 0, -1 afterwards (Eq. 72, 77)
+            for (int q = warp; q < f.nc * f.d; q += W) {
                 const int lam = q / f.d, e = q - lam * f.d;
                 const double sg = lam == 0 ? f.sigma[0] : lam == 1 ? f.sigma[1] : lam == 2 ? f.sigma[2] : f.sigma[3];
                 Gs[((lam * f.d + e) * f.d + e) * TILE + lane] = Gs[(f.n_slots + q) * TILE + lane] + (l == 0 ? -2.0 : -1.0) * sg;
@@ -427,7 +364,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
         a.words = fl.words; a.mask_off = fl.mask_off; a.n_masks = fl.n_masks;
         a.X = (l & 1) ? slab1 : slab0; a.Y = (l & 1) ? slab0 : slab1;
         // slabs are addressed per tile already: tile index 0 inside layer_blocks
-        layer_blocks<MAXL, NC, SHIFT, 0, true>(a, 0u, fl.n_masks, 0u, s_next, gs_lane, gd_lane, 0u, 0u, lane, valid, b);
+        layer_blocks<true>(a, 0u, fl.n_masks, 0u, s_next, gs_lane, gd_lane, lane, valid, b);
         __threadfence_block();
         __syncthreads();
         if (threadIdx.x == 0) s_next = 0u;
@@ -436,111 +373,57 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
 }
 
 // ------------------------------------------------------------------------------------------------------
-typedef void (*layer_fn)(const LayerArgs);
-
-template <int MAXL, int RING>
-static layer_fn pick_nc(int nc, bool shift)
+size_t layer_smem_bytes(int n_slots, int nc, int d)
 {
-    if (!shift) {
-        switch (nc) {
-            case 1: return cos_layer_kernel<MAXL, 1, false, RING>;
-            case 2: return cos_layer_kernel<MAXL, 2, false, RING>;
-            case 3: return cos_layer_kernel<MAXL, 3, false, RING>;
-            default: return cos_layer_kernel<MAXL, 4, false, RING>;
-        }
-    }
-    switch (nc) {
-        case 1: return cos_layer_kernel<MAXL, 1, true, RING>;
-        case 2: return cos_layer_kernel<MAXL, 2, true, RING>;
-        case 3: return cos_layer_kernel<MAXL, 3, true, RING>;
-        default: return cos_layer_kernel<MAXL, 4, true, RING>;
-    }
-}
-
-// ring = 0: source rows loaded straight into registers; ring = LAYER_RING: streamed through shared memory
-// (needs LAYER_RING >= 2 * MAXL, so only the max_L <= 12 instantiations have it).
-static layer_fn pick_layer_fn(int max_L, int nc, bool shift, int ring)
-{
-    if (ring > 0) {
-        if (max_L <= 4) return pick_nc<4, LAYER_RING>(nc, shift);
-        if (max_L <= 8) return pick_nc<8, LAYER_RING>(nc, shift);
-        if (max_L <= 12) return pick_nc<12, LAYER_RING>(nc, shift);
-        return nullptr;
-    }
-    if (max_L <= 4) return pick_nc<4, 0>(nc, shift);
-    if (max_L <= 8) return pick_nc<8, 0>(nc, shift);
-    if (max_L <= 12) return pick_nc<12, 0>(nc, shift);
-    if (max_L <= 20) return pick_nc<20, 0>(nc, shift);
-    return pick_nc<24, 0>(nc, shift);
-}
-
-size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift, int ring, int warps_per_cta)
-{
-    return (size_t)(n_slots + (shift ? nc * d : 0) + (ring > 0 ? ring * warps_per_cta : 0)) * TILE * sizeof(double);
+    return (size_t)(n_slots + nc * d) * TILE * sizeof(double);
 }
 
 cudaError_t configure_layer_kernels()
 {
-    static const int Ls[5] = {4, 8, 12, 20, 24};
-    for (int i = 0; i < 5; ++i)
-        for (int nc = 1; nc <= 4; ++nc)
-            for (int sh = 0; sh < 2; ++sh)
-                for (int ring = 0; ring <= LAYER_RING; ring += LAYER_RING) {
-                    layer_fn fn = pick_layer_fn(Ls[i], nc, sh != 0, ring);
-                    if (!fn) continue;
-                    cudaError_t e = cudaFuncSetAttribute((const void*)fn, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                                         (int)LAYER_SMEM_MAX);
-                    if (e != cudaSuccess) return e;
-                }
+    cudaError_t e = cudaFuncSetAttribute((const void*)cos_layer_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)LAYER_SMEM_MAX);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute((const void*)cos_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                (int)LAYER_SMEM_MAX);
+}
+
+// Launch shape: the CTA size that maximises resident warps per SM (ties: the smaller CTA).
+cudaError_t pick_layer_shape(int nc, int d, int n_slots, int* warps_per_cta, int* ctas_per_sm)
+{
+    static const int cand[6] = {4, 6, 8, 10, 12, 16};
+    const size_t smem = layer_smem_bytes(n_slots, nc, d);
+    if (smem > LAYER_SMEM_MAX) return cudaErrorInvalidConfiguration;
+    int best_w = 0, best_total = 0, best_ctas = 0;
+    for (int i = 0; i < 6; ++i) {
+        if (cand[i] > MAX_WARPS) continue;
+        int nb = 0;
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)cos_layer_kernel, cand[i] * 32, smem);
+        if (e != cudaSuccess) return e;
+        if (nb * cand[i] > best_total) { best_total = nb * cand[i]; best_w = cand[i]; best_ctas = nb; }
+    }
+    if (best_w == 0) return cudaErrorInvalidConfiguration;
+    *warps_per_cta = best_w; *ctas_per_sm = best_ctas;
     return cudaSuccess;
 }
 
-// Launch shape for this instantiation: ring or not, warps per CTA.
-//   ring path  (max_L <= 12 and the table leaves room for >= 8 rings): the CTA size with the most resident warps
-//              per SM counting each warp's ring; look-ahead, not occupancy, hides the HBM latency there.
-//   direct path: the CTA size that maximises resident warps per SM (ties: the smaller CTA).
-cudaError_t pick_layer_shape(int max_L, int nc, int d, int n_slots, bool shift, int want_ring, int* ring,
-                             int* warps_per_cta, int* ctas_per_sm)
+cudaError_t layer_ctas_per_sm(int nc, int d, int n_slots, int warps_per_cta, int* ctas_per_sm)
 {
-    static const int cand[8] = {4, 6, 8, 10, 12, 16, 20, 24};
-    for (int pass = 0; pass < 2; ++pass) {
-        const int rg = (pass == 0) ? LAYER_RING : 0;
-        const int max_w = max_warps_of(max_L <= 4 ? 4 : max_L <= 8 ? 8 : max_L <= 12 ? 12 : max_L <= 20 ? 20 : 24, rg);
-        if (pass == 0 && (want_ring == 0 || max_L > 12)) continue;
-        layer_fn fn = pick_layer_fn(max_L, nc, shift, rg);
-        if (!fn) continue;
-        int best_w = 0, best_total = 0, best_ctas = 0;
-        for (int i = 0; i < 8; ++i) {
-            const size_t smem = layer_smem_bytes(n_slots, nc, d, shift, rg, cand[i]);
-            if (smem > LAYER_SMEM_MAX || cand[i] > max_w) continue;
-            int nb = 0;
-            cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)fn, cand[i] * 32, smem);
-            if (e != cudaSuccess) return e;
-            if (nb * cand[i] > best_total) { best_total = nb * cand[i]; best_w = cand[i]; best_ctas = nb; }
-        }
-        if (best_w == 0 || (pass == 0 && best_total < 8)) continue;
-        *ring = rg; *warps_per_cta = best_w; *ctas_per_sm = best_ctas;
-        return cudaSuccess;
-    }
-    return cudaErrorInvalidConfiguration;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, (const void*)cos_layer_kernel, warps_per_cta * 32,
+                                                         layer_smem_bytes(n_slots, nc, d));
 }
 
-cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, int ring, uint32_t tiles,
-                         int warps_per_cta, cudaStream_t stream)
+cudaError_t launch_layer(const LayerArgs& a, uint32_t tiles, int warps_per_cta, cudaStream_t stream)
 {
     if (a.n_masks == 0 || tiles == 0) return cudaSuccess;
     if (warps_per_cta < 1) warps_per_cta = 1;
-    const int max_w = max_warps_of(max_L <= 4 ? 4 : max_L <= 8 ? 8 : max_L <= 12 ? 12 : max_L <= 20 ? 20 : 24, ring);
-    if (warps_per_cta > max_w) warps_per_cta = max_w;
+    if (warps_per_cta > MAX_WARPS) warps_per_cta = MAX_WARPS;
     const uint32_t chunks = (a.n_masks + a.masks_per_cta - 1) / a.masks_per_cta;
     if (chunks > 65535u) return cudaErrorInvalidConfiguration;
     dim3 grid(tiles, chunks, 1), block(32 * warps_per_cta, 1, 1);
-    layer_fn fn = pick_layer_fn(max_L, nc, shift, ring);
-    if (!fn) return cudaErrorInvalidConfiguration;
-    const size_t smem = layer_smem_bytes(a.n_slots, nc, a.d, shift, ring, warps_per_cta);
+    const size_t smem = layer_smem_bytes(a.n_slots, a.nc, a.d);
     if (smem > LAYER_SMEM_MAX) return cudaErrorInvalidConfiguration;
     if (!a.pdl) {
-        fn<<<grid, block, smem, stream>>>(a);
+        cos_layer_kernel<<<grid, block, smem, stream>>>(a);
         return cudaGetLastError();
     }
     cudaLaunchConfig_t cfg = {};
@@ -549,58 +432,16 @@ cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, int 
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, fn, a);
+    return cudaLaunchKernelEx(&cfg, cos_layer_kernel, a);
 }
 
-typedef void (*fused_fn)(const FusedArgs);
-template <int MAXL>
-static fused_fn pick_fused_nc(int nc, bool shift)
-{
-    if (!shift) {
-        switch (nc) {
-            case 1: return cos_fused_kernel<MAXL, 1, false>;
-            case 2: return cos_fused_kernel<MAXL, 2, false>;
-            case 3: return cos_fused_kernel<MAXL, 3, false>;
-            default: return cos_fused_kernel<MAXL, 4, false>;
-        }
-    }
-    switch (nc) {
-        case 1: return cos_fused_kernel<MAXL, 1, true>;
-        case 2: return cos_fused_kernel<MAXL, 2, true>;
-        case 3: return cos_fused_kernel<MAXL, 3, true>;
-        default: return cos_fused_kernel<MAXL, 4, true>;
-    }
-}
-static fused_fn pick_fused_fn(int max_L, int nc, bool shift)
-{
-    if (max_L <= 4) return pick_fused_nc<4>(nc, shift);
-    if (max_L <= 8) return pick_fused_nc<8>(nc, shift);
-    if (max_L <= 12) return pick_fused_nc<12>(nc, shift);
-    return nullptr;
-}
-
-cudaError_t configure_fused_kernels()
-{
-    static const int Ls[3] = {4, 8, 12};
-    for (int i = 0; i < 3; ++i)
-        for (int nc = 1; nc <= 4; ++nc)
-            for (int sh = 0; sh < 2; ++sh) {
-                cudaError_t e = cudaFuncSetAttribute((const void*)pick_fused_fn(Ls[i], nc, sh != 0),
-                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LAYER_SMEM_MAX);
-                if (e != cudaSuccess) return e;
-            }
-    return cudaSuccess;
-}
-
-cudaError_t launch_fused(const FusedArgs& f, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
-                         cudaStream_t stream)
+cudaError_t launch_fused(const FusedArgs& f, uint32_t tiles, int warps_per_cta, cudaStream_t stream)
 {
     if (tiles == 0) return cudaSuccess;
-    fused_fn fn = pick_fused_fn(max_L, nc, shift);
-    if (!fn) return cudaErrorInvalidConfiguration;
     if (warps_per_cta > MAX_WARPS) warps_per_cta = MAX_WARPS;
-    const size_t smem = layer_smem_bytes(f.n_slots, nc, f.d, shift, 0, 0);
-    fn<<<tiles, 32 * warps_per_cta, smem, stream>>>(f);
+    const size_t smem = layer_smem_bytes(f.n_slots, f.nc, f.d);
+    if (smem > LAYER_SMEM_MAX) return cudaErrorInvalidConfiguration;
+    cos_fused_kernel<<<tiles, 32 * warps_per_cta, smem, stream>>>(f);
     return cudaGetLastError();
 }
 

@@ -6,7 +6,6 @@
 namespace cosb {
 
 static const int TILE = 32;              // configurations per batch tile = one warp, lane = configuration
-static const int LAYER_RING = 16;        // states per warp of the shared-memory source ring (>= 12, power of two)
 static const size_t LAYER_SMEM_MAX = 227 * 1024 - 1024;   // minus the static counter and the 128-byte alignment of the table
 
 struct LayerArgs {
@@ -19,23 +18,23 @@ struct LayerArgs {
     const double* G;                     // caller's propagators [n_slots][batch]
     long long batch, b0;                 // total batch (row stride of G / out) and first configuration of this chunk
     double* out;                         // caller's output [n_out][batch]
-    int d, n_slots;                      // n_slots = n_blocks * d * d
+    int d, nc, n_slots;                  // table dimension, colours carried in the state, n_slots = n_blocks * d * d
+    int has_shift;                       // SB mode: the counterterm is folded into the staged diagonal
     double neg_kappa;                    // -kappa: -N_f (uniform) or -1 (SB)
-    int prefetch;                        // > 0: per row, prefetch into L2 the source states this many states ahead;
-                                         // < 0: prefetch the next block's states; 0: off
+    int prefetch;                        // > 0: per group record, prefetch into L2 the source states this many states
+                                         // further down the slab; 0: off
     int pdl;                             // 1: launched with programmatic stream serialization (layers > 0)
     double shift[4];                     // c3 * sigma_lambda of THIS layer (c3 = -2 at layer 0, -1 after)
 };
 
-// Picks the instantiation (max row length, colours, shift) and launches one layer step.
-// grid = (tiles, ceil(n_masks / masks_per_cta)); returns cudaGetLastError().
-cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, int ring, uint32_t tiles,
-                         int warps_per_cta, cudaStream_t stream);
-// Opt-in to > 48 KB dynamic shared memory for every instantiation (once per process).
+// Launches one layer step: grid = (tiles, ceil(n_masks / masks_per_cta)); returns cudaGetLastError().
+cudaError_t launch_layer(const LayerArgs& a, uint32_t tiles, int warps_per_cta, cudaStream_t stream);
+// Opt-in to > 48 KB dynamic shared memory (once per process): the per-layer and the fused kernel.
 cudaError_t configure_layer_kernels();
-size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift, int ring, int warps_per_cta);
-cudaError_t pick_layer_shape(int max_L, int nc, int d, int n_slots, bool shift, int want_ring, int* ring,
-                             int* warps_per_cta, int* ctas_per_sm);
+// staged table + plain diagonal of one batch tile
+size_t layer_smem_bytes(int n_slots, int nc, int d);
+cudaError_t pick_layer_shape(int nc, int d, int n_slots, int* warps_per_cta, int* ctas_per_sm);
+cudaError_t layer_ctas_per_sm(int nc, int d, int n_slots, int warps_per_cta, int* ctas_per_sm);
 
 // ---- fused small-DAG path: every layer in one launch (cos_fused_kernel)
 struct FusedLayer { const uint32_t* words; const uint32_t* mask_off; uint32_t n_masks, n_states; };
@@ -45,13 +44,11 @@ struct FusedArgs {
     double* ws;                          // two slabs [2][tiles][S_max][32]
     uint32_t S_max;
     const double* G; long long batch, b0; double* out;
-    int d, n_slots;
+    int d, nc, n_slots, has_shift;
     double neg_kappa;
     double sigma[4];
 };
-cudaError_t configure_fused_kernels();
-cudaError_t launch_fused(const FusedArgs& f, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
-                         cudaStream_t stream);
+cudaError_t launch_fused(const FusedArgs& f, uint32_t tiles, int warps_per_cta, cudaStream_t stream);
 
 cudaError_t launch_fill_ones(double* X, size_t n_doubles, cudaStream_t stream);
 

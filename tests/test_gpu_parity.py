@@ -32,14 +32,16 @@ def cos():
     return cos_mod
 
 
-def gpu_eval(cos, G, n, n_flavors, lattice, sigmas, all_subsets, ws_limit=None):
+def gpu_eval(cos, G, n, n_flavors, lattice, sigmas, all_subsets, ws_limit=None, flags=0, tune=None):
     """G: numpy [n_blocks][d][d][B] -> numpy [n_out][B] through cos_build / cos_eval / cos_free."""
     import torch
     B = G.shape[-1]
-    h = cos.cos_build(n, n_flavors, lattice, sigmas, n if all_subsets else 0)
+    h = cos.cos_build_ex(n, n_flavors, lattice, sigmas, n if all_subsets else 0, flags)
     try:
         if ws_limit is not None:
             cos.cos_set_workspace_limit(h, ws_limit)
+        for k, v in (tune or {}).items():
+            cos.cos_set_tuning(h, k, v)
         n_out = cos.cos_info(h, "n_out")
         Gd = torch.from_numpy(np.ascontiguousarray(G.reshape(-1, B))).cuda()
         out = torch.full((n_out, B), float("nan"), dtype=torch.float64, device="cuda")
@@ -386,41 +388,37 @@ def test_config3_full_sampled(cos):
 
 @pytest.mark.parametrize("n,nf,lattice,sb,all_subsets", [(4, 2, 0, False, False), (5, 3, 0, True, True),
                                                           (3, 2, 1, True, True), (6, 3, 0, True, False)])
-def test_fused_and_layered_paths_agree(cos, n, nf, lattice, sb, all_subsets, monkeypatch):
-    """Small DAGs run in ONE launch (cos_fused_kernel); COS_FUSED=0 forces the per-layer kernels.  Both walk the same
-    program with the same arithmetic order, so the outputs must be bit-identical (and equal the oracle, tested above)."""
+def test_fused_and_layered_paths_agree(cos, n, nf, lattice, sb, all_subsets):
+    """Small DAGs run in ONE launch (cos_fused_kernel); COS_BUILD_NO_FUSED / cos_set_tuning("fused", 0) force the
+    per-layer kernels.  Both walk the same program with the same arithmetic order, so the outputs must be bit-identical
+    (and equal the oracle, tested above).  The launch tuning knobs must not change a bit either."""
     n_sub = 2 if lattice else 1
     sig = [0.3, -0.2, 0.1][:nf] if sb else None
     G = random_matrices(50 + n, nf if sb else 1, n * n_sub, 77, scale=0.5)
-    monkeypatch.setenv("COS_FUSED", "1")
     a = gpu_eval(cos, G, n, nf, lattice, sig, all_subsets)
     a_chunked = gpu_eval(cos, G, n, nf, lattice, sig, all_subsets, ws_limit=1)      # one tile per chunk
-    monkeypatch.setenv("COS_FUSED", "0")
-    b = gpu_eval(cos, G, n, nf, lattice, sig, all_subsets)
+    b = gpu_eval(cos, G, n, nf, lattice, sig, all_subsets, flags=cos.COS_BUILD_NO_FUSED)
+    b2 = gpu_eval(cos, G, n, nf, lattice, sig, all_subsets, tune={"fused": 0, "pdl": 0, "prefetch": 0, "warps_per_cta": 4,
+                                                                   "blocks_per_cta_cap": 3, "tiles_per_chunk": 2})
     assert np.all(np.isfinite(a))
-    assert np.array_equal(a, b) and np.array_equal(a, a_chunked)
+    assert np.array_equal(a, b) and np.array_equal(a, a_chunked) and np.array_equal(a, b2)
 
 
-@pytest.mark.parametrize("n,nf,sb,all_subsets", [(8, 2, False, True), (7, 3, True, False)])
-def test_tma_ring_path_agrees(cos, n, nf, sb, all_subsets, monkeypatch):
-    """COS_RING=1 streams the source rows through a per-warp shared-memory ring with TMA bulk copies + mbarriers
-    (measured slower, off by default).  Same program, same arithmetic order: bit-identical to the default path."""
-    sig = [0.3, -0.2, 0.1][:nf] if sb else None
-    G = random_matrices(70 + n, nf if sb else 1, n, 101, scale=0.5, diag=-0.4)
-    monkeypatch.setenv("COS_RING", "0")
-    a = gpu_eval(cos, G, n, nf, 0, sig, all_subsets)
-    monkeypatch.setenv("COS_RING", "1")
-    b = gpu_eval(cos, G, n, nf, 0, sig, all_subsets)
-    assert np.all(np.isfinite(a)) and np.array_equal(a, b)
-    for c in (0, 100):
-        A = np.ascontiguousarray(G[..., c])
-        if sb:
-            ref = oracle.o2b_polynomial(A, sig)[-1:]
-            M = np.array([M_lower_bound(A, n, 1, nf, False)])
-        else:
-            ref = oracle.o2a_twospin(A[0], A[0])
-            M = oracle.o3_uniform(A[0], 2, 0.0, True, absolute=True)
-        check(a[:, c], ref, M, ("ring", n, c))
+def test_fused_flag_is_reported(cos):
+    h = cos.cos_build(4, 2, cos.COS_LATTICE_SQUARE, None, 0)
+    h2 = cos.cos_build_ex(4, 2, cos.COS_LATTICE_SQUARE, None, 0, cos.COS_BUILD_NO_FUSED)
+    h3 = cos.cos_build(8, 2, cos.COS_LATTICE_SQUARE, None, 0)       # too large for the fused kernel
+    try:
+        assert cos.cos_info(h, "fused") == 1 and cos.cos_info(h2, "fused") == 0 and cos.cos_info(h3, "fused") == 0
+        cos.cos_set_tuning(h3, "fused", 1)                           # ignored: the DAG does not qualify
+        assert cos.cos_info(h3, "fused") == 0
+        with pytest.raises(cos.CosError) as ei:
+            cos.cos_set_tuning(h, "warps_per_cta", 17)
+        assert ei.value.code == cos.COS_EINVAL
+        with pytest.raises(cos.CosError):
+            cos.cos_set_tuning(h, 99, 1)
+    finally:
+        cos.cos_free(h); cos.cos_free(h2); cos.cos_free(h3)
 
 
 def test_four_flavours_per_layer_kernels(cos):
