@@ -48,6 +48,8 @@ def parse_args():
     ap.add_argument("--batch", type=int, default=0, help="override the configuration count (0 = BASELINE's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--layers", action="store_true", help="print the per-layer table to stderr")
+    ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
+                    help="launch tuning through cos_set_tuning (prefetch, warps_per_cta, blocks_per_cta_cap, pdl, ...)")
     ap.add_argument("--route", default="dag", choices=["dag", "det"],
                     help="dag: the hot path (default, the driver's contract); det: the determinant-polynomial route "
                          "cos_det_eval (SURVEY 8(f).3) on the same workload, all 2^n-1 subsets, its own JSON line")
@@ -237,6 +239,9 @@ def run_ours(args):
     t0 = time.perf_counter()
     h = cos.cos_build(w.n, w.n_flavors, w.lattice, w.sigmas, w.n if w.all_subsets else 0)
     build_s = time.perf_counter() - t0
+    for kv in args.tune:
+        k, val = kv.split("=")
+        cos.cos_set_tuning(h, k, int(val))
     info = cos.dag_summary(h)
     NL = info["n_layers"]
     n_slots = info["n_blocks"] * info["d"] ** 2

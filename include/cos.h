@@ -109,7 +109,7 @@ int cos_set_workspace_limit(cos_handle h, long long bytes);
 /* Launch tuning of a handle.  These are the ONLY knobs; the library reads no environment variable.  Results do not
  * depend on them (same arithmetic, same summation order).  Bad parameter or value: COS_EINVAL. */
 enum {
-    COS_TUNE_PREFETCH = 0,           /* L2 look-ahead of the layer kernel, in states (0 = off; default 32) */
+    COS_TUNE_PREFETCH = 0,           /* L2 look-ahead of the layer kernel, in states (0 = off; default 256) */
     COS_TUNE_WARPS_PER_CTA = 1,      /* 1..16; default: the CTA size with the most resident warps per SM */
     COS_TUNE_BLOCKS_PER_CTA_CAP = 2, /* upper bound of occupancy-mask blocks per CTA (0 = default: one per staged table slot) */
     COS_TUNE_PDL = 3,                /* programmatic dependent launch between layers (default 1) */

@@ -41,7 +41,7 @@ struct cos_handle_s {
     long long ws_limit = 64ll << 30;
     // launch shape and tuning (cos_set_tuning); nothing here is read from the environment
     int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148;
-    int prefetch = 32;                    // L2 look-ahead distance in states
+    int prefetch = 256;                   // L2 look-ahead distance in states
     int blocks_per_cta_cap = 0;           // 0: one block per staged table slot (64 .. 1024)
     int pdl = 1;                          // programmatic dependent launch between layers
     int host_slices = 8;                  // cos_eval_host: at most this many output slices (1: no second stream)

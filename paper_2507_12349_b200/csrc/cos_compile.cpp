@@ -194,7 +194,26 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                 for (int h = 0; h < d; ++h) any = any || b.alive[(size_t)id * d + h];
                 if (any) keep.push_back(id);
             }
-            std::sort(keep.begin(), keep.end(), [&](uint32_t x, uint32_t y) { return b.codes[x] < b.codes[y]; });
+            // Blocks of equal shape (live destination endpoints, heads) are neighbours in the slab and in the program: the
+            // warps of an SM then run the same instance of the kernel's source loop at the same time (instruction cache).
+            std::vector<uint32_t> shape(b.codes.size(), 0u);
+            for (uint32_t id : keep) {
+                const uint32_t code = b.codes[id];
+                const int nJ = (l + 1 < NL) ? b.jlist(code, J) : 0;
+                uint32_t n_heads = 0, n_cols = 0;
+                for (int h = 0; h < d; ++h) n_heads += b.alive[(size_t)id * d + h] != 0u;
+                for (int q = 0; q < nJ; ++q) {
+                    const int32_t did = b.index_of[J[q].dest_code];
+                    bool any = false;
+                    for (int h = 0; h < d && !any && did >= 0; ++h)
+                        any = b.alive[(size_t)id * d + h] && ((b.alive[(size_t)did * d + h] >> J[q].j_a) & 1u);
+                    n_cols += any;
+                }
+                shape[id] = (n_cols << 8) | n_heads;
+            }
+            std::sort(keep.begin(), keep.end(), [&](uint32_t x, uint32_t y) {
+                return shape[x] != shape[y] ? shape[x] < shape[y] : b.codes[x] < b.codes[y];
+            });
             ids.swap(keep);
             uint64_t counter = 0;
             for (uint32_t id : ids) {
@@ -208,7 +227,7 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                 b.colour_stride[id] = per_colour;
                 counter += (uint64_t)per_colour * nc;
             }
-            if (counter >= DIDX_DEFER) return "unsupported: a layer has more than 2^32 - 2 states (32-bit destination index)";
+            if (counter >= DIDX_DEAD) return "unsupported: a layer has more than 2^32 - 2 states (32-bit destination index)";
             out.layers[l].n_states = (uint32_t)counter;
             out.layers[l].n_masks = (uint32_t)ids.size();
         }
@@ -269,10 +288,10 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                 for (int lam = 0; lam < 4; ++lam)
                     P.words.push_back((lam < nc && (flags & FLAG_FRESH))
                                           ? b.state_index((uint32_t)fresh_did, (int)fresh_a, lam, (int)fresh_a) : DIDX_DEAD);
-                uint32_t n_groups = 0;
+                uint32_t n_groups = 0, merged = 0;
                 for (int ch = 0; ch < n_chunks; ++ch) {
                     const int c0 = n_cols * ch / n_chunks, c1 = n_cols * (ch + 1) / n_chunks, TJ = c1 - c0;
-                    const int th_max = std::max(1, std::min(GROUP_MAX_HEADS, TJ ? GROUP_MAX_ACC / TJ : GROUP_MAX_HEADS));
+                    const int th_max = TJ <= TILE_A_COLS ? TILE_A_HEADS : TILE_B_HEADS;
                     const int n_hgroups = (n_heads + th_max - 1) / th_max;
                     for (int lam = 0; lam < nc; ++lam)
                         for (int g = 0; g < n_hgroups; ++g) {
@@ -280,7 +299,8 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                             uint32_t emask = 0, jmask = 0;
                             for (int k = h0; k < h1; ++k) emask |= b.alive[(size_t)id * d + heads[k]];
                             for (int c = c0; c < c1; ++c) jmask |= 1u << J[cols[c]].j_a;
-                            const uint32_t len = 4u + 4u * (uint32_t)TH + (((uint32_t)(TH * TJ) + 3u) & ~3u);
+                            const uint32_t row_words = ((uint32_t)TJ + 1u) & ~1u;      // destination rows are 8-byte aligned
+                            const uint32_t len = 4u + 4u * (uint32_t)TH + (((uint32_t)TH * row_words + 3u) & ~3u);
                             if (P.words.size() + len >= 0xFFFFFFF0ull) return "unsupported: layer program exceeds 2^32 words";
                             P.words.push_back((uint32_t)TH | ((uint32_t)TJ << 3) | ((uint32_t)lam << 8) |
                                               ((need_close && ch == 0) ? 1u << 10 : 0u) | ((len / 4u) << 24));
@@ -306,11 +326,14 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                                         P.n_factor_loads_unshared += L;
                                         // the continuation into the canonical open interaction from its own head lands on the
                                         // fresh-head state (coalesced E2/E4 pair)
-                                        if ((flags & FLAG_FRESH) && (uint32_t)h == fresh_a && J[q].j_a == fresh_a) w = DIDX_DEFER;
-                                        else w = b.state_index((uint32_t)dest[q], h, lam, J[q].j_a);
+                                        // (same destination state as the block's fresh-head state of this colour; the
+                                        // kernel adds the closing sum to it at the end of the block, header w3 bit lam)
+                                        if ((flags & FLAG_FRESH) && (uint32_t)h == fresh_a && J[q].j_a == fresh_a) merged |= 1u << lam;
+                                        w = b.state_index((uint32_t)dest[q], h, lam, J[q].j_a);
                                     }
                                     P.words.push_back(w);
                                 }
+                                if (TJ & 1) P.words.push_back(DIDX_DEAD);
                             }
                             while (P.words.size() & 3u) P.words.push_back(DIDX_DEAD);
                             P.n_fma += (uint64_t)TH * U * (uint64_t)TJ;
@@ -333,6 +356,7 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                 }
                 if (n_groups > 0xFFFFu) return "unsupported: more than 65535 group records in one block";
                 P.words[w_block] |= n_groups;
+                P.words[w_block + 3] = merged;
                 P.n_groups += n_groups;
                 P.n_rows += (uint32_t)n_heads * nc;
                 P.max_L = std::max(P.max_L, Lmax);

@@ -21,7 +21,9 @@ namespace cosb {
 //                                                  bit1 READOUT (terminal readout, Eq. 14-15)
 //   w1 : (|S| - 1) of a readout block (the deferred multiplicity 2^(|S|-1), see below)
 //   w2 : out_idx (readout row of out_dev)
-//   w3 : 0
+//   w3 : bit lambda: a row of the block stores its continuation into the fresh-head state of colour lambda (the
+//        coalesced E2/E4 pair: continuation from the canonical open interaction's own head); the kernel
+//        then ADDS the closing sum to that state at the end of the block instead of overwriting it
 //   w4..w7 : destination state index (next layer) of the fresh-head state of colour lambda' (DIDX_DEAD: pruned / unused)
 // group record: up to GROUP_MAX_HEADS rows (heads) of ONE colour of the block that share the factor loads -- the
 // factor-application sharing of PAPER.md Eq. 29-31: G_lambda[e][j] does not depend on the head, so one staged factor
@@ -32,20 +34,22 @@ namespace cosb {
 //        jmask = destination endpoints j_a of the TJ columns of this record (bit j_a), in increasing order
 //        first = slab index of the group's first state (its states are contiguous: heads in increasing order)
 //   TH x qh : base | alive | h_a | 0     base = slab index of the head's first state, alive = its live endpoints (bit e_a)
-//   TH x TJ destination words (row-major, padded to a multiple of 4): index of the destination state in the next layer's
-//        slab, DIDX_DEAD (pruned, Eq. 23) or DIDX_DEFER (the value merges with the fresh-head state: coalesced E2/E4 pair).
-//   Blocks with more than GROUP_MAX_COLS live destination endpoints are split into column chunks (one set of records per
-//   chunk; do_close is set in the first chunk only, so that the cycle-closing sum is taken once).
+//   TH rows of TJ destination words, each row padded to an even number of words (and the record to a multiple of 4):
+//        index of the destination state in the next layer's slab, or DIDX_DEAD (pruned, Eq. 23, or padding).
+//   Register tiles of the kernel: up to TILE_A_HEADS heads when the block has at most TILE_A_COLS live destination
+//   endpoints, else up to TILE_B_HEADS heads x GROUP_MAX_COLS endpoints.  Blocks with more than GROUP_MAX_COLS live
+//   destination endpoints are split into column chunks (one set of records per chunk; do_close is set in the first
+//   chunk only, so that the cycle-closing sum is taken once).
 // The multiplicity 2 - m_j = 2 of a continuation into an untouched interaction (Lemma 7) is NOT applied per edge:
 // every path into a state of mask m has taken exactly nz(m) - 1 such edges (nz = interactions with m_i >= 1; the root
 // enters with factor 1), so the slabs hold x / 2^(nz(m)-1) and a readout of subset S is scaled by 2^(|S|-1), exactly.
 static const uint32_t DIDX_DEAD = 0xFFFFFFFFu;     // pruned destination
-static const uint32_t DIDX_DEFER = 0xFFFFFFFEu;    // destination merged with the fresh-head state
 static const uint32_t FLAG_FRESH = 1u, FLAG_READOUT = 2u;
 static const int HDR_WORDS = 8;
-static const int GROUP_MAX_HEADS = 4;              // rows sharing one factor load
-static const int GROUP_MAX_COLS = 12;              // destination columns of one record
-static const int GROUP_MAX_ACC = 24;               // TH * TJ accumulators a record may need
+static const int TILE_A_HEADS = 4, TILE_A_COLS = 6;    // register tile A: 4 heads x 6 destination endpoints
+static const int TILE_B_HEADS = 2;                     // register tile B: 2 heads x GROUP_MAX_COLS endpoints (C: 1 head)
+static const int GROUP_MAX_HEADS = 4;                  // rows sharing one factor load
+static const int GROUP_MAX_COLS = 12;                  // destination columns of one record
 
 struct LayerProgram {
     uint32_t n_states = 0, n_masks = 0, n_rows = 0, n_groups = 0, max_L = 0;

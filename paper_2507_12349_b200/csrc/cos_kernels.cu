@@ -46,23 +46,27 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 struct TileCtx {
     const char* Xl;                      // source slab of the tile + lane * 8
     char* Yl;                            // destination slab of the tile + lane * 8
-    uint32_t gs_lane;                    // shared-memory byte address of Gs[0][lane]
-    uint32_t gd_lane;                    // ... of the plain diagonal Gd[0][lane]
+    const char* gs_base;                 // the staged table Gs (shared memory)
+    uint32_t gs_off;                     // byte offset of Gs[0][lane] from gs_base (= lane * 8)
+    uint32_t gd_off;                     // ... of the plain diagonal Gd[0][lane]
     uint32_t d, dstride;                 // table dimension, d * 256 bytes (one table row of 32 configurations)
     uint32_t S_src;                      // states of the source layer
     int prefetch;                        // L2 look-ahead distance in states (0: off)
     int lane;
 };
 
-// The source values of endpoint e for the TH heads of a record (0 where a head has no such state).
-template <int TH, bool FUSED>
-__device__ __forceinline__ void load_x(const uint32_t e, double (&x)[TH], uint32_t (&idx)[TH], const uint32_t (&al)[TH],
+// Keeps a loop-invariant value in a register: the compiler may not rematerialise it inside the loops below.
+__device__ __forceinline__ void pin(uint32_t& v) { asm volatile("" : "+r"(v)); }
+
+// The source values of endpoint e (bit = 1 << e; bit = 0: none) for the heads of a record, 0 where a head has no such state.
+template <int THM, bool FUSED>
+__device__ __forceinline__ void load_x(const uint32_t bit, double (&x)[THM], uint32_t (&idx)[THM], const uint32_t (&al)[THM],
                                        const char* __restrict__ Xl)
 {
 #pragma unroll
-    for (int t = 0; t < TH; ++t) {
+    for (int t = 0; t < THM; ++t) {
         x[t] = 0.0;
-        if ((al[t] >> e) & 1u) {
+        if (al[t] & bit) {
             const double* p = (const double*)(Xl + ((size_t)idx[t] << 8));
             x[t] = FUSED ? __ldcg(p) : __ldcs(p);
             ++idx[t];
@@ -70,131 +74,154 @@ __device__ __forceinline__ void load_x(const uint32_t e, double (&x)[TH], uint32
     }
 }
 
-// One source endpoint e of a record: TJ factor loads, TH x TJ FMAs; the cycle-closing factor G_lambda[e][h] (Eq. 12, 15)
-// is per head and never carries the counterterm (plain diagonal Gd when e == h).
-template <int TH, int TJ>
-__device__ __forceinline__ void apply_e(const uint32_t e, const double (&x)[TH], double (&acc)[TH][TJ > 0 ? TJ : 1],
-                                        double (&cl)[TH], const uint32_t (&joff)[TJ > 0 ? TJ : 1],
-                                        const uint32_t (&hoff)[TH], const uint32_t (&al)[TH], const uint32_t row0,
-                                        const uint32_t dstride, const uint32_t gdl, const bool do_close)
-{
-    const uint32_t ra = row0 + e * dstride;
-    double g[TJ > 0 ? TJ : 1];
-#pragma unroll
-    for (int q = 0; q < TJ; ++q) g[q] = lds64(ra + joff[q]);
-#pragma unroll
-    for (int q = 0; q < TJ; ++q)
-#pragma unroll
-        for (int t = 0; t < TH; ++t) acc[t][q] = fma(g[q], x[t], acc[t][q]);
-    if (do_close) {
-#pragma unroll
-        for (int t = 0; t < TH; ++t)
-            if ((al[t] >> e) & 1u) {
-                const uint32_t p = hoff[t] + ((hoff[t] == (e << 8)) ? gdl : ra);
-                cl[t] = fma(lds64(p), x[t], cl[t]);
-            }
-    }
-}
-
-// ------------------------------------------------------------------------------------------------------
-// One group record (cos_compile.h): TH heads x TJ destination endpoints of one colour.
-template <int TH, int TJ, bool FUSED>
-__device__ __forceinline__ void group_body(const uint4* __restrict__ rec, const uint4 q0, const TileCtx& c,
-                                           double& close, double (&sp)[4])
+// One group record (cos_compile.h) with exactly TJ destination endpoints on a register tile of THM heads (the record's
+// TH <= THM heads are a run-time value; unused rows carry x = 0):
+//   for every source endpoint e (increasing): TJ factor loads G_lambda[e][j] (shared by the heads), THM x TJ FMAs, and per
+//   head the cycle-closing factor G_lambda[e][h] (Eq. 12, 15), which never carries the counterterm (plain diagonal Gd
+//   when e == h); then one store per live (head, endpoint).
+// The source values stream through D register stages: the loads of endpoint k + D - 1 are in flight while endpoint k is
+// applied (stages are named statically -- a register move from a pending load would wait for it).
+template <int THM, int TJ, int D, bool FUSED>
+__device__ __forceinline__ void group_run(const uint4* __restrict__ rec, const uint4 q0, const int TH, uint32_t (&idx)[THM],
+                                          const uint32_t (&al)[THM], const uint32_t (&hoff)[THM], const TileCtx& c,
+                                          double& close)
 {
     constexpr int TJ1 = TJ > 0 ? TJ : 1;
-    const uint32_t g0 = q0.x, lam = (g0 >> 8) & 3u;
-    const bool do_close = (g0 >> 10) & 1u;
-    uint32_t idx[TH], al[TH], hoff[TH];
+    const uint32_t lam = (q0.x >> 8) & 3u;
+    const bool do_close = (q0.x >> 10) & 1u;
+    uint32_t joff[TJ1];
+    {
+        uint32_t jm = q0.z;
 #pragma unroll
-    for (int t = 0; t < TH; ++t) {
-        const uint4 qh = __ldg(rec + 1 + t);
-        idx[t] = qh.x; al[t] = qh.y; hoff[t] = qh.z << 8;
+        for (int q = 0; q < TJ; ++q) { joff[q] = (uint32_t)(__ffs((int)jm) - 1) << 8; jm &= jm - 1u; pin(joff[q]); }
+    }
+    uint32_t row0 = c.gs_off + lam * c.d * c.dstride, gdl = c.gd_off + ((lam * c.d) << 8), dstride = c.dstride;
+    pin(row0); pin(gdl); pin(dstride);
+    double acc[THM][TJ1];
+#pragma unroll
+    for (int t = 0; t < THM; ++t)
+#pragma unroll
+        for (int q = 0; q < TJ1; ++q) acc[t][q] = 0.0;
+    double cl0 = 0.0, cl1 = 0.0;
+
+    uint32_t em = q0.y;
+    uint32_t bq[D];
+    double xs[D][THM];
+#pragma unroll
+    for (int s = 0; s < D; ++s) {
+        bq[s] = em & (0u - em);                        // 0 after the last endpoint: load_x then loads nothing
+        em ^= bq[s];
+        load_x<THM, FUSED>(bq[s], xs[s], idx, al, c.Xl);
+    }
+    bool live = true;
+    while (live) {
+#pragma unroll
+        for (int s = 0; s < D; ++s) {
+            if (live) {
+                const uint32_t bit = bq[s];
+                const uint32_t e = 31u - (uint32_t)__clz((int)bit);
+                const uint32_t ra = row0 + e * dstride;
+                double g[TJ1];
+#pragma unroll
+                for (int q = 0; q < TJ; ++q) g[q] = *(const double*)(c.gs_base + (ra + joff[q]));
+#pragma unroll
+                for (int q = 0; q < TJ; ++q)
+#pragma unroll
+                    for (int t = 0; t < THM; ++t) acc[t][q] = fma(g[q], xs[s][t], acc[t][q]);
+                if (do_close) {
+#pragma unroll
+                    for (int t = 0; t < THM; ++t)
+                        if (al[t] & bit) {
+                            const uint32_t p = hoff[t] + ((hoff[t] == (e << 8)) ? gdl : ra);
+                            const double gc = *(const double*)(c.gs_base + p);
+                            if (t & 1) cl1 = fma(gc, xs[s][t], cl1); else cl0 = fma(gc, xs[s][t], cl0);
+                        }
+                }
+                bq[s] = em & (0u - em);
+                em ^= bq[s];
+                load_x<THM, FUSED>(bq[s], xs[s], idx, al, c.Xl);
+                live = bq[(s + 1) % D] != 0u;
+            }
+        }
+    }
+    if (TJ > 0) {
+        const uint2* dw = (const uint2*)(rec + 1 + TH);
+        constexpr int ROW2 = (TJ + 1) / 2;          // uint2 per destination row
+#pragma unroll
+        for (int t = 0; t < THM; ++t) {
+            if (t < TH) {
+#pragma unroll
+                for (int i = 0; i < ROW2; ++i) {
+                    const uint2 w2 = __ldg(dw + t * ROW2 + i);
+#pragma unroll
+                    for (int k = 0; k < 2; ++k) {
+                        if (2 * i + k < TJ) {
+                            const uint32_t w = k == 0 ? w2.x : w2.y;
+                            if (w != DIDX_DEAD) {
+                                double* y = (double*)(c.Yl + ((size_t)w << 8));
+                                if (FUSED) *y = acc[t][2 * i + k]; else __stcs(y, acc[t][2 * i + k]);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+    }
+    if (do_close) close += cl0 + cl1;
+}
+
+// Dispatch of a record on its register tile (THM heads, up to TJM endpoints, D source stages).
+template <int THM, int TJM, int D, bool FUSED>
+__device__ __forceinline__ void group_tile(const uint4* __restrict__ rec, const uint4 q0, const TileCtx& c, double& close)
+{
+    const int TH = (int)(q0.x & 7u), TJ = (int)((q0.x >> 3) & 31u);
+    uint32_t idx[THM], al[THM], hoff[THM];
+#pragma unroll
+    for (int t = 0; t < THM; ++t) {
+        idx[t] = 0u; al[t] = 0u; hoff[t] = 0u;
+        if (t < TH) {
+            const uint4 qh = __ldg(rec + 1 + t);
+            idx[t] = qh.x; al[t] = qh.y; hoff[t] = qh.z << 8;
+        }
     }
     if (c.prefetch > 0) {                // L2 look-ahead: the states `prefetch` states further down the slab
         uint32_t cnt = 0;
 #pragma unroll
-        for (int t = 0; t < TH; ++t) cnt += (uint32_t)__popc(al[t]);
+        for (int t = 0; t < THM; ++t) cnt += (uint32_t)__popc(al[t]);
         const char* X0 = c.Xl - c.lane * 8;
         for (uint32_t q = (uint32_t)c.lane; q < 2u * cnt; q += 32u) {
             const uint32_t st = q0.w + (uint32_t)c.prefetch + (q >> 1);
             if (st < c.S_src) prefetch_l2(X0 + ((size_t)st << 8) + (size_t)(q & 1u) * 128);
         }
     }
-    uint32_t joff[TJ1];
-    {
-        uint32_t jm = q0.z;
-#pragma unroll
-        for (int q = 0; q < TJ; ++q) { joff[q] = (uint32_t)(__ffs((int)jm) - 1) << 8; jm &= jm - 1u; }
-    }
-    const uint32_t row0 = c.gs_lane + lam * c.d * c.dstride;
-    const uint32_t gdl = c.gd_lane + ((lam * c.d) << 8);
-    double acc[TH][TJ1], cl[TH];
-#pragma unroll
-    for (int t = 0; t < TH; ++t) {
-        cl[t] = 0.0;
-#pragma unroll
-        for (int q = 0; q < TJ1; ++q) acc[t][q] = 0.0;
-    }
-    // source endpoints in increasing order, the loads of the next one issued before the FMAs of the current one
-    uint32_t em = q0.y;
-    double xa[TH], xb[TH];
-    uint32_t e0 = (uint32_t)(__ffs((int)em) - 1), e1;
-    em &= em - 1u;
-    load_x<TH, FUSED>(e0, xa, idx, al, c.Xl);
-    for (;;) {
-        e1 = 32u;
-        if (em) { e1 = (uint32_t)(__ffs((int)em) - 1); em &= em - 1u; load_x<TH, FUSED>(e1, xb, idx, al, c.Xl); }
-        apply_e<TH, TJ>(e0, xa, acc, cl, joff, hoff, al, row0, c.dstride, gdl, do_close);
-        if (e1 == 32u) break;
-        e0 = 32u;
-        if (em) { e0 = (uint32_t)(__ffs((int)em) - 1); em &= em - 1u; load_x<TH, FUSED>(e0, xa, idx, al, c.Xl); }
-        apply_e<TH, TJ>(e1, xb, acc, cl, joff, hoff, al, row0, c.dstride, gdl, do_close);
-        if (e0 == 32u) break;
-    }
-    // destinations: one store per live (head, endpoint); the one that merges with the fresh-head state is kept
-    if (TJ > 0) {
-        const uint4* dw = rec + 1 + TH;
-        double spv = 0.0;
-        bool has_sp = false;
-#pragma unroll
-        for (int i = 0; i < (TH * TJ + 3) / 4; ++i) {
-            const uint4 w4 = __ldg(dw + i);
-#pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const int f = 4 * i + k;
-                if (f < TH * TJ) {
-                    const uint32_t w = k == 0 ? w4.x : k == 1 ? w4.y : k == 2 ? w4.z : w4.w;
-                    const double v = acc[f / TJ1][f % TJ1];
-                    if (w < DIDX_DEFER) {
-                        double* y = (double*)(c.Yl + ((size_t)w << 8));
-                        if (FUSED) *y = v; else __stcs(y, v);
-                    } else if (w == DIDX_DEFER) { spv = v; has_sp = true; }
+#define COS_RUN_CASE(TJ_) \
+    case TJ_: group_run<THM, (TJ_ <= TJM ? TJ_ : 0), D, FUSED>(rec, q0, TH, idx, al, hoff, c, close); break;
+    switch (TJ) {
+        COS_RUN_CASE(0) COS_RUN_CASE(1) COS_RUN_CASE(2) COS_RUN_CASE(3) COS_RUN_CASE(4) COS_RUN_CASE(5) COS_RUN_CASE(6)
+        default:
+            if (TJM > 6) {
+                switch (TJ) {
+                    COS_RUN_CASE(7) COS_RUN_CASE(8) COS_RUN_CASE(9) COS_RUN_CASE(10) COS_RUN_CASE(11) COS_RUN_CASE(12)
+                    default: break;
                 }
             }
-        }
-#pragma unroll
-        for (int k = 0; k < 4; ++k) sp[k] = (has_sp && (uint32_t)k == lam) ? spv : sp[k];
+            break;
     }
-    if (do_close) {
-        double s = cl[0];
-#pragma unroll
-        for (int t = 1; t < TH; ++t) s += cl[t];
-        close += s;
-    }
+#undef COS_RUN_CASE
 }
 
 // All source blocks [m_begin, m_end) of one layer for one batch tile: the body shared by the per-layer kernel and the
 // fused small-DAG kernel.  s_next (shared) must be 0 and visible to the CTA on entry.
 template <bool FUSED>
 __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t m_begin, const uint32_t m_end,
-                                             const uint32_t tile, unsigned int& s_next, const uint32_t gs_lane,
-                                             const uint32_t gd_lane, const int lane, const bool valid, const long long b)
+                                             const uint32_t tile, unsigned int& s_next, const double* Gs,
+                                             const int lane, const bool valid, const long long b)
 {
     TileCtx c;
     c.Xl = (const char*)(a.X + (size_t)tile * a.S_src * TILE + lane);
     c.Yl = (char*)(a.Y + (size_t)tile * a.S_dst * TILE + lane);
-    c.gs_lane = gs_lane; c.gd_lane = gd_lane; c.d = (uint32_t)a.d; c.dstride = (uint32_t)a.d * (TILE * 8u);
+    c.gs_base = (const char*)Gs; c.gs_off = (uint32_t)lane * 8u; c.gd_off = c.gs_off + (uint32_t)a.n_slots * (TILE * 8u);
+    c.d = (uint32_t)a.d; c.dstride = (uint32_t)a.d * (TILE * 8u);
     c.S_src = a.S_src; c.prefetch = a.prefetch; c.lane = lane;
     const uint2* mtab = (const uint2*)a.mask_off;
 
@@ -222,7 +249,6 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
         const int n_groups = (int)(h0.x & 0xFFFFu);
         const uint32_t flags = h0.x >> 24;
         double close = 0.0;
-        double sp[4] = {0.0, 0.0, 0.0, 0.0};
 
         const uint4* rec = bp + 2;
         uint4 q0 = n_groups > 0 ? __ldg(rec) : make_uint4(0u, 0u, 0u, 0u);
@@ -233,32 +259,26 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
                 q0_n = __ldg(rec_n);
                 prefetch_l1((const char*)rec_n + 128);
             }
-#define COS_GROUP_CASE(TH_, TJ_) \
-    case ((TH_) | ((TJ_) << 3)): group_body<TH_, TJ_, FUSED>(rec, q0, c, close, sp); break;
-            switch (q0.x & 0xFFu) {
-                COS_GROUP_CASE(1, 0) COS_GROUP_CASE(1, 1) COS_GROUP_CASE(1, 2) COS_GROUP_CASE(1, 3) COS_GROUP_CASE(1, 4)
-                COS_GROUP_CASE(1, 5) COS_GROUP_CASE(1, 6) COS_GROUP_CASE(1, 7) COS_GROUP_CASE(1, 8) COS_GROUP_CASE(1, 9)
-                COS_GROUP_CASE(1, 10) COS_GROUP_CASE(1, 11) COS_GROUP_CASE(1, 12)
-                COS_GROUP_CASE(2, 0) COS_GROUP_CASE(2, 1) COS_GROUP_CASE(2, 2) COS_GROUP_CASE(2, 3) COS_GROUP_CASE(2, 4)
-                COS_GROUP_CASE(2, 5) COS_GROUP_CASE(2, 6) COS_GROUP_CASE(2, 7) COS_GROUP_CASE(2, 8) COS_GROUP_CASE(2, 9)
-                COS_GROUP_CASE(2, 10) COS_GROUP_CASE(2, 11) COS_GROUP_CASE(2, 12)
-                COS_GROUP_CASE(3, 0) COS_GROUP_CASE(3, 1) COS_GROUP_CASE(3, 2) COS_GROUP_CASE(3, 3) COS_GROUP_CASE(3, 4)
-                COS_GROUP_CASE(3, 5) COS_GROUP_CASE(3, 6) COS_GROUP_CASE(3, 7) COS_GROUP_CASE(3, 8)
-                COS_GROUP_CASE(4, 0) COS_GROUP_CASE(4, 1) COS_GROUP_CASE(4, 2) COS_GROUP_CASE(4, 3) COS_GROUP_CASE(4, 4)
-                COS_GROUP_CASE(4, 5) COS_GROUP_CASE(4, 6)
-                default: break;
+            {   // register tile by head count (cos_compile.h): A = 4 x 6, B = 2 x 12, C = 1 x 12
+                const uint32_t th = q0.x & 7u;
+                if (th >= 3u) group_tile<4, 6, 3, FUSED>(rec, q0, c, close);
+                else if (th == 2u) group_tile<2, 12, 3, FUSED>(rec, q0, c, close);
+                else group_tile<1, 12, 4, FUSED>(rec, q0, c, close);
             }
-#undef COS_GROUP_CASE
             rec = rec_n; q0 = q0_n;
         }
         if (flags & FLAG_FRESH) {            // close-and-open: fresh head of every colour (Eq. 12, 70-71)
+            // h0.w bit k: a row of this block has already stored its continuation into the fresh-head state of colour k
+            // (the coalesced E2/E4 pair): add the closing sum to it
             const uint4 fd = __ldg(bp + 1);
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const uint32_t didx = k == 0 ? fd.x : k == 1 ? fd.y : k == 2 ? fd.z : fd.w;
                 if (didx != DIDX_DEAD) {
                     double* y = (double*)(c.Yl + ((size_t)didx << 8));
-                    const double v = fma(a.neg_kappa, close, sp[k]);
+                    double v = 0.0;
+                    if ((h0.w >> k) & 1u) v = __ldcg(y);
+                    v = fma(a.neg_kappa, close, v);
                     if (FUSED) *y = v; else __stcs(y, v);
                 }
             }
@@ -280,7 +300,6 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
     const uint32_t tile = blockIdx.x;
 
     const uint32_t gs_lane = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)lane * 8u;
-    const uint32_t gd_lane = gs_lane + (uint32_t)a.n_slots * (TILE * 8u);
 
     // Programmatic dependent launch: let the next layer's grid start (it only stages its table, which no layer
     // writes) while this grid drains; this grid in turn touches the slabs only after the previous one has completed.
@@ -311,7 +330,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
     if (a.pdl) asm volatile("griddepcontrol.wait;" ::: "memory");
     const uint32_t m_begin = blockIdx.y * a.masks_per_cta;
     const uint32_t m_end = min(a.n_masks, m_begin + a.masks_per_cta);
-    layer_blocks<false>(a, m_begin, m_end, tile, s_next, gs_lane, gd_lane, lane, valid, b);
+    layer_blocks<false>(a, m_begin, m_end, tile, s_next, Gs, lane, valid, b);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -327,7 +346,6 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
     const uint32_t tile = blockIdx.x;
     const uint32_t gs_lane = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)lane * 8u;
-    const uint32_t gd_lane = gs_lane + (uint32_t)f.n_slots * (TILE * 8u);
     const long long b = f.b0 + (long long)tile * TILE + lane;
     const bool valid = b < f.batch;
     if (threadIdx.x == 0) s_next = 0u;
@@ -364,7 +382,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
         a.words = fl.words; a.mask_off = fl.mask_off; a.n_masks = fl.n_masks;
         a.X = (l & 1) ? slab1 : slab0; a.Y = (l & 1) ? slab0 : slab1;
         // slabs are addressed per tile already: tile index 0 inside layer_blocks
-        layer_blocks<true>(a, 0u, fl.n_masks, 0u, s_next, gs_lane, gd_lane, lane, valid, b);
+        layer_blocks<true>(a, 0u, fl.n_masks, 0u, s_next, Gs, lane, valid, b);
         __threadfence_block();
         __syncthreads();
         if (threadIdx.x == 0) s_next = 0u;
