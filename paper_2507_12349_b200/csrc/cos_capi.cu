@@ -41,7 +41,7 @@ struct cos_handle_s {
     long long ws_limit = 64ll << 30;
     // launch shape and tuning (cos_set_tuning); nothing here is read from the environment
     int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148;
-    int prefetch = 256;                   // L2 look-ahead distance in states
+    int prefetch = 8;                     // L2 look-ahead: states fetched ahead when a block is claimed
     int blocks_per_cta_cap = 0;           // 0: one block per staged table slot (64 .. 1024)
     int pdl = 1;                          // programmatic dependent launch between layers
     int host_slices = 8;                  // cos_eval_host: at most this many output slices (1: no second stream)
@@ -118,7 +118,7 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
     }
 
     const CompiledDag& D = h->dag;
-    const size_t smem = layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d);
+    const size_t smem = layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d, 4);
     if (smem > LAYER_SMEM_MAX) {
         delete h;
         return fail(COS_EUNSUPPORTED, "cos_build: propagator tile does not fit the 227 KB shared memory of one SM");
@@ -234,7 +234,8 @@ static int grow_workspace(cos_handle h, size_t need, const char* who)
 {
     if (need <= h->ws_bytes) return COS_OK;
     if (h->ws) { cudaFree(h->ws); h->ws = nullptr; h->ws_bytes = 0; }
-    cudaError_t e = cudaMalloc(&h->ws, need);
+    // (+ 4 KB: the layer kernel prefetches a few states past the one it reads)
+    cudaError_t e = cudaMalloc(&h->ws, need + 4096);
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, who); }
     h->ws_bytes = need;
     return COS_OK;

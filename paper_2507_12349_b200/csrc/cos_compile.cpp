@@ -289,9 +289,10 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                     P.words.push_back((lam < nc && (flags & FLAG_FRESH))
                                           ? b.state_index((uint32_t)fresh_did, (int)fresh_a, lam, (int)fresh_a) : DIDX_DEAD);
                 uint32_t n_groups = 0, merged = 0;
+                std::vector<uint32_t> rec_at;                    // word offsets of the block's records, in program order
                 for (int ch = 0; ch < n_chunks; ++ch) {
                     const int c0 = n_cols * ch / n_chunks, c1 = n_cols * (ch + 1) / n_chunks, TJ = c1 - c0;
-                    const int th_max = TJ <= TILE_A_COLS ? TILE_A_HEADS : TILE_B_HEADS;
+                    const int th_max = TJ <= TILE_A_COLS ? TILE_A_HEADS : TJ <= TILE_B_COLS ? TILE_B_HEADS : 1;
                     const int n_hgroups = (n_heads + th_max - 1) / th_max;
                     for (int lam = 0; lam < nc; ++lam)
                         for (int g = 0; g < n_hgroups; ++g) {
@@ -302,8 +303,11 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                             const uint32_t row_words = ((uint32_t)TJ + 1u) & ~1u;      // destination rows are 8-byte aligned
                             const uint32_t len = 4u + 4u * (uint32_t)TH + (((uint32_t)TH * row_words + 3u) & ~3u);
                             if (P.words.size() + len >= 0xFFFFFFF0ull) return "unsupported: layer program exceeds 2^32 words";
+                            uint32_t n_src = 0;                                  // source states of the record
+                            for (int k = h0; k < h1; ++k) n_src += (uint32_t)__builtin_popcount(b.alive[(size_t)id * d + heads[k]]);
+                            rec_at.push_back((uint32_t)P.words.size());
                             P.words.push_back((uint32_t)TH | ((uint32_t)TJ << 3) | ((uint32_t)lam << 8) |
-                                              ((need_close && ch == 0) ? 1u << 10 : 0u) | ((len / 4u) << 24));
+                                              ((need_close && ch == 0) ? 1u << 10 : 0u) | (n_src << 11) | ((len / 4u) << 24));
                             P.words.push_back(emask);
                             P.words.push_back(jmask);
                             P.words.push_back(b.row_base[(size_t)id * d + heads[h0]] + (uint32_t)lam * b.colour_stride[id]);
@@ -353,6 +357,13 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                         if (flags & FLAG_READOUT) P.readout_edges += L;
                         if (need_close) { P.n_fma += L; P.n_factor_loads += L; P.n_factor_loads_unshared += L; }
                     }
+                }
+                // L2 look-ahead hints: record i names the source range of record i + GROUP_LOOKAHEAD of the same block
+                for (size_t i = 0; i + GROUP_LOOKAHEAD < rec_at.size(); ++i) {
+                    const uint32_t tgt = rec_at[i + GROUP_LOOKAHEAD];
+                    const uint32_t cnt = (P.words[tgt] >> 11) & 0x7Fu;
+                    P.words[rec_at[i]] |= ((cnt + 1u) / 2u) << 18;
+                    P.words[rec_at[i] + 7] = P.words[tgt + 3];
                 }
                 if (n_groups > 0xFFFFu) return "unsupported: more than 65535 group records in one block";
                 P.words[w_block] |= n_groups;

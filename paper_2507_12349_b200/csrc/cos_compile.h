@@ -29,15 +29,19 @@ namespace cosb {
 // factor-application sharing of PAPER.md Eq. 29-31: G_lambda[e][j] does not depend on the head, so one staged factor
 // feeds the rows of all heads of the group (N_mult = min(|S_f|, |D_f|) -> one load per group instead of one per row):
 //   q0 : g0 | emask | jmask | first
-//        g0    = TH[0:3) | TJ[3:8) | lambda[8:10) | do_close[10] | len4[24:32)   (len4 = record length in uint4 units)
+//        g0    = TH[0:3) | TJ[3:8) | lambda[8:10) | do_close[10] | n_src[11:18) | ahead2[18:24) | len4[24:32)
+//                (n_src = source states of the record, len4 = record length in uint4 units; ahead2 * 2 states starting
+//                at slab index `ahead` below are the sources of the record GROUP_LOOKAHEAD records later in this block:
+//                the kernel prefetches them into L2 when it starts this record; 0 = nothing to prefetch)
 //        emask = union over the heads of their live current endpoints e_a (bit e_a)
 //        jmask = destination endpoints j_a of the TJ columns of this record (bit j_a), in increasing order
 //        first = slab index of the group's first state (its states are contiguous: heads in increasing order)
-//   TH x qh : base | alive | h_a | 0     base = slab index of the head's first state, alive = its live endpoints (bit e_a)
+//   TH x qh : base | alive | h_a | ahead   base = slab index of the head's first state, alive = its live endpoints (bit
+//        e_a); ahead: look-ahead range start (first head only, see g0)
 //   TH rows of TJ destination words, each row padded to an even number of words (and the record to a multiple of 4):
 //        index of the destination state in the next layer's slab, or DIDX_DEAD (pruned, Eq. 23, or padding).
 //   Register tiles of the kernel: up to TILE_A_HEADS heads when the block has at most TILE_A_COLS live destination
-//   endpoints, else up to TILE_B_HEADS heads x GROUP_MAX_COLS endpoints.  Blocks with more than GROUP_MAX_COLS live
+//   endpoints, up to TILE_B_HEADS heads for at most TILE_B_COLS, else one head x GROUP_MAX_COLS endpoints.  Blocks with more than GROUP_MAX_COLS live
 //   destination endpoints are split into column chunks (one set of records per chunk; do_close is set in the first
 //   chunk only, so that the cycle-closing sum is taken once).
 // The multiplicity 2 - m_j = 2 of a continuation into an untouched interaction (Lemma 7) is NOT applied per edge:
@@ -47,9 +51,10 @@ static const uint32_t DIDX_DEAD = 0xFFFFFFFFu;     // pruned destination
 static const uint32_t FLAG_FRESH = 1u, FLAG_READOUT = 2u;
 static const int HDR_WORDS = 8;
 static const int TILE_A_HEADS = 4, TILE_A_COLS = 6;    // register tile A: 4 heads x 6 destination endpoints
-static const int TILE_B_HEADS = 2;                     // register tile B: 2 heads x GROUP_MAX_COLS endpoints (C: 1 head)
+static const int TILE_B_HEADS = 2, TILE_B_COLS = 8;    // register tile B: 2 heads x 8 endpoints; tile C: 1 head x GROUP_MAX_COLS
 static const int GROUP_MAX_HEADS = 4;                  // rows sharing one factor load
 static const int GROUP_MAX_COLS = 12;                  // destination columns of one record
+static const int GROUP_LOOKAHEAD = 1;                  // L2 look-ahead distance in records
 
 struct LayerProgram {
     uint32_t n_states = 0, n_masks = 0, n_rows = 0, n_groups = 0, max_L = 0;

@@ -21,6 +21,23 @@
 #include "cos_kernels.cuh"
 #include "cos_compile.h"
 
+// source-value stages (prefetch depth) of the three register tiles
+#ifndef COS_BULK_PREFETCH
+#define COS_BULK_PREFETCH 1
+#endif
+#ifndef COS_L1_AHEAD
+#define COS_L1_AHEAD 2
+#endif
+#ifndef COS_STAGES_A
+#define COS_STAGES_A 2
+#endif
+#ifndef COS_STAGES_B
+#define COS_STAGES_B 3
+#endif
+#ifndef COS_STAGES_C
+#define COS_STAGES_C 4
+#endif
+
 namespace cosb {
 
 static const int MAX_WARPS = 16;         // 128 registers per thread
@@ -33,10 +50,32 @@ __device__ __forceinline__ double lds64(uint32_t addr)
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
+// one bulk (TMA) prefetch of a contiguous range into L2; bytes is a multiple of 16
+__device__ __forceinline__ void prefetch_l2_bulk(const void* p, uint32_t bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
 // asynchronous 8-byte global -> shared copy (LDGSTS): no register staging, completion by commit / wait groups
 __device__ __forceinline__ void cp_async8(uint32_t dst, const void* src)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
+}
+// 16-byte variant (L2 only): program records -> the warp's record slots
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src)
+{
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ uint4 lds128u(uint32_t addr)
+{
+    uint4 v;
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ uint2 lds64u(uint32_t addr)
+{
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+    return v;
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
@@ -46,12 +85,11 @@ __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_gr
 struct TileCtx {
     const char* Xl;                      // source slab of the tile + lane * 8
     char* Yl;                            // destination slab of the tile + lane * 8
-    const char* gs_base;                 // the staged table Gs (shared memory)
-    uint32_t gs_off;                     // byte offset of Gs[0][lane] from gs_base (= lane * 8)
-    uint32_t gd_off;                     // ... of the plain diagonal Gd[0][lane]
+    uint32_t gs_lane;                    // shared-memory byte address of Gs[0][lane]
+    uint32_t gd_lane;                    // ... of the plain diagonal Gd[0][lane]
     uint32_t d, dstride;                 // table dimension, d * 256 bytes (one table row of 32 configurations)
     uint32_t S_src;                      // states of the source layer
-    int prefetch;                        // L2 look-ahead distance in states (0: off)
+    int prefetch;                        // L2 look-ahead (0: off; else the states fetched ahead when a block is claimed)
     int lane;
 };
 
@@ -69,6 +107,10 @@ __device__ __forceinline__ void load_x(const uint32_t bit, double (&x)[THM], uin
         if (al[t] & bit) {
             const double* p = (const double*)(Xl + ((size_t)idx[t] << 8));
             x[t] = FUSED ? __ldcg(p) : __ldcs(p);
+#if COS_L1_AHEAD > 0
+            // pull the line this head reads COS_L1_AHEAD states later into L1 (no register needed; the slab is padded)
+            if (!FUSED) asm volatile("prefetch.global.L1 [%0+%1];" ::"l"(p), "n"(COS_L1_AHEAD * 256));
+#endif
             ++idx[t];
         }
     }
@@ -82,27 +124,31 @@ __device__ __forceinline__ void load_x(const uint32_t bit, double (&x)[THM], uin
 // The source values stream through D register stages: the loads of endpoint k + D - 1 are in flight while endpoint k is
 // applied (stages are named statically -- a register move from a pending load would wait for it).
 template <int THM, int TJ, int D, bool FUSED>
-__device__ __forceinline__ void group_run(const uint4* __restrict__ rec, const uint4 q0, const int TH, uint32_t (&idx)[THM],
+__device__ __forceinline__ void group_run(const uint32_t rec, const uint4 q0, const int TH, uint32_t (&idx)[THM],
                                           const uint32_t (&al)[THM], const uint32_t (&hoff)[THM], const TileCtx& c,
                                           double& close)
 {
     constexpr int TJ1 = TJ > 0 ? TJ : 1;
     const uint32_t lam = (q0.x >> 8) & 3u;
     const bool do_close = (q0.x >> 10) & 1u;
-    uint32_t joff[TJ1];
+    uint32_t dstride = c.dstride;
+    pin(dstride);
+    // shared-memory byte addresses: column j of table row 0 of this colour (+ e * dstride = G_lambda[e][j]), the
+    // closing column of every head, and its plain-diagonal entry Gd_lambda[h]
+    uint32_t colq[TJ1];
+    uint32_t row0 = c.gs_lane + lam * c.d * dstride, gdl = c.gd_lane + ((lam * c.d) << 8);
+    pin(row0); pin(gdl);
     {
         uint32_t jm = q0.z;
 #pragma unroll
-        for (int q = 0; q < TJ; ++q) { joff[q] = (uint32_t)(__ffs((int)jm) - 1) << 8; jm &= jm - 1u; pin(joff[q]); }
+        for (int q = 0; q < TJ; ++q) { colq[q] = row0 + ((uint32_t)(__ffs((int)jm) - 1) << 8); jm &= jm - 1u; pin(colq[q]); }
     }
-    uint32_t row0 = c.gs_off + lam * c.d * c.dstride, gdl = c.gd_off + ((lam * c.d) << 8), dstride = c.dstride;
-    pin(row0); pin(gdl); pin(dstride);
     double acc[THM][TJ1];
 #pragma unroll
     for (int t = 0; t < THM; ++t)
 #pragma unroll
         for (int q = 0; q < TJ1; ++q) acc[t][q] = 0.0;
-    double cl0 = 0.0, cl1 = 0.0;
+    double cl = 0.0;
 
     uint32_t em = q0.y;
     uint32_t bq[D];
@@ -118,24 +164,19 @@ __device__ __forceinline__ void group_run(const uint4* __restrict__ rec, const u
 #pragma unroll
         for (int s = 0; s < D; ++s) {
             if (live) {
-                const uint32_t bit = bq[s];
-                const uint32_t e = 31u - (uint32_t)__clz((int)bit);
-                const uint32_t ra = row0 + e * dstride;
+                const uint32_t e = 31u - (uint32_t)__clz((int)bq[s]);
+                const uint32_t ro = e * dstride;
                 double g[TJ1];
 #pragma unroll
-                for (int q = 0; q < TJ; ++q) g[q] = *(const double*)(c.gs_base + (ra + joff[q]));
+                for (int q = 0; q < TJ; ++q) g[q] = lds64(colq[q] + ro);
 #pragma unroll
                 for (int q = 0; q < TJ; ++q)
 #pragma unroll
                     for (int t = 0; t < THM; ++t) acc[t][q] = fma(g[q], xs[s][t], acc[t][q]);
-                if (do_close) {
+                if (do_close) {      // a head without this source state has x = 0: its (valid) factor load is harmless
 #pragma unroll
                     for (int t = 0; t < THM; ++t)
-                        if (al[t] & bit) {
-                            const uint32_t p = hoff[t] + ((hoff[t] == (e << 8)) ? gdl : ra);
-                            const double gc = *(const double*)(c.gs_base + p);
-                            if (t & 1) cl1 = fma(gc, xs[s][t], cl1); else cl0 = fma(gc, xs[s][t], cl0);
-                        }
+                        cl = fma(lds64(hoff[t] + ((hoff[t] == (e << 8)) ? gdl : row0 + ro)), xs[s][t], cl);
                 }
                 bq[s] = em & (0u - em);
                 em ^= bq[s];
@@ -145,14 +186,14 @@ __device__ __forceinline__ void group_run(const uint4* __restrict__ rec, const u
         }
     }
     if (TJ > 0) {
-        const uint2* dw = (const uint2*)(rec + 1 + TH);
+        const uint32_t dw = rec + 16u * (uint32_t)(1 + TH);
         constexpr int ROW2 = (TJ + 1) / 2;          // uint2 per destination row
 #pragma unroll
         for (int t = 0; t < THM; ++t) {
             if (t < TH) {
 #pragma unroll
                 for (int i = 0; i < ROW2; ++i) {
-                    const uint2 w2 = __ldg(dw + t * ROW2 + i);
+                    const uint2 w2 = lds64u(dw + 8u * (uint32_t)(t * ROW2 + i));
 #pragma unroll
                     for (int k = 0; k < 2; ++k) {
                         if (2 * i + k < TJ) {
@@ -167,12 +208,12 @@ __device__ __forceinline__ void group_run(const uint4* __restrict__ rec, const u
             }
         }
     }
-    if (do_close) close += cl0 + cl1;
+    if (do_close) close += cl;
 }
 
 // Dispatch of a record on its register tile (THM heads, up to TJM endpoints, D source stages).
 template <int THM, int TJM, int D, bool FUSED>
-__device__ __forceinline__ void group_tile(const uint4* __restrict__ rec, const uint4 q0, const TileCtx& c, double& close)
+__device__ __forceinline__ void group_tile(const uint32_t rec, const uint4 q0, const TileCtx& c, double& close)
 {
     const int TH = (int)(q0.x & 7u), TJ = (int)((q0.x >> 3) & 31u);
     uint32_t idx[THM], al[THM], hoff[THM];
@@ -180,18 +221,13 @@ __device__ __forceinline__ void group_tile(const uint4* __restrict__ rec, const 
     for (int t = 0; t < THM; ++t) {
         idx[t] = 0u; al[t] = 0u; hoff[t] = 0u;
         if (t < TH) {
-            const uint4 qh = __ldg(rec + 1 + t);
+            const uint4 qh = lds128u(rec + 16u * (uint32_t)(1 + t));
             idx[t] = qh.x; al[t] = qh.y; hoff[t] = qh.z << 8;
-        }
-    }
-    if (c.prefetch > 0) {                // L2 look-ahead: the states `prefetch` states further down the slab
-        uint32_t cnt = 0;
-#pragma unroll
-        for (int t = 0; t < THM; ++t) cnt += (uint32_t)__popc(al[t]);
-        const char* X0 = c.Xl - c.lane * 8;
-        for (uint32_t q = (uint32_t)c.lane; q < 2u * cnt; q += 32u) {
-            const uint32_t st = q0.w + (uint32_t)c.prefetch + (q >> 1);
-            if (st < c.S_src) prefetch_l2(X0 + ((size_t)st << 8) + (size_t)(q & 1u) * 128);
+            // L2 look-ahead: the sources of the record GROUP_LOOKAHEAD records later (contiguous: one bulk prefetch)
+            if (t == 0 && c.prefetch > 0 && c.lane == 0) {
+                const uint32_t ahead2 = (q0.x >> 18) & 0x3Fu;
+                if (ahead2) prefetch_l2_bulk(c.Xl + ((size_t)qh.w << 8), ahead2 << 9);
+            }
         }
     }
 #define COS_RUN_CASE(TJ_) \
@@ -201,8 +237,15 @@ __device__ __forceinline__ void group_tile(const uint4* __restrict__ rec, const 
         default:
             if (TJM > 6) {
                 switch (TJ) {
-                    COS_RUN_CASE(7) COS_RUN_CASE(8) COS_RUN_CASE(9) COS_RUN_CASE(10) COS_RUN_CASE(11) COS_RUN_CASE(12)
-                    default: break;
+                    COS_RUN_CASE(7) COS_RUN_CASE(8)
+                    default:
+                        if (TJM > 8) {
+                            switch (TJ) {
+                                COS_RUN_CASE(9) COS_RUN_CASE(10) COS_RUN_CASE(11) COS_RUN_CASE(12)
+                                default: break;
+                            }
+                        }
+                        break;
                 }
             }
             break;
@@ -214,63 +257,80 @@ __device__ __forceinline__ void group_tile(const uint4* __restrict__ rec, const 
 // fused small-DAG kernel.  s_next (shared) must be 0 and visible to the CTA on entry.
 template <bool FUSED>
 __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t m_begin, const uint32_t m_end,
-                                             const uint32_t tile, unsigned int& s_next, const double* Gs,
-                                             const int lane, const bool valid, const long long b)
+                                             const uint32_t tile, unsigned int& s_next, const uint32_t gs_lane,
+                                             const uint32_t rs_warp, const int lane, const bool valid, const long long b)
 {
     TileCtx c;
     c.Xl = (const char*)(a.X + (size_t)tile * a.S_src * TILE + lane);
     c.Yl = (char*)(a.Y + (size_t)tile * a.S_dst * TILE + lane);
-    c.gs_base = (const char*)Gs; c.gs_off = (uint32_t)lane * 8u; c.gd_off = c.gs_off + (uint32_t)a.n_slots * (TILE * 8u);
+    c.gs_lane = gs_lane; c.gd_lane = gs_lane + (uint32_t)a.n_slots * (TILE * 8u);
+    pin(c.gs_lane); pin(c.gd_lane);
     c.d = (uint32_t)a.d; c.dstride = (uint32_t)a.d * (TILE * 8u);
     c.S_src = a.S_src; c.prefetch = a.prefetch; c.lane = lane;
     const uint2* mtab = (const uint2*)a.mask_off;
 
-    // Blocks are handed to warps dynamically (block sizes vary).  A warp always knows its current AND its next block:
-    // the next block's header is fetched while the current block is processed.
+    // Blocks are handed to warps dynamically (block sizes vary).  A warp always knows its current AND its next block.
+    // The program is read through per-warp shared-memory slots of 256 bytes filled by asynchronous copies one step ahead
+    // (lanes 0..15 copy 16 bytes each): slots 0/1 take a block header together with the block's first record, slots 2/3
+    // the following records, so that no record field is ever waited for at global-memory latency.
+    const uint32_t slot_lane = rs_warp + (uint32_t)(lane & 15) * 16u;
     uint32_t mi = 0;
     if (lane == 0) mi = atomicAdd(&s_next, 1u);
     mi = __shfl_sync(0xFFFFFFFFu, mi, 0) + m_begin;
     const uint4* bp = nullptr;
-    uint4 h0 = make_uint4(0u, 0u, 0u, 0u);
+    uint32_t pb = 0u;                        // block slot of the current block
     if (mi < m_end) {
         bp = (const uint4*)(a.words + __ldg(&mtab[mi]).x);
-        h0 = __ldg(bp);
+        if (lane < 16) cp_async16(slot_lane, bp + lane);
     }
+    cp_async_commit();
     while (mi < m_end) {
         uint32_t mi_n = 0;
         if (lane == 0) mi_n = atomicAdd(&s_next, 1u);
         mi_n = __shfl_sync(0xFFFFFFFFu, mi_n, 0) + m_begin;
         const uint4* bp_n = nullptr;
-        uint4 h0_n = make_uint4(0u, 0u, 0u, 0u);
         if (mi_n < m_end) {
-            bp_n = (const uint4*)(a.words + __ldg(&mtab[mi_n]).x);
-            h0_n = __ldg(bp_n);
+            const uint2 mt = __ldg(&mtab[mi_n]);
+            bp_n = (const uint4*)(a.words + mt.x);
+            if (lane < 16) cp_async16(slot_lane + ((pb ^ 1u) << 8), bp_n + lane);
+            // L2 look-ahead: the first states of the block this warp takes next (one bulk prefetch, a block away in time)
+            if (a.prefetch > 0 && lane == 0) {
+                uint32_t cnt = __ldg(&mtab[mi_n + 1].y) - mt.y;
+                if (cnt > (uint32_t)a.prefetch) cnt = (uint32_t)a.prefetch;
+                if (cnt) prefetch_l2_bulk(c.Xl + ((size_t)mt.y << 8), cnt << 8);
+            }
         }
+        cp_async_commit();
+        cp_async_wait<1>();                  // everything but the copy just issued: the current block's slot is complete
+        __syncwarp();
+        const uint32_t bs = rs_warp + (pb << 8);
+        const uint4 h0 = lds128u(bs);
         const int n_groups = (int)(h0.x & 0xFFFFu);
         const uint32_t flags = h0.x >> 24;
         double close = 0.0;
 
-        const uint4* rec = bp + 2;
-        uint4 q0 = n_groups > 0 ? __ldg(rec) : make_uint4(0u, 0u, 0u, 0u);
+        const uint4* rec_g = bp + 2;         // global address of the current record
+        uint32_t rec = bs + 32u;             // its shared-memory copy
         for (int g = 0; g < n_groups; ++g) {
-            const uint4* rec_n = rec + (q0.x >> 24);
-            uint4 q0_n = make_uint4(0u, 0u, 0u, 0u);
-            if (g + 1 < n_groups) {
-                q0_n = __ldg(rec_n);
-                prefetch_l1((const char*)rec_n + 128);
-            }
-            {   // register tile by head count (cos_compile.h): A = 4 x 6, B = 2 x 12, C = 1 x 12
+            const uint4 q0 = lds128u(rec);
+            rec_g += q0.x >> 24;
+            const uint32_t rec_n = rs_warp + 512u + (((uint32_t)g & 1u) << 8);
+            if (g + 1 < n_groups && lane < 16) cp_async16(rec_n + (uint32_t)lane * 16u, rec_g + lane);
+            cp_async_commit();
+            {   // register tile by head count (cos_compile.h): A = 4 x 6, B = 2 x 8, C = 1 x 12
                 const uint32_t th = q0.x & 7u;
-                if (th >= 3u) group_tile<4, 6, 3, FUSED>(rec, q0, c, close);
-                else if (th == 2u) group_tile<2, 12, 3, FUSED>(rec, q0, c, close);
-                else group_tile<1, 12, 4, FUSED>(rec, q0, c, close);
+                if (th >= 3u) group_tile<TILE_A_HEADS, TILE_A_COLS, COS_STAGES_A, FUSED>(rec, q0, c, close);
+                else if (th == 2u) group_tile<TILE_B_HEADS, TILE_B_COLS, COS_STAGES_B, FUSED>(rec, q0, c, close);
+                else group_tile<1, GROUP_MAX_COLS, COS_STAGES_C, FUSED>(rec, q0, c, close);
             }
-            rec = rec_n; q0 = q0_n;
+            cp_async_wait<0>();
+            __syncwarp();
+            rec = rec_n;
         }
         if (flags & FLAG_FRESH) {            // close-and-open: fresh head of every colour (Eq. 12, 70-71)
             // h0.w bit k: a row of this block has already stored its continuation into the fresh-head state of colour k
             // (the coalesced E2/E4 pair): add the closing sum to it
-            const uint4 fd = __ldg(bp + 1);
+            const uint4 fd = lds128u(bs + 16u);
 #pragma unroll
             for (int k = 0; k < 4; ++k) {
                 const uint32_t didx = k == 0 ? fd.x : k == 1 ? fd.y : k == 2 ? fd.z : fd.w;
@@ -288,8 +348,9 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
             const double scale = (double)(1u << h0.y);
             if (valid) a.out[(size_t)h0.z * (size_t)a.batch + (size_t)b] = (a.neg_kappa * close) * scale;
         }
-        mi = mi_n; bp = bp_n; h0 = h0_n;
+        mi = mi_n; bp = bp_n; pb ^= 1u;
     }
+    cp_async_wait<0>();
 }
 
 __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerArgs a)
@@ -330,7 +391,9 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
     if (a.pdl) asm volatile("griddepcontrol.wait;" ::: "memory");
     const uint32_t m_begin = blockIdx.y * a.masks_per_cta;
     const uint32_t m_end = min(a.n_masks, m_begin + a.masks_per_cta);
-    layer_blocks<false>(a, m_begin, m_end, tile, s_next, Gs, lane, valid, b);
+    const uint32_t rs_warp = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)(a.n_slots + a.nc * a.d) * (TILE * 8u) +
+                             (uint32_t)warp * RECORD_SLOT_BYTES;
+    layer_blocks<false>(a, m_begin, m_end, tile, s_next, gs_lane, rs_warp, lane, valid, b);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -365,6 +428,8 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
         Gs[(f.n_slots + q) * TILE + lane] = Gs[((lam * f.d + e) * f.d + e) * TILE + lane];
     }
     __syncthreads();
+    const uint32_t rs_warp = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)(f.n_slots + f.nc * f.d) * (TILE * 8u) +
+                             (uint32_t)warp * RECORD_SLOT_BYTES;
     LayerArgs a;
     a.G = f.G; a.batch = f.batch; a.b0 = f.b0; a.out = f.out; a.d = f.d; a.nc = f.nc; a.n_slots = f.n_slots;
     a.has_shift = f.has_shift;
@@ -382,7 +447,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
         a.words = fl.words; a.mask_off = fl.mask_off; a.n_masks = fl.n_masks;
         a.X = (l & 1) ? slab1 : slab0; a.Y = (l & 1) ? slab0 : slab1;
         // slabs are addressed per tile already: tile index 0 inside layer_blocks
-        layer_blocks<true>(a, 0u, fl.n_masks, 0u, s_next, Gs, lane, valid, b);
+        layer_blocks<true>(a, 0u, fl.n_masks, 0u, s_next, gs_lane, rs_warp, lane, valid, b);
         __threadfence_block();
         __syncthreads();
         if (threadIdx.x == 0) s_next = 0u;
@@ -391,9 +456,9 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
 }
 
 // ------------------------------------------------------------------------------------------------------
-size_t layer_smem_bytes(int n_slots, int nc, int d)
+size_t layer_smem_bytes(int n_slots, int nc, int d, int warps_per_cta)
 {
-    return (size_t)(n_slots + nc * d) * TILE * sizeof(double);
+    return (size_t)(n_slots + nc * d) * TILE * sizeof(double) + (size_t)warps_per_cta * RECORD_SLOT_BYTES;
 }
 
 cudaError_t configure_layer_kernels()
@@ -409,11 +474,11 @@ cudaError_t configure_layer_kernels()
 cudaError_t pick_layer_shape(int nc, int d, int n_slots, int* warps_per_cta, int* ctas_per_sm)
 {
     static const int cand[6] = {4, 6, 8, 10, 12, 16};
-    const size_t smem = layer_smem_bytes(n_slots, nc, d);
-    if (smem > LAYER_SMEM_MAX) return cudaErrorInvalidConfiguration;
     int best_w = 0, best_total = 0, best_ctas = 0;
     for (int i = 0; i < 6; ++i) {
         if (cand[i] > MAX_WARPS) continue;
+        const size_t smem = layer_smem_bytes(n_slots, nc, d, cand[i]);
+        if (smem > LAYER_SMEM_MAX) continue;
         int nb = 0;
         cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)cos_layer_kernel, cand[i] * 32, smem);
         if (e != cudaSuccess) return e;
@@ -427,7 +492,7 @@ cudaError_t pick_layer_shape(int nc, int d, int n_slots, int* warps_per_cta, int
 cudaError_t layer_ctas_per_sm(int nc, int d, int n_slots, int warps_per_cta, int* ctas_per_sm)
 {
     return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, (const void*)cos_layer_kernel, warps_per_cta * 32,
-                                                         layer_smem_bytes(n_slots, nc, d));
+                                                         layer_smem_bytes(n_slots, nc, d, warps_per_cta));
 }
 
 cudaError_t launch_layer(const LayerArgs& a, uint32_t tiles, int warps_per_cta, cudaStream_t stream)
@@ -438,7 +503,7 @@ cudaError_t launch_layer(const LayerArgs& a, uint32_t tiles, int warps_per_cta, 
     const uint32_t chunks = (a.n_masks + a.masks_per_cta - 1) / a.masks_per_cta;
     if (chunks > 65535u) return cudaErrorInvalidConfiguration;
     dim3 grid(tiles, chunks, 1), block(32 * warps_per_cta, 1, 1);
-    const size_t smem = layer_smem_bytes(a.n_slots, a.nc, a.d);
+    const size_t smem = layer_smem_bytes(a.n_slots, a.nc, a.d, warps_per_cta);
     if (smem > LAYER_SMEM_MAX) return cudaErrorInvalidConfiguration;
     if (!a.pdl) {
         cos_layer_kernel<<<grid, block, smem, stream>>>(a);
@@ -457,7 +522,7 @@ cudaError_t launch_fused(const FusedArgs& f, uint32_t tiles, int warps_per_cta, 
 {
     if (tiles == 0) return cudaSuccess;
     if (warps_per_cta > MAX_WARPS) warps_per_cta = MAX_WARPS;
-    const size_t smem = layer_smem_bytes(f.n_slots, f.nc, f.d);
+    const size_t smem = layer_smem_bytes(f.n_slots, f.nc, f.d, warps_per_cta);
     if (smem > LAYER_SMEM_MAX) return cudaErrorInvalidConfiguration;
     cos_fused_kernel<<<tiles, 32 * warps_per_cta, smem, stream>>>(f);
     return cudaGetLastError();

@@ -31,8 +31,9 @@ struct LayerArgs {
 cudaError_t launch_layer(const LayerArgs& a, uint32_t tiles, int warps_per_cta, cudaStream_t stream);
 // Opt-in to > 48 KB dynamic shared memory (once per process): the per-layer and the fused kernel.
 cudaError_t configure_layer_kernels();
-// staged table + plain diagonal of one batch tile
-size_t layer_smem_bytes(int n_slots, int nc, int d);
+// staged table + plain diagonal of one batch tile + the warps' program-record slots
+static const uint32_t RECORD_SLOT_BYTES = 4 * 256;      // per warp: two block slots and two record slots of 256 bytes
+size_t layer_smem_bytes(int n_slots, int nc, int d, int warps_per_cta);
 cudaError_t pick_layer_shape(int nc, int d, int n_slots, int* warps_per_cta, int* ctas_per_sm);
 cudaError_t layer_ctas_per_sm(int nc, int d, int n_slots, int warps_per_cta, int* ctas_per_sm);
 
