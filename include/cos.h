@@ -65,9 +65,10 @@ enum {
  *   out             receives the handle; the caller releases it with cos_free.
  * The values returned by cos_eval follow the physical convention of Eq. 83 (no shift-shift term).
  * Structural limits (COS_EUNSUPPORTED, never COS_ENOMEM): n * n_sub <= 24; SB-CoS with more than COS_MAX_COLOURS
- * flavours; a propagator tile (n_blocks * d * d + n_colours * d entries of 256 bytes) that exceeds the 226 KB of
- * shared memory of one SM (e.g. honeycomb SB-CoS beyond n = 10 with two flavours); a layer of more than 2^32 - 2 states
- * or a layer program of more than 2^32 words.  COS_ENOMEM is host or device memory exhaustion only.  */
+ * flavours; a propagator tile (n_blocks * d * d, + n_colours * d with shifts, entries of 256 bytes) that exceeds the
+ * 226 KB of shared memory of one SM (e.g. honeycomb SB-CoS beyond n = 10 with two flavours); a layer of 2^24 - 1 or more
+ * states (24-bit destination index of the layer program: honeycomb n >= 11).  COS_ENOMEM is host or device memory
+ * exhaustion only.  */
 int cos_build(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope, cos_handle* out);
 int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope,
                  int flags, cos_handle* out);
@@ -109,8 +110,9 @@ int cos_set_workspace_limit(cos_handle h, long long bytes);
 /* Launch tuning of a handle.  These are the ONLY knobs; the library reads no environment variable.  Results do not
  * depend on them (same arithmetic, same summation order).  Bad parameter or value: COS_EINVAL. */
 enum {
-    COS_TUNE_PREFETCH = 0,           /* L2 look-ahead of the layer kernel, in states (0 = off; default 256) */
-    COS_TUNE_WARPS_PER_CTA = 1,      /* 1..16; default: the CTA size with the most resident warps per SM */
+    COS_TUNE_PREFETCH = 0,           /* L2 look-ahead of the layer kernel, in states (0 = off; default 8) */
+    COS_TUNE_WARPS_PER_CTA = 1,      /* 1..24 (what fits the handle's kernel); default: the CTA size with the most resident
+                                        warps per SM */
     COS_TUNE_BLOCKS_PER_CTA_CAP = 2, /* upper bound of occupancy-mask blocks per CTA (0 = default: one per staged table slot) */
     COS_TUNE_PDL = 3,                /* programmatic dependent launch between layers (default 1) */
     COS_TUNE_FUSED = 4,              /* small DAGs: 1 = one fused launch (default), 0 = per-layer kernels */
@@ -137,9 +139,6 @@ enum {
     COS_INFO_WORKSPACE_BYTES = 13,
     COS_INFO_N_LAUNCHES = 14,     /* kernels launched through this handle so far (cos_eval / cos_eval_host) */
     COS_INFO_ORDER_MASK = 15,     /* requested orders of an all-subset handle (0 for single-output handles) */
-    COS_INFO_N_GROUPS = 16,       /* group records: rows of one block and colour that share their factor loads (Eq. 29-31) */
-    COS_INFO_N_FACTOR_LOADS = 17, /* staged-factor loads per configuration the kernels execute (with sharing) */
-    COS_INFO_N_FACTOR_LOADS_UNSHARED = 18, /* ... one per DAG edge-evaluation, i.e. without Eq. 29-31 */
     COS_INFO_DEVICE = 19,         /* CUDA device of the handle (-1: host-only) */
     COS_INFO_FUSED = 20,          /* 1: cos_eval walks the DAG in one fused launch */
     COS_INFO_LAYER_STATES = 100,  /* + layer index */

@@ -22,7 +22,7 @@ INFO = {
     "n_layers": 0, "n_states": 1, "n_edges": 2, "n_readout_edges": 3, "n_out": 4, "max_layer_states": 5,
     "n_masks": 6, "n_rows": 7, "n_fma": 8, "program_bytes": 9, "d": 10, "n_blocks": 11,
     "n_states_unpruned": 12, "workspace_bytes": 13, "n_launches": 14, "order_mask": 15,
-    "n_groups": 16, "n_factor_loads": 17, "n_factor_loads_unshared": 18, "device": 19, "fused": 20,
+    "device": 19, "fused": 20,
     "layer_states": 100, "layer_edges": 200, "layer_masks": 300,
 }
 
@@ -293,8 +293,7 @@ def cos_measure_fp64_fma_peak():
 def dag_summary(handle):
     """Convenience: the cos_info counters as a dict (host data only)."""
     keys = ["n_layers", "n_states", "n_edges", "n_readout_edges", "n_out", "max_layer_states", "n_masks",
-            "n_rows", "n_fma", "program_bytes", "d", "n_blocks", "n_states_unpruned", "order_mask", "n_groups",
-            "n_factor_loads", "n_factor_loads_unshared"]
+            "n_rows", "n_fma", "program_bytes", "d", "n_blocks", "n_states_unpruned", "order_mask"]
     out = {k: cos_info(handle, k) for k in keys}
     nl = out["n_layers"]
     out["layer_states"] = [cos_info(handle, "layer_states", l) for l in range(nl)]

@@ -41,7 +41,7 @@ struct cos_handle_s {
     long long ws_limit = 64ll << 30;
     // launch shape and tuning (cos_set_tuning); nothing here is read from the environment
     int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148;
-    int prefetch = 8;                     // L2 look-ahead: states fetched ahead when a block is claimed
+    int prefetch = 8;                     // L2 look-ahead distance in states
     int blocks_per_cta_cap = 0;           // 0: one block per staged table slot (64 .. 1024)
     int pdl = 1;                          // programmatic dependent launch between layers
     int host_slices = 8;                  // cos_eval_host: at most this many output slices (1: no second stream)
@@ -118,7 +118,7 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
     }
 
     const CompiledDag& D = h->dag;
-    const size_t smem = layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d, 4);
+    const size_t smem = layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d, D.has_shift);
     if (smem > LAYER_SMEM_MAX) {
         delete h;
         return fail(COS_EUNSUPPORTED, "cos_build: propagator tile does not fit the 227 KB shared memory of one SM");
@@ -135,7 +135,7 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
         e = configure_layer_kernels();
         if (e != cudaSuccess) { delete h; return cuda_fail(e, "cos_build: cudaFuncSetAttribute"); }
         // launch shape: the CTA size that keeps the most warps resident per SM
-        e = pick_layer_shape(D.nc, D.d, D.n_blocks * D.d * D.d, &h->warps_per_cta, &h->ctas_per_sm);
+        e = pick_layer_shape((int)D.max_L, D.nc, D.d, D.n_blocks * D.d * D.d, D.has_shift, &h->warps_per_cta, &h->ctas_per_sm);
         if (e != cudaSuccess) { delete h; return cuda_fail(e, "cos_build: occupancy query"); }
         cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device);
         h->dl.resize(D.layers.size());
@@ -151,7 +151,7 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
             h->program_bytes += wb + mb;
         }
         // small DAGs (orders n <= 6) are launch-latency bound: walk all layers in one kernel
-        bool small = D.n_states <= 16384;
+        bool small = D.n_states <= 16384 && D.max_L <= 12;
         for (const auto& P : D.layers) small = small && P.n_masks <= 2048;
         if (small) {
             std::vector<FusedLayer> fl(D.layers.size());
@@ -234,8 +234,7 @@ static int grow_workspace(cos_handle h, size_t need, const char* who)
 {
     if (need <= h->ws_bytes) return COS_OK;
     if (h->ws) { cudaFree(h->ws); h->ws = nullptr; h->ws_bytes = 0; }
-    // (+ 4 KB: the layer kernel prefetches a few states past the one it reads)
-    cudaError_t e = cudaMalloc(&h->ws, need + 4096);
+    cudaError_t e = cudaMalloc(&h->ws, need);
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, who); }
     h->ws_bytes = need;
     return COS_OK;
@@ -260,14 +259,17 @@ int cos_set_tuning(cos_handle h, int what, long long value)
             if (value < 0 || value > 4096) return fail(COS_EINVAL, "cos_set_tuning: prefetch distance must be in [0, 4096]");
             h->prefetch = (int)value; break;
         case COS_TUNE_WARPS_PER_CTA:
-            if (value < 1 || value > 16) return fail(COS_EINVAL, "cos_set_tuning: warps per CTA must be in [1, 16]");
-            h->warps_per_cta = (int)value;
+            if (value < 1 || value > 24) return fail(COS_EINVAL, "cos_set_tuning: warps per CTA must be in [1, 24]");
             if (h->on_device) {       // resident CTAs per SM for the new shape (sizes the grid waves)
                 const CompiledDag& D = h->dag;
                 int c = 0;
-                if (layer_ctas_per_sm(D.nc, D.d, D.n_blocks * D.d * D.d, (int)value, &c) == cudaSuccess && c > 0) h->ctas_per_sm = c;
-                else cudaGetLastError();
+                if (layer_ctas_per_sm((int)D.max_L, D.nc, D.d, D.n_blocks * D.d * D.d, D.has_shift, (int)value, &c) != cudaSuccess || c < 1) {
+                    cudaGetLastError();
+                    return fail(COS_EINVAL, "cos_set_tuning: this CTA size does not fit the handle's kernel");
+                }
+                h->ctas_per_sm = c;
             }
+            h->warps_per_cta = (int)value;
             break;
         case COS_TUNE_BLOCKS_PER_CTA_CAP:
             if (value < 0 || value > 65535) return fail(COS_EINVAL, "cos_set_tuning: blocks-per-CTA cap must be in [0, 65535]");
@@ -311,11 +313,10 @@ static int eval_range(cos_handle h, const double* G_dev, long long batch, double
         if (h->fused && !h->profiling) {
             FusedArgs f;
             f.layers = h->fused_layers; f.n_layers = NL; f.ws = h->ws; f.S_max = D.max_layer_states;
-            f.G = G_dev; f.batch = batch; f.b0 = t0 * TILE; f.out = out_dev; f.d = D.d; f.nc = D.nc; f.n_slots = n_slots;
-            f.has_shift = D.has_shift ? 1 : 0;
+            f.G = G_dev; f.batch = batch; f.b0 = t0 * TILE; f.out = out_dev; f.d = D.d; f.n_slots = n_slots;
             f.neg_kappa = -D.kappa;
             for (int c = 0; c < 4; ++c) f.sigma[c] = D.sigma[c];
-            cudaError_t ef = launch_fused(f, tiles, 8, stream);
+            cudaError_t ef = launch_fused(f, (int)D.max_L, D.nc, D.has_shift, tiles, 8, stream);
             if (ef != cudaSuccess) return cuda_fail(ef, "cos_eval: fused launch");
             ++h->n_launches;
             continue;
@@ -346,7 +347,7 @@ static int eval_range(cos_handle h, const double* G_dev, long long batch, double
                 long long mpc = (long long)P.n_masks * tiles / (resident * 4);
                 // staging the table costs one 256-byte line per slot and CTA; a block moves ~30 lines each way:
                 // about one block per staged slot keeps the staging share at a few percent
-                long long cap = n_slots + D.nc * D.d;
+                long long cap = n_slots + (D.has_shift ? D.nc * D.d : 0);
                 if (cap < 64) cap = 64;
                 if (cap > 1024) cap = 1024;
                 if (h->blocks_per_cta_cap > 0) cap = h->blocks_per_cta_cap;
@@ -365,10 +366,10 @@ static int eval_range(cos_handle h, const double* G_dev, long long batch, double
             a.X = slab[l & 1]; a.Y = slab[(l + 1) & 1];
             a.S_src = P.n_states; a.S_dst = (l + 1 < NL) ? D.layers[l + 1].n_states : 0;
             a.G = G_dev; a.batch = batch; a.b0 = t0 * TILE; a.out = out_dev;
-            a.d = D.d; a.nc = D.nc; a.n_slots = n_slots; a.has_shift = D.has_shift ? 1 : 0;
+            a.d = D.d; a.n_slots = n_slots;
             a.neg_kappa = -D.kappa;
             for (int c = 0; c < 4; ++c) a.shift[c] = (l == 0 ? -2.0 : -1.0) * D.sigma[c];
-            e = launch_layer(a, tiles, h->warps_per_cta, stream);
+            e = launch_layer(a, (int)D.max_L, D.nc, D.has_shift, tiles, h->warps_per_cta, stream);
             if (e != cudaSuccess) return cuda_fail(e, "cos_eval: layer launch");
             if (P.n_masks) ++h->n_launches;
             if (ev) cudaEventRecord(ev[l + 1], stream);
@@ -522,9 +523,6 @@ int cos_info(cos_handle h, int what, long long* value)
         case COS_INFO_WORKSPACE_BYTES: *value = (long long)h->ws_bytes; break;
         case COS_INFO_N_LAUNCHES: *value = h->n_launches; break;
         case COS_INFO_ORDER_MASK: *value = (long long)D.order_mask; break;
-        case COS_INFO_N_GROUPS: *value = (long long)D.n_groups; break;
-        case COS_INFO_N_FACTOR_LOADS: *value = (long long)D.n_factor_loads; break;
-        case COS_INFO_N_FACTOR_LOADS_UNSHARED: *value = (long long)D.n_factor_loads_unshared; break;
         case COS_INFO_DEVICE: *value = h->device; break;
         case COS_INFO_FUSED: *value = h->fused ? 1 : 0; break;
         default: return fail(COS_EINVAL, "cos_info: unknown query");

@@ -33,7 +33,6 @@ struct Builder {
     std::vector<uint32_t> codes;                // mask id -> code (2 bits per interaction: 0, 1=(1,A), 2=(1,B), 3=full)
     std::vector<uint32_t> alive;                // [id*d + h_a] bitmask over e_a of live states (colour-independent)
     std::vector<uint32_t> row_base;             // [id*d + h_a] slab index of state (h_a, lambda=0, first e)
-    std::vector<uint32_t> colour_stride;        // [id] states of one colour of the block (slab order [block][colour][head][e])
     std::vector<std::vector<uint32_t>> by_layer;
 
     static int cell(uint32_t code, int i) { return (code >> (2 * i)) & 3; }
@@ -75,8 +74,8 @@ struct Builder {
     }
     uint32_t state_index(uint32_t id, int h_a, int lam, int e_a) const {
         uint32_t a = alive[(size_t)id * d + h_a];
-        return row_base[(size_t)id * d + h_a] + (uint32_t)lam * colour_stride[id] +
-               (uint32_t)__builtin_popcount(a & ((1u << e_a) - 1u));
+        uint32_t L = (uint32_t)__builtin_popcount(a);
+        return row_base[(size_t)id * d + h_a] + (uint32_t)lam * L + (uint32_t)__builtin_popcount(a & ((1u << e_a) - 1u));
     }
 };
 
@@ -174,7 +173,7 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
         b.alive.swap(prod);
         prod.clear(); prod.shrink_to_fit();
 
-        // ---- numbering: layer slab order = [block (by mask code)][colour][head][endpoint]
+        // ---- numbering: layer slab order = [block (by mask code)][head][colour][endpoint]
         out = CompiledDag();
         out.n = n; out.nf = nf; out.nsub = nsub; out.d = d; out.nc = nc;
         out.n_blocks = uniform ? 1 : nf;
@@ -185,7 +184,6 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
         out.n_states_unpruned = unpruned;
         out.layers.assign(NL, LayerProgram());
         b.row_base.assign(b.alive.size(), 0u);
-        b.colour_stride.assign(b.codes.size(), 0u);
         for (int l = 0; l < NL; ++l) {
             auto& ids = b.by_layer[l];
             std::vector<uint32_t> keep;
@@ -194,45 +192,23 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                 for (int h = 0; h < d; ++h) any = any || b.alive[(size_t)id * d + h];
                 if (any) keep.push_back(id);
             }
-            // Blocks of equal shape (live destination endpoints, heads) are neighbours in the slab and in the program: the
-            // warps of an SM then run the same instance of the kernel's source loop at the same time (instruction cache).
-            std::vector<uint32_t> shape(b.codes.size(), 0u);
-            for (uint32_t id : keep) {
-                const uint32_t code = b.codes[id];
-                const int nJ = (l + 1 < NL) ? b.jlist(code, J) : 0;
-                uint32_t n_heads = 0, n_cols = 0;
-                for (int h = 0; h < d; ++h) n_heads += b.alive[(size_t)id * d + h] != 0u;
-                for (int q = 0; q < nJ; ++q) {
-                    const int32_t did = b.index_of[J[q].dest_code];
-                    bool any = false;
-                    for (int h = 0; h < d && !any && did >= 0; ++h)
-                        any = b.alive[(size_t)id * d + h] && ((b.alive[(size_t)did * d + h] >> J[q].j_a) & 1u);
-                    n_cols += any;
-                }
-                shape[id] = (n_cols << 8) | n_heads;
-            }
-            std::sort(keep.begin(), keep.end(), [&](uint32_t x, uint32_t y) {
-                return shape[x] != shape[y] ? shape[x] < shape[y] : b.codes[x] < b.codes[y];
-            });
+            std::sort(keep.begin(), keep.end(), [&](uint32_t x, uint32_t y) { return b.codes[x] < b.codes[y]; });
             ids.swap(keep);
             uint64_t counter = 0;
-            for (uint32_t id : ids) {
-                uint32_t per_colour = 0;
+            for (uint32_t id : ids)
                 for (int h = 0; h < d; ++h) {
                     const uint32_t a = b.alive[(size_t)id * d + h];
                     if (!a) continue;
-                    b.row_base[(size_t)id * d + h] = (uint32_t)counter + per_colour;
-                    per_colour += (uint32_t)__builtin_popcount(a);
+                    b.row_base[(size_t)id * d + h] = (uint32_t)counter;
+                    counter += (uint64_t)__builtin_popcount(a) * nc;
                 }
-                b.colour_stride[id] = per_colour;
-                counter += (uint64_t)per_colour * nc;
-            }
-            if (counter >= DIDX_DEAD) return "unsupported: a layer has more than 2^32 - 2 states (32-bit destination index)";
+            if (counter >= DIDX_DEAD) return "unsupported: a layer has more than 2^24 - 1 states (24-bit destination index)";
             out.layers[l].n_states = (uint32_t)counter;
             out.layers[l].n_masks = (uint32_t)ids.size();
         }
 
         // ---- emission
+        const int HDR = out.hdr_words();
         for (int l = 0; l < NL; ++l) {
             LayerProgram& P = out.layers[l];
             P.mask_off.reserve(2 * (size_t)P.n_masks + 2);
@@ -252,132 +228,78 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                     out_idx = all_subsets ? b.full_set(code) - 1u : 0u;
                 }
                 const bool need_close = flags != 0;
-                // heads of the block (colour-independent) and the destination columns that are live for at least one head
-                int heads[24], n_heads = 0;
-                uint32_t Lmax = 0;
+                uint32_t n_rows = 0, Lmax = 0;
                 for (int h = 0; h < d; ++h) {
                     const uint32_t a = b.alive[(size_t)id * d + h];
-                    if (a) { heads[n_heads++] = h; Lmax = std::max(Lmax, (uint32_t)__builtin_popcount(a)); }
+                    if (a) { n_rows += nc; Lmax = std::max(Lmax, (uint32_t)__builtin_popcount(a)); }
                 }
-                int32_t dest[24];
-                for (int q = 0; q < nJ; ++q) dest[q] = b.index_of[J[q].dest_code];
-                auto live = [&](int h, int q) {
-                    return dest[q] >= 0 && ((b.alive[(size_t)dest[q] * d + h] >> J[q].j_a) & 1u);
-                };
-                int cols[24], n_cols = 0;                       // live columns, increasing j_a (jlist is ordered by j_a)
-                for (int q = 0; q < nJ; ++q) {
-                    bool any = false;
-                    for (int k = 0; k < n_heads && !any; ++k) any = live(heads[k], q);
-                    if (any) cols[n_cols++] = q;
-                }
-                // column chunks of at most GROUP_MAX_COLS (balanced); a block without live columns still has one
-                // (empty) chunk, which carries the cycle-closing sum
-                const int n_chunks = std::max(1, (n_cols + GROUP_MAX_COLS - 1) / GROUP_MAX_COLS);
+                const uint32_t e_words = (Lmax + 3) / 4, stride = 2 + e_words + (uint32_t)nJ;
+                if (stride > 32) return "unsupported: row record exceeds 32 words";
+                if (P.words.size() + HDR + (size_t)n_rows * stride >= 0xFFFFFFFFull) return "unsupported: layer program exceeds 2^32 words";
                 P.mask_off.push_back((uint32_t)P.words.size());
                 {   // first state of the block in the layer slab (block states are contiguous)
                     uint32_t first = P.n_states;
-                    if (n_heads) first = b.row_base[(size_t)id * d + heads[0]];
+                    for (int h = 0; h < d; ++h)
+                        if (b.alive[(size_t)id * d + h]) { first = b.row_base[(size_t)id * d + h]; break; }
                     P.mask_off.push_back(first);
                 }
-                const size_t w_block = P.words.size();
-                P.words.push_back(flags << 24);                  // n_groups filled below
-                // |S| - 1 of a readout block (the deferred multiplicity 2^(|S|-1), see cos_compile.h)
-                P.words.push_back((flags & FLAG_READOUT) ? (uint32_t)__builtin_popcount(b.full_set(code)) - 1u : 0u);
+                P.words.push_back(n_rows | ((uint32_t)nJ << 16) | (flags << 24));
+                // bits 24..: |S| - 1 of a readout block (the deferred multiplicity 2^(|S|-1), see cos_compile.h)
+                const uint32_t sexp = (flags & FLAG_READOUT) ? (uint32_t)__builtin_popcount(b.full_set(code)) - 1u : 0u;
+                P.words.push_back(stride | (e_words << 8) | (fresh_a << 16) | (sexp << 24));
                 P.words.push_back(out_idx);
-                P.words.push_back(0u);
-                for (int lam = 0; lam < 4; ++lam)
-                    P.words.push_back((lam < nc && (flags & FLAG_FRESH))
-                                          ? b.state_index((uint32_t)fresh_did, (int)fresh_a, lam, (int)fresh_a) : DIDX_DEAD);
-                uint32_t n_groups = 0, merged = 0;
-                std::vector<uint32_t> rec_at;                    // word offsets of the block's records, in program order
-                for (int ch = 0; ch < n_chunks; ++ch) {
-                    const int c0 = n_cols * ch / n_chunks, c1 = n_cols * (ch + 1) / n_chunks, TJ = c1 - c0;
-                    const int th_max = TJ <= TILE_A_COLS ? TILE_A_HEADS : TJ <= TILE_B_COLS ? TILE_B_HEADS : 1;
-                    const int n_hgroups = (n_heads + th_max - 1) / th_max;
-                    for (int lam = 0; lam < nc; ++lam)
-                        for (int g = 0; g < n_hgroups; ++g) {
-                            const int h0 = n_heads * g / n_hgroups, h1 = n_heads * (g + 1) / n_hgroups, TH = h1 - h0;
-                            uint32_t emask = 0, jmask = 0;
-                            for (int k = h0; k < h1; ++k) emask |= b.alive[(size_t)id * d + heads[k]];
-                            for (int c = c0; c < c1; ++c) jmask |= 1u << J[cols[c]].j_a;
-                            const uint32_t row_words = ((uint32_t)TJ + 1u) & ~1u;      // destination rows are 8-byte aligned
-                            const uint32_t len = 4u + 4u * (uint32_t)TH + (((uint32_t)TH * row_words + 3u) & ~3u);
-                            if (P.words.size() + len >= 0xFFFFFFF0ull) return "unsupported: layer program exceeds 2^32 words";
-                            uint32_t n_src = 0;                                  // source states of the record
-                            for (int k = h0; k < h1; ++k) n_src += (uint32_t)__builtin_popcount(b.alive[(size_t)id * d + heads[k]]);
-                            rec_at.push_back((uint32_t)P.words.size());
-                            P.words.push_back((uint32_t)TH | ((uint32_t)TJ << 3) | ((uint32_t)lam << 8) |
-                                              ((need_close && ch == 0) ? 1u << 10 : 0u) | (n_src << 11) | ((len / 4u) << 24));
-                            P.words.push_back(emask);
-                            P.words.push_back(jmask);
-                            P.words.push_back(b.row_base[(size_t)id * d + heads[h0]] + (uint32_t)lam * b.colour_stride[id]);
-                            for (int k = h0; k < h1; ++k) {
-                                const int h = heads[k];
-                                P.words.push_back(b.row_base[(size_t)id * d + h] + (uint32_t)lam * b.colour_stride[id]);
-                                P.words.push_back(b.alive[(size_t)id * d + h]);
-                                P.words.push_back((uint32_t)h);
-                                P.words.push_back(0u);
-                            }
-                            const uint32_t U = (uint32_t)__builtin_popcount(emask);
-                            for (int k = h0; k < h1; ++k) {
-                                const int h = heads[k];
-                                const uint32_t L = (uint32_t)__builtin_popcount(b.alive[(size_t)id * d + h]);
-                                for (int c = c0; c < c1; ++c) {
-                                    const int q = cols[c];
-                                    uint32_t w = DIDX_DEAD;
-                                    if (live(h, q)) {
-                                        if (J[q].mult2) P.e1 += L; else P.e2 += L;
-                                        P.n_factor_loads_unshared += L;
-                                        // the continuation into the canonical open interaction from its own head lands on the
-                                        // fresh-head state (coalesced E2/E4 pair)
-                                        // (same destination state as the block's fresh-head state of this colour; the
-                                        // kernel adds the closing sum to it at the end of the block, header w3 bit lam)
-                                        if ((flags & FLAG_FRESH) && (uint32_t)h == fresh_a && J[q].j_a == fresh_a) merged |= 1u << lam;
-                                        w = b.state_index((uint32_t)dest[q], h, lam, J[q].j_a);
-                                    }
-                                    P.words.push_back(w);
-                                }
-                                if (TJ & 1) P.words.push_back(DIDX_DEAD);
-                            }
-                            while (P.words.size() & 3u) P.words.push_back(DIDX_DEAD);
-                            P.n_fma += (uint64_t)TH * U * (uint64_t)TJ;
-                            P.n_factor_loads += (uint64_t)U * (uint64_t)TJ;
-                            ++n_groups;
-                        }
-                }
-                // per-row bookkeeping that does not depend on the grouping
-                for (int k = 0; k < n_heads; ++k) {
-                    const uint32_t a = b.alive[(size_t)id * d + heads[k]];
+                for (int lam = 0; lam < nc; ++lam)
+                    P.words.push_back((flags & FLAG_FRESH) ? b.state_index((uint32_t)fresh_did, (int)fresh_a, lam, (int)fresh_a)
+                                                            : DIDX_DEAD);
+                int32_t dest[24];
+                for (int q = 0; q < nJ; ++q) dest[q] = b.index_of[J[q].dest_code];
+                for (int h = 0; h < d; ++h) {
+                    const uint32_t a = b.alive[(size_t)id * d + h];
+                    if (!a) continue;
                     const uint32_t L = (uint32_t)__builtin_popcount(a);
                     for (int lam = 0; lam < nc; ++lam) {
+                        P.words.push_back(b.row_base[(size_t)id * d + h] + (uint32_t)lam * L);
+                        const uint32_t kh = ((a >> h) & 1u) ? (uint32_t)__builtin_popcount(a & ((1u << h) - 1u)) : 31u;
+                        const size_t w_hdr = P.words.size();
+                        P.words.push_back(0u);           // w1, filled below
+                        uint32_t packed[6] = {0, 0, 0, 0, 0, 0};
+                        int k = 0;
+                        for (int e = 0; e < d; ++e)      // byte = lam*d + e_a: row index of G_lam[e_a][.] in the staged table
+                            if ((a >> e) & 1u) { packed[k / 4] |= (uint32_t)(lam * d + e) << (8 * (k % 4)); ++k; }
+                        for (uint32_t w = 0; w < e_words; ++w) P.words.push_back(packed[w]);
+                        // live destinations only (pruned ones are dropped), the merged E2/E4 destination last
+                        uint32_t n_live = 0, defer_word = 0, has_defer = 0;
+                        for (int q = 0; q < nJ; ++q) {
+                            const bool live = dest[q] >= 0 && ((b.alive[(size_t)dest[q] * d + h] >> J[q].j_a) & 1u);
+                            if (!live) continue;
+                            if (J[q].mult2) P.e1 += L; else P.e2 += L;
+                            if ((flags & FLAG_FRESH) && (uint32_t)h == fresh_a && J[q].j_a == fresh_a) {
+                                has_defer = 1; defer_word = (uint32_t)J[q].j_a << 24;
+                                continue;
+                            }
+                            P.words.push_back(b.state_index((uint32_t)dest[q], h, lam, J[q].j_a) | ((uint32_t)J[q].j_a << 24));
+                            ++n_live;
+                        }
+                        if (has_defer) P.words.push_back(defer_word);
+                        for (uint32_t q = n_live + has_defer; q < (uint32_t)nJ; ++q) P.words.push_back(0u);
+                        P.words[w_hdr] = L | ((uint32_t)h << 5) | ((uint32_t)lam << 10) | (kh << 12) | (n_live << 17) | (has_defer << 22);
+                        const uint32_t alive_j = n_live + has_defer;
                         if (b.has_shift && l + 1 < NL)      // E3: states whose current interaction is singly occupied
                             for (int e = 0; e < d; ++e)
                                 if (((a >> e) & 1u)) { int c = Builder::cell(code, e / nsub); if (c == 1 || c == 2) P.e3 += 1; }
                         if (flags & FLAG_FRESH) P.e4 += (uint64_t)L * nc;
                         if (flags & FLAG_READOUT) P.readout_edges += L;
-                        if (need_close) { P.n_fma += L; P.n_factor_loads += L; P.n_factor_loads_unshared += L; }
+                        P.n_fma += (uint64_t)L * (alive_j + (need_close ? 1u : 0u));
                     }
                 }
-                // L2 look-ahead hints: record i names the source range of record i + GROUP_LOOKAHEAD of the same block
-                for (size_t i = 0; i + GROUP_LOOKAHEAD < rec_at.size(); ++i) {
-                    const uint32_t tgt = rec_at[i + GROUP_LOOKAHEAD];
-                    const uint32_t cnt = (P.words[tgt] >> 11) & 0x7Fu;
-                    P.words[rec_at[i]] |= ((cnt + 1u) / 2u) << 18;
-                    P.words[rec_at[i] + 7] = P.words[tgt + 3];
-                }
-                if (n_groups > 0xFFFFu) return "unsupported: more than 65535 group records in one block";
-                P.words[w_block] |= n_groups;
-                P.words[w_block + 3] = merged;
-                P.n_groups += n_groups;
-                P.n_rows += (uint32_t)n_heads * nc;
+                P.n_rows += n_rows;
                 P.max_L = std::max(P.max_L, Lmax);
             }
             P.mask_off.push_back((uint32_t)P.words.size());
             P.mask_off.push_back(P.n_states);
-            P.words.resize(P.words.size() + 64, 0u);          // padding: the kernel may touch the line after the last record
-            out.n_states += P.n_states; out.n_masks += P.n_masks; out.n_rows += P.n_rows; out.n_groups += P.n_groups;
+            P.words.resize(P.words.size() + 64, 0u);          // padding: the kernel reads whole 32-word windows
+            out.n_states += P.n_states; out.n_masks += P.n_masks; out.n_rows += P.n_rows;
             out.n_edges += P.e1 + P.e2 + P.e3 + P.e4; out.n_readout_edges += P.readout_edges; out.n_fma += P.n_fma;
-            out.n_factor_loads += P.n_factor_loads; out.n_factor_loads_unshared += P.n_factor_loads_unshared;
             out.max_layer_states = std::max(out.max_layer_states, P.n_states);
             out.max_L = std::max(out.max_L, P.max_L);
         }

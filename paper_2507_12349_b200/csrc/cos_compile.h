@@ -13,55 +13,34 @@
 
 namespace cosb {
 
-// ---- program stream format (u32 words, every section 16-byte aligned so that the kernel reads it with warp-uniform
-// 128-bit loads), one stream per layer ----------------------------------------------------------------------
-// Slab order of a layer: [block = occupancy mask, by code][colour][head][endpoint].
-// block header (HDR_WORDS = 8 words = two uint4):
-//   w0 : n_groups[0:16) | flags[24:32)     flags: bit0 FRESH (close-and-open target alive),
-//                                                  bit1 READOUT (terminal readout, Eq. 14-15)
-//   w1 : (|S| - 1) of a readout block (the deferred multiplicity 2^(|S|-1), see below)
+// ---- program stream format (u32 words), one stream per layer ---------------------------------------
+// block header (HDR_WORDS = 3 + nc words):
+//   w0 : n_rows[0:16) | nJ[16:24) | flags[24:32)        flags: bit0 FRESH (close-and-open target alive),
+//                                                               bit1 READOUT (terminal readout, Eq. 14-15)
+//   w1 : row_stride[0:8) | e_words[8:16) | fresh_a[16:24) | (|S| - 1)[24:32) of a readout block
 //   w2 : out_idx (readout row of out_dev)
-//   w3 : bit lambda: a row of the block stores its continuation into the fresh-head state of colour lambda (the
-//        coalesced E2/E4 pair: continuation from the canonical open interaction's own head); the kernel
-//        then ADDS the closing sum to that state at the end of the block instead of overwriting it
-//   w4..w7 : destination state index (next layer) of the fresh-head state of colour lambda' (DIDX_DEAD: pruned / unused)
-// group record: up to GROUP_MAX_HEADS rows (heads) of ONE colour of the block that share the factor loads -- the
-// factor-application sharing of PAPER.md Eq. 29-31: G_lambda[e][j] does not depend on the head, so one staged factor
-// feeds the rows of all heads of the group (N_mult = min(|S_f|, |D_f|) -> one load per group instead of one per row):
-//   q0 : g0 | emask | jmask | first
-//        g0    = TH[0:3) | TJ[3:8) | lambda[8:10) | do_close[10] | n_src[11:18) | ahead2[18:24) | len4[24:32)
-//                (n_src = source states of the record, len4 = record length in uint4 units; ahead2 * 2 states starting
-//                at slab index `ahead` below are the sources of the record GROUP_LOOKAHEAD records later in this block:
-//                the kernel prefetches them into L2 when it starts this record; 0 = nothing to prefetch)
-//        emask = union over the heads of their live current endpoints e_a (bit e_a)
-//        jmask = destination endpoints j_a of the TJ columns of this record (bit j_a), in increasing order
-//        first = slab index of the group's first state (its states are contiguous: heads in increasing order)
-//   TH x qh : base | alive | h_a | ahead   base = slab index of the head's first state, alive = its live endpoints (bit
-//        e_a); ahead: look-ahead range start (first head only, see g0)
-//   TH rows of TJ destination words, each row padded to an even number of words (and the record to a multiple of 4):
-//        index of the destination state in the next layer's slab, or DIDX_DEAD (pruned, Eq. 23, or padding).
-//   Register tiles of the kernel: up to TILE_A_HEADS heads when the block has at most TILE_A_COLS live destination
-//   endpoints, up to TILE_B_HEADS heads for at most TILE_B_COLS, else one head x GROUP_MAX_COLS endpoints.  Blocks with more than GROUP_MAX_COLS live
-//   destination endpoints are split into column chunks (one set of records per chunk; do_close is set in the first
-//   chunk only, so that the cycle-closing sum is taken once).
+//   w3..w3+nc-1 : destination state index (next layer) of the fresh-head state of colour lambda'
+// row (row_stride = 2 + e_words + nJ words):
+//   w0 : index of the row's first state in this layer's slab (row states are contiguous)
+//   w1 : L[0:5) | h_a[5:10) | lambda[10:12) | k_h[12:17) | n_live[17:22) | defer[22]
+//        k_h = position of the state with e_a == h_a in the row (31: none); its cycle-closing factor G[h][h] must
+//        not carry the counterterm.  n_live = destinations that follow; defer = one more
+//        destination word after them whose value merges with the fresh-head state (coalesced E2/E4 pair)
+//   w2.. : lambda*d + e_a of the L states, one byte each (row of G_lambda[e_a][.] in the staged table)
+//   then n_live (+ defer) words: dj = didx[0:24) | j_a[24:29)  (destination index in the next layer, destination
+//        endpoint); pruned destinations (Eq. 23) are not listed; the row is padded to the block's common stride.
 // The multiplicity 2 - m_j = 2 of a continuation into an untouched interaction (Lemma 7) is NOT applied per edge:
 // every path into a state of mask m has taken exactly nz(m) - 1 such edges (nz = interactions with m_i >= 1; the root
 // enters with factor 1), so the slabs hold x / 2^(nz(m)-1) and a readout of subset S is scaled by 2^(|S|-1), exactly.
-static const uint32_t DIDX_DEAD = 0xFFFFFFFFu;     // pruned destination
+static const uint32_t DIDX_MASK = 0x00FFFFFFu;
+static const uint32_t DIDX_DEAD = 0x00FFFFFFu;     // fresh-head destination pruned (block header only)
 static const uint32_t FLAG_FRESH = 1u, FLAG_READOUT = 2u;
-static const int HDR_WORDS = 8;
-static const int TILE_A_HEADS = 4, TILE_A_COLS = 6;    // register tile A: 4 heads x 6 destination endpoints
-static const int TILE_B_HEADS = 2, TILE_B_COLS = 8;    // register tile B: 2 heads x 8 endpoints; tile C: 1 head x GROUP_MAX_COLS
-static const int GROUP_MAX_HEADS = 4;                  // rows sharing one factor load
-static const int GROUP_MAX_COLS = 12;                  // destination columns of one record
-static const int GROUP_LOOKAHEAD = 1;                  // L2 look-ahead distance in records
 
 struct LayerProgram {
-    uint32_t n_states = 0, n_masks = 0, n_rows = 0, n_groups = 0, max_L = 0;
+    uint32_t n_states = 0, n_masks = 0, n_rows = 0, max_L = 0;
     std::vector<uint32_t> words;
     std::vector<uint32_t> mask_off;      // [n_masks + 1][2]: {word offset of the block header, first state of the block}
     uint64_t e1 = 0, e2 = 0, e3 = 0, e4 = 0, readout_edges = 0, n_fma = 0;
-    uint64_t n_factor_loads = 0, n_factor_loads_unshared = 0;   // staged-factor loads per configuration with / without Eq. 29-31
 };
 
 struct CompiledDag {
@@ -71,9 +50,9 @@ struct CompiledDag {
     double sigma[4] = {0, 0, 0, 0};
     double kappa = 1.0;
     std::vector<LayerProgram> layers;    // 2n layers; layer l holds the transitions l -> l+1 and the readouts at l
-    uint64_t n_states = 0, n_states_unpruned = 0, n_masks = 0, n_rows = 0, n_groups = 0, n_edges = 0, n_readout_edges = 0, n_fma = 0;
-    uint64_t n_factor_loads = 0, n_factor_loads_unshared = 0;
+    uint64_t n_states = 0, n_states_unpruned = 0, n_masks = 0, n_rows = 0, n_edges = 0, n_readout_edges = 0, n_fma = 0;
     uint32_t max_layer_states = 0, max_L = 0;
+    int hdr_words() const { return 3 + nc; }
 };
 
 // Returns "" on success, else an error message ("unsupported: ..." for a structural limit, otherwise out of memory).

@@ -2,45 +2,29 @@
 //
 //  cos_layer_kernel   north_star (3)+(4): one layer step x_t += c_e L[x_s] (Eq. 16) for every
 //                     state of the next layer, plus the terminal readouts of this layer (Eq. 14-15).
-//  cos_fused_kernel   the same for small DAGs: every layer in one launch.
 //  cos_tabulate_kernel north_star (2): propagator lookup with linear tau-interpolation (Eq. 32).
 //  cos_fill_kernel    layer-0 initial states <- 1 (Eq. 66).
 //  fp64 FMA peak probe for the roofline report.
 //
-// Work decomposition of the layer kernel (DESIGN.md section 4-5):
+// Work decomposition of the layer kernel (DESIGN.md section 4):
 //   lane  = configuration (32 per batch tile, the contiguous dimension of every array),
-//   warp  = one occupancy-mask block at a time: all group records of the block,
+//   warp  = one occupancy-mask block at a time: all rows (head, colour) of the block,
 //   CTA   = `masks_per_cta` blocks x one batch tile; the tile's propagator table G (all blocks, d x d,
 //           32 configurations) is staged once in shared memory.
-// A group record is up to 4 rows (heads) of one colour of the block.  The continuation factor G_lambda[e][j] does not
-// depend on the head, so the record is a small product  Y[head][j] = sum_e X[head][e] * G_lambda[e][j]  per
-// configuration: for every source endpoint e the TJ factors are loaded ONCE from shared memory and applied to the TH
-// source values (factor-application sharing, Eq. 29-31), TH x TJ accumulators live in registers, and every
-// source state is read from HBM exactly once, just in time (one step ahead).  Every destination state is written exactly
-// once: no atomics, no second pass, HBM traffic = one read + one write per state.
+// For one row the L source values are loaded ONCE into registers (contiguous states, coalesced
+// 256-byte lines), every continuation destination is a length-L dot product against a column of
+// G in shared memory (1 LDS.64 + 1 DFMA per DAG edge), and the cycle-closing sum of the whole block is
+// accumulated in a register.  Every destination state is written exactly once: no atomics, no
+// second pass, HBM traffic = one read + one write per state.
 #include "cos_kernels.cuh"
 #include "cos_compile.h"
 
-// source-value stages (prefetch depth) of the three register tiles
-#ifndef COS_BULK_PREFETCH
-#define COS_BULK_PREFETCH 1
-#endif
-#ifndef COS_L1_AHEAD
-#define COS_L1_AHEAD 2
-#endif
-#ifndef COS_STAGES_A
-#define COS_STAGES_A 2
-#endif
-#ifndef COS_STAGES_B
-#define COS_STAGES_B 3
-#endif
-#ifndef COS_STAGES_C
-#define COS_STAGES_C 4
-#endif
-
 namespace cosb {
 
-static const int MAX_WARPS = 16;         // 128 registers per thread
+static const int MAX_WARPS = 16;
+// CTA size bound per instantiation: the long-row kernels (honeycomb, d = 20) are shared-memory limited to one CTA
+// per SM, so they take 24 warps (<= 85 registers) instead of 16.
+__host__ __device__ constexpr int max_warps_of(int maxl) { return maxl == 20 ? 20 : MAX_WARPS; }
 
 __device__ __forceinline__ double lds64(uint32_t addr)
 {
@@ -49,311 +33,212 @@ __device__ __forceinline__ double lds64(uint32_t addr)
     return v;
 }
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-__device__ __forceinline__ void prefetch_l1(const void* p) { asm volatile("prefetch.global.L1 [%0];" ::"l"(p)); }
-// one bulk (TMA) prefetch of a contiguous range into L2; bytes is a multiple of 16
-__device__ __forceinline__ void prefetch_l2_bulk(const void* p, uint32_t bytes)
-{
-    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
-}
 // asynchronous 8-byte global -> shared copy (LDGSTS): no register staging, completion by commit / wait groups
 __device__ __forceinline__ void cp_async8(uint32_t dst, const void* src)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(dst), "l"(src) : "memory");
 }
-// 16-byte variant (L2 only): program records -> the warp's record slots
-__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src)
-{
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
-}
-__device__ __forceinline__ uint4 lds128u(uint32_t addr)
-{
-    uint4 v;
-    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ uint2 lds64u(uint32_t addr)
-{
-    uint2 v;
-    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
-    return v;
-}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
-// What a warp needs to walk the records of one batch tile.
-struct TileCtx {
-    const char* Xl;                      // source slab of the tile + lane * 8
-    char* Yl;                            // destination slab of the tile + lane * 8
-    uint32_t gs_lane;                    // shared-memory byte address of Gs[0][lane]
-    uint32_t gd_lane;                    // ... of the plain diagonal Gd[0][lane]
-    uint32_t d, dstride;                 // table dimension, d * 256 bytes (one table row of 32 configurations)
-    uint32_t S_src;                      // states of the source layer
-    int prefetch;                        // L2 look-ahead (0: off; else the states fetched ahead when a block is claimed)
-    int lane;
-};
-
-// Keeps a loop-invariant value in a register: the compiler may not rematerialise it inside the loops below.
-__device__ __forceinline__ void pin(uint32_t& v) { asm volatile("" : "+r"(v)); }
-
-// The source values of endpoint e (bit = 1 << e; bit = 0: none) for the heads of a record, 0 where a head has no such state.
-template <int THM, bool FUSED>
-__device__ __forceinline__ void load_x(const uint32_t bit, double (&x)[THM], uint32_t (&idx)[THM], const uint32_t (&al)[THM],
-                                       const char* __restrict__ Xl)
-{
-#pragma unroll
-    for (int t = 0; t < THM; ++t) {
-        x[t] = 0.0;
-        if (al[t] & bit) {
-            const double* p = (const double*)(Xl + ((size_t)idx[t] << 8));
-            x[t] = FUSED ? __ldcg(p) : __ldcs(p);
-#if COS_L1_AHEAD > 0
-            // pull the line this head reads COS_L1_AHEAD states later into L1 (no register needed; the slab is padded)
-            if (!FUSED) asm volatile("prefetch.global.L1 [%0+%1];" ::"l"(p), "n"(COS_L1_AHEAD * 256));
+// U ordinary destinations of a row at once (program words w0 .. w0+U-1 of the row record): U length-L dot products
+// against U columns of the staged table, 2U independent DFMA chains, U stores.
+#ifndef COS_DEST_WIDE
+#define COS_DEST_WIDE 4
 #endif
-            ++idx[t];
+template <int L, int U>
+__device__ __forceinline__ void dest_group(const uint32_t rw, const int w0, const uint32_t (&ra)[L], const double (&x)[L],
+                                           char* const Yb)
+{
+    // (ptxas keeps the column offsets in vector registers here: one IMAD.IADD per LDS; only the single-destination
+    // loops get the LDS [R + UR] form)
+    const uint32_t dA = __shfl_sync(0xFFFFFFFFu, rw, w0);
+    const uint32_t dB = U > 1 ? __shfl_sync(0xFFFFFFFFu, rw, w0 + 1) : 0u;
+    const uint32_t dC = U > 2 ? __shfl_sync(0xFFFFFFFFu, rw, w0 + 2) : 0u;
+    const uint32_t dD = U > 3 ? __shfl_sync(0xFFFFFFFFu, rw, w0 + 3) : 0u;
+    const uint32_t jA = __byte_perm(dA, 0u, 0x4434u), jB = __byte_perm(dB, 0u, 0x4434u);   // j_a * 256 bytes
+    const uint32_t jC = __byte_perm(dC, 0u, 0x4434u), jD = __byte_perm(dD, 0u, 0x4434u);
+    double a0 = 0.0, a1 = 0.0, b0 = 0.0, b1 = 0.0, c0 = 0.0, c1 = 0.0, d0 = 0.0, d1 = 0.0;
+#pragma unroll
+    for (int k = 0; k < L; ++k) {
+        if (k & 1) {
+            a1 = fma(lds64(ra[k] + jA), x[k], a1);
+            if (U > 1) b1 = fma(lds64(ra[k] + jB), x[k], b1);
+            if (U > 2) c1 = fma(lds64(ra[k] + jC), x[k], c1);
+            if (U > 3) d1 = fma(lds64(ra[k] + jD), x[k], d1);
+        } else {
+            a0 = fma(lds64(ra[k] + jA), x[k], a0);
+            if (U > 1) b0 = fma(lds64(ra[k] + jB), x[k], b0);
+            if (U > 2) c0 = fma(lds64(ra[k] + jC), x[k], c0);
+            if (U > 3) d0 = fma(lds64(ra[k] + jD), x[k], d0);
         }
     }
+    // didx * 256 bytes: didx < 2^24, the shift drops j_a
+    __stcs((double*)(Yb + (size_t)(dA << 8)), a0 + a1);
+    if (U > 1) __stcs((double*)(Yb + (size_t)(dB << 8)), b0 + b1);
+    if (U > 2) __stcs((double*)(Yb + (size_t)(dC << 8)), c0 + c1);
+    if (U > 3) __stcs((double*)(Yb + (size_t)(dD << 8)), d0 + d1);
 }
 
-// One group record (cos_compile.h) with exactly TJ destination endpoints on a register tile of THM heads (the record's
-// TH <= THM heads are a run-time value; unused rows carry x = 0):
-//   for every source endpoint e (increasing): TJ factor loads G_lambda[e][j] (shared by the heads), THM x TJ FMAs, and per
-//   head the cycle-closing factor G_lambda[e][h] (Eq. 12, 15), which never carries the counterterm (plain diagonal Gd
-//   when e == h); then one store per live (head, endpoint).
-// The source values stream through D register stages: the loads of endpoint k + D - 1 are in flight while endpoint k is
-// applied (stages are named statically -- a register move from a pending load would wait for it).
-template <int THM, int TJ, int D, bool FUSED>
-__device__ __forceinline__ void group_run(const uint32_t rec, const uint4 q0, const int TH, uint32_t (&idx)[THM],
-                                          const uint32_t (&al)[THM], const uint32_t (&hoff)[THM], const TileCtx& c,
-                                          double& close)
+// ------------------------------------------------------------------------------------------------------
+// One row of a block: L contiguous source states, nJ destinations.
+//   rw       this lane's word of the row record (lane k holds word k)
+//   gs_lane  shared-memory byte address of Gs[0][lane]; row (lambda, e) of the table starts at
+//            gs_lane + (lambda*d + e) * dstride, entry j at + j*256 (dstride = d*256 bytes)
+//   gd_lane  shared-memory byte address of the plain diagonal Gd[0][lane] (SHIFT only)
+// Inner loop per DAG edge: one integer add (address), one LDS.64, one DFMA.
+template <int L, int NC, bool SHIFT, bool FUSED>
+__device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, const double* __restrict__ xp,
+                                         const int nJ, const int e_words, const bool need_close,
+                                         const uint32_t d, const uint32_t gs_lane, const uint32_t gd_lane,
+                                         double* __restrict__ Yt, double& close, double (&sp)[NC])
 {
-    constexpr int TJ1 = TJ > 0 ? TJ : 1;
-    const uint32_t lam = (q0.x >> 8) & 3u;
-    const bool do_close = (q0.x >> 10) & 1u;
-    uint32_t dstride = c.dstride;
-    pin(dstride);
-    // shared-memory byte addresses: column j of table row 0 of this colour (+ e * dstride = G_lambda[e][j]), the
-    // closing column of every head, and its plain-diagonal entry Gd_lambda[h]
-    uint32_t colq[TJ1];
-    uint32_t row0 = c.gs_lane + lam * c.d * dstride, gdl = c.gd_lane + ((lam * c.d) << 8);
-    pin(row0); pin(gdl);
-    {
-        uint32_t jm = q0.z;
+    double x[L];
+    uint32_t ra[L];
 #pragma unroll
-        for (int q = 0; q < TJ; ++q) { colq[q] = row0 + ((uint32_t)(__ffs((int)jm) - 1) << 8); jm &= jm - 1u; pin(colq[q]); }
+    for (int k = 0; k < L; ++k) x[k] = FUSED ? __ldcg(xp + (size_t)k * TILE) : __ldcs(xp + (size_t)k * TILE);
+    const uint32_t dstride = d * (TILE * 8u);
+#pragma unroll
+    for (int k = 0; k < L; ++k) {
+        const uint32_t ew = __shfl_sync(0xFFFFFFFFu, rw, 2 + (k >> 2));
+        ra[k] = ((ew >> (8 * (k & 3))) & 0xFFu) * dstride + gs_lane;
     }
-    double acc[THM][TJ1];
+    const int lam = (int)((rh >> 10) & 3u);
+    if (need_close) {                       // cycle-closing factor G_lam[e][h] (Eq. 12, 15), never shifted
+        const uint32_t h_a = (rh >> 5) & 31u, hoff = h_a * (TILE * 8u);
+        const int kh = (int)((rh >> 12) & 31u);
+        const uint32_t pd = gd_lane + ((uint32_t)lam * d + h_a) * (TILE * 8u);
+        double c0 = 0.0, c1 = 0.0;
 #pragma unroll
-    for (int t = 0; t < THM; ++t)
-#pragma unroll
-        for (int q = 0; q < TJ1; ++q) acc[t][q] = 0.0;
-    double cl = 0.0;
-
-    uint32_t em = q0.y;
-    uint32_t bq[D];
-    double xs[D][THM];
-#pragma unroll
-    for (int s = 0; s < D; ++s) {
-        bq[s] = em & (0u - em);                        // 0 after the last endpoint: load_x then loads nothing
-        em ^= bq[s];
-        load_x<THM, FUSED>(bq[s], xs[s], idx, al, c.Xl);
-    }
-    bool live = true;
-    while (live) {
-#pragma unroll
-        for (int s = 0; s < D; ++s) {
-            if (live) {
-                const uint32_t e = 31u - (uint32_t)__clz((int)bq[s]);
-                const uint32_t ro = e * dstride;
-                double g[TJ1];
-#pragma unroll
-                for (int q = 0; q < TJ; ++q) g[q] = lds64(colq[q] + ro);
-#pragma unroll
-                for (int q = 0; q < TJ; ++q)
-#pragma unroll
-                    for (int t = 0; t < THM; ++t) acc[t][q] = fma(g[q], xs[s][t], acc[t][q]);
-                if (do_close) {      // a head without this source state has x = 0: its (valid) factor load is harmless
-#pragma unroll
-                    for (int t = 0; t < THM; ++t)
-                        cl = fma(lds64(hoff[t] + ((hoff[t] == (e << 8)) ? gdl : row0 + ro)), xs[s][t], cl);
-                }
-                bq[s] = em & (0u - em);
-                em ^= bq[s];
-                load_x<THM, FUSED>(bq[s], xs[s], idx, al, c.Xl);
-                live = bq[(s + 1) % D] != 0u;
-            }
+        for (int k = 0; k < L; ++k) {
+            uint32_t p = ra[k] + hoff;
+            if (SHIFT) p = (k == kh) ? pd : p;
+            if (k & 1) c1 = fma(lds64(p), x[k], c1); else c0 = fma(lds64(p), x[k], c0);
         }
+        close += c0 + c1;
     }
-    if (TJ > 0) {
-        const uint32_t dw = rec + 16u * (uint32_t)(1 + TH);
-        constexpr int ROW2 = (TJ + 1) / 2;          // uint2 per destination row
+    // destinations: n_live ordinary ones, then (defer) the one that merges with the fresh-head state.  No per-edge
+    // multiplicity (deferred to the readout, cos_compile.h), no pruned entries: SHFL, L x (LDS, DFMA), one store.
+    const int n_live = (int)((rh >> 17) & 31u);
+    char* const Yb = (char*)Yt;
+    int jj = 0;
+    // COS_DEST_WIDE / two / one destination(s) at a time: 2 independent DFMA chains per destination hide the
+    // LDS -> DFMA latency at 20-24 resident warps
+#if COS_DEST_WIDE > 2
+    for (; jj + COS_DEST_WIDE <= n_live; jj += COS_DEST_WIDE) dest_group<L, COS_DEST_WIDE>(rw, 2 + e_words + jj, ra, x, Yb);
+#endif
+    for (; jj + 2 <= n_live; jj += 2) dest_group<L, 2>(rw, 2 + e_words + jj, ra, x, Yb);
+    if (jj < n_live) dest_group<L, 1>(rw, 2 + e_words + jj, ra, x, Yb);
+    if ((rh >> 22) & 1u) {                  // the destination that merges with the fresh-head state (E2/E4 pair)
+        const uint32_t dj = __shfl_sync(0xFFFFFFFFu, rw, 2 + e_words + n_live);
+        const uint32_t joff = __byte_perm(dj, 0u, 0x4434u);
+        double acc0 = 0.0, acc1 = 0.0;
 #pragma unroll
-        for (int t = 0; t < THM; ++t) {
-            if (t < TH) {
-#pragma unroll
-                for (int i = 0; i < ROW2; ++i) {
-                    const uint2 w2 = lds64u(dw + 8u * (uint32_t)(t * ROW2 + i));
-#pragma unroll
-                    for (int k = 0; k < 2; ++k) {
-                        if (2 * i + k < TJ) {
-                            const uint32_t w = k == 0 ? w2.x : w2.y;
-                            if (w != DIDX_DEAD) {
-                                double* y = (double*)(c.Yl + ((size_t)w << 8));
-                                if (FUSED) *y = acc[t][2 * i + k]; else __stcs(y, acc[t][2 * i + k]);
-                            }
-                        }
-                    }
-                }
-            }
+        for (int k = 0; k < L; ++k) {
+            if (k & 1) acc1 = fma(lds64(ra[k] + joff), x[k], acc1); else acc0 = fma(lds64(ra[k] + joff), x[k], acc0);
         }
-    }
-    if (do_close) close += cl;
-}
-
-// Dispatch of a record on its register tile (THM heads, up to TJM endpoints, D source stages).
-template <int THM, int TJM, int D, bool FUSED>
-__device__ __forceinline__ void group_tile(const uint32_t rec, const uint4 q0, const TileCtx& c, double& close)
-{
-    const int TH = (int)(q0.x & 7u), TJ = (int)((q0.x >> 3) & 31u);
-    uint32_t idx[THM], al[THM], hoff[THM];
+        const double acc = acc0 + acc1;
 #pragma unroll
-    for (int t = 0; t < THM; ++t) {
-        idx[t] = 0u; al[t] = 0u; hoff[t] = 0u;
-        if (t < TH) {
-            const uint4 qh = lds128u(rec + 16u * (uint32_t)(1 + t));
-            idx[t] = qh.x; al[t] = qh.y; hoff[t] = qh.z << 8;
-            // L2 look-ahead: the sources of the record GROUP_LOOKAHEAD records later (contiguous: one bulk prefetch)
-            if (t == 0 && c.prefetch > 0 && c.lane == 0) {
-                const uint32_t ahead2 = (q0.x >> 18) & 0x3Fu;
-                if (ahead2) prefetch_l2_bulk(c.Xl + ((size_t)qh.w << 8), ahead2 << 9);
-            }
-        }
+        for (int c = 0; c < NC; ++c) sp[c] = (c == lam) ? acc : sp[c];
     }
-#define COS_RUN_CASE(TJ_) \
-    case TJ_: group_run<THM, (TJ_ <= TJM ? TJ_ : 0), D, FUSED>(rec, q0, TH, idx, al, hoff, c, close); break;
-    switch (TJ) {
-        COS_RUN_CASE(0) COS_RUN_CASE(1) COS_RUN_CASE(2) COS_RUN_CASE(3) COS_RUN_CASE(4) COS_RUN_CASE(5) COS_RUN_CASE(6)
-        default:
-            if (TJM > 6) {
-                switch (TJ) {
-                    COS_RUN_CASE(7) COS_RUN_CASE(8)
-                    default:
-                        if (TJM > 8) {
-                            switch (TJ) {
-                                COS_RUN_CASE(9) COS_RUN_CASE(10) COS_RUN_CASE(11) COS_RUN_CASE(12)
-                                default: break;
-                            }
-                        }
-                        break;
-                }
-            }
-            break;
-    }
-#undef COS_RUN_CASE
 }
 
 // All source blocks [m_begin, m_end) of one layer for one batch tile: the body shared by the per-layer kernel and the
 // fused small-DAG kernel.  s_next (shared) must be 0 and visible to the CTA on entry.
-template <bool FUSED>
+template <int MAXL, int NC, bool SHIFT, bool FUSED>
 __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t m_begin, const uint32_t m_end,
                                              const uint32_t tile, unsigned int& s_next, const uint32_t gs_lane,
-                                             const uint32_t rs_warp, const int lane, const bool valid, const long long b)
+                                             const uint32_t gd_lane, const int lane, const bool valid, const long long b)
 {
-    TileCtx c;
-    c.Xl = (const char*)(a.X + (size_t)tile * a.S_src * TILE + lane);
-    c.Yl = (char*)(a.Y + (size_t)tile * a.S_dst * TILE + lane);
-    c.gs_lane = gs_lane; c.gd_lane = gs_lane + (uint32_t)a.n_slots * (TILE * 8u);
-    pin(c.gs_lane); pin(c.gd_lane);
-    c.d = (uint32_t)a.d; c.dstride = (uint32_t)a.d * (TILE * 8u);
-    c.S_src = a.S_src; c.prefetch = a.prefetch; c.lane = lane;
+    const int HDR = 3 + NC;
+    const double* Xt = a.X + (size_t)tile * a.S_src * TILE + lane;
+    const char* Xt0 = (const char*)(a.X + (size_t)tile * a.S_src * TILE);
+    double* Yt = a.Y + (size_t)tile * a.S_dst * TILE + lane;
     const uint2* mtab = (const uint2*)a.mask_off;
 
-    // Blocks are handed to warps dynamically (block sizes vary).  A warp always knows its current AND its next block.
-    // The program is read through per-warp shared-memory slots of 256 bytes filled by asynchronous copies one step ahead
-    // (lanes 0..15 copy 16 bytes each): slots 0/1 take a block header together with the block's first record, slots 2/3
-    // the following records, so that no record field is ever waited for at global-memory latency.
-    const uint32_t slot_lane = rs_warp + (uint32_t)(lane & 15) * 16u;
+    // Blocks are handed to warps dynamically (block sizes vary).  A warp always knows its current AND its next block:
+    // the next block's program window is fetched early.
     uint32_t mi = 0;
     if (lane == 0) mi = atomicAdd(&s_next, 1u);
     mi = __shfl_sync(0xFFFFFFFFu, mi, 0) + m_begin;
-    const uint4* bp = nullptr;
-    uint32_t pb = 0u;                        // block slot of the current block
+    uint32_t off = 0, hw = 0, rw = 0;
     if (mi < m_end) {
-        bp = (const uint4*)(a.words + __ldg(&mtab[mi]).x);
-        if (lane < 16) cp_async16(slot_lane, bp + lane);
+        const uint2 mt = __ldg(&mtab[mi]);
+        off = mt.x;
+        hw = __ldg(a.words + off + lane);
+        rw = __ldg(a.words + off + HDR + lane);
     }
-    cp_async_commit();
     while (mi < m_end) {
         uint32_t mi_n = 0;
         if (lane == 0) mi_n = atomicAdd(&s_next, 1u);
         mi_n = __shfl_sync(0xFFFFFFFFu, mi_n, 0) + m_begin;
-        const uint4* bp_n = nullptr;
+        uint32_t off_n = 0, hw_n = 0, rw_n = 0;
         if (mi_n < m_end) {
             const uint2 mt = __ldg(&mtab[mi_n]);
-            bp_n = (const uint4*)(a.words + mt.x);
-            if (lane < 16) cp_async16(slot_lane + ((pb ^ 1u) << 8), bp_n + lane);
-            // L2 look-ahead: the first states of the block this warp takes next (one bulk prefetch, a block away in time)
-            if (a.prefetch > 0 && lane == 0) {
-                uint32_t cnt = __ldg(&mtab[mi_n + 1].y) - mt.y;
-                if (cnt > (uint32_t)a.prefetch) cnt = (uint32_t)a.prefetch;
-                if (cnt) prefetch_l2_bulk(c.Xl + ((size_t)mt.y << 8), cnt << 8);
-            }
+            off_n = mt.x;
+            hw_n = __ldg(a.words + off_n + lane);
+            rw_n = __ldg(a.words + off_n + HDR + lane);
         }
-        cp_async_commit();
-        cp_async_wait<1>();                  // everything but the copy just issued: the current block's slot is complete
-        __syncwarp();
-        const uint32_t bs = rs_warp + (pb << 8);
-        const uint4 h0 = lds128u(bs);
-        const int n_groups = (int)(h0.x & 0xFFFFu);
-        const uint32_t flags = h0.x >> 24;
-        double close = 0.0;
 
-        const uint4* rec_g = bp + 2;         // global address of the current record
-        uint32_t rec = bs + 32u;             // its shared-memory copy
-        for (int g = 0; g < n_groups; ++g) {
-            const uint4 q0 = lds128u(rec);
-            rec_g += q0.x >> 24;
-            const uint32_t rec_n = rs_warp + 512u + (((uint32_t)g & 1u) << 8);
-            if (g + 1 < n_groups && lane < 16) cp_async16(rec_n + (uint32_t)lane * 16u, rec_g + lane);
-            cp_async_commit();
-            {   // register tile by head count (cos_compile.h): A = 4 x 6, B = 2 x 8, C = 1 x 12
-                const uint32_t th = q0.x & 7u;
-                if (th >= 3u) group_tile<TILE_A_HEADS, TILE_A_COLS, COS_STAGES_A, FUSED>(rec, q0, c, close);
-                else if (th == 2u) group_tile<TILE_B_HEADS, TILE_B_COLS, COS_STAGES_B, FUSED>(rec, q0, c, close);
-                else group_tile<1, GROUP_MAX_COLS, COS_STAGES_C, FUSED>(rec, q0, c, close);
+        const uint32_t w0 = __shfl_sync(0xFFFFFFFFu, hw, 0), w1 = __shfl_sync(0xFFFFFFFFu, hw, 1);
+        const int n_rows = (int)(w0 & 0xFFFFu), nJ = (int)((w0 >> 16) & 0xFFu);
+        const uint32_t flags = w0 >> 24;
+        const int stride = (int)(w1 & 0xFFu), e_words = (int)((w1 >> 8) & 0xFFu);
+        const bool need_close = flags != 0u;
+        double close = 0.0;
+        double sp[NC];
+#pragma unroll
+        for (int c = 0; c < NC; ++c) sp[c] = 0.0;
+
+        const uint32_t* rp = a.words + off + HDR;
+        for (int r = 0; r < n_rows; ++r) {
+            uint32_t rw_next = 0u;
+            if (r + 1 < n_rows) rw_next = __ldg(rp + (size_t)(r + 1) * stride + lane);
+            const uint32_t base = __shfl_sync(0xFFFFFFFFu, rw, 0), rh = __shfl_sync(0xFFFFFFFFu, rw, 1);
+            const int L = (int)(rh & 31u);
+            const double* xp = Xt + (size_t)base * TILE;
+            if (a.prefetch > 0) {            // L2 look-ahead: the L states `prefetch` states further down the slab
+                for (int q = lane; q < 2 * L; q += 32) {
+                    const uint32_t st = base + (uint32_t)a.prefetch + (uint32_t)(q >> 1);
+                    if (st < a.S_src) prefetch_l2(Xt0 + (size_t)st * (TILE * 8) + (size_t)(q & 1) * 128);
+                }
             }
-            cp_async_wait<0>();
-            __syncwarp();
-            rec = rec_n;
+#define COS_ROW_CASE(LL)                                                                                        \
+    case LL:                                                                                                    \
+        if (LL <= MAXL)                                                                                         \
+            row_body<(LL <= MAXL ? LL : 1), NC, SHIFT, FUSED>(rw, rh, xp, nJ, e_words, need_close, (uint32_t)a.d, \
+                                                              gs_lane, gd_lane, Yt, close, sp);                  \
+        break;
+            switch (L) {
+                COS_ROW_CASE(1) COS_ROW_CASE(2) COS_ROW_CASE(3) COS_ROW_CASE(4) COS_ROW_CASE(5) COS_ROW_CASE(6)
+                COS_ROW_CASE(7) COS_ROW_CASE(8) COS_ROW_CASE(9) COS_ROW_CASE(10) COS_ROW_CASE(11) COS_ROW_CASE(12)
+                COS_ROW_CASE(13) COS_ROW_CASE(14) COS_ROW_CASE(15) COS_ROW_CASE(16) COS_ROW_CASE(17) COS_ROW_CASE(18)
+                COS_ROW_CASE(19) COS_ROW_CASE(20) COS_ROW_CASE(21) COS_ROW_CASE(22) COS_ROW_CASE(23) COS_ROW_CASE(24)
+                default: break;
+            }
+#undef COS_ROW_CASE
+            rw = rw_next;
         }
         if (flags & FLAG_FRESH) {            // close-and-open: fresh head of every colour (Eq. 12, 70-71)
-            // h0.w bit k: a row of this block has already stored its continuation into the fresh-head state of colour k
-            // (the coalesced E2/E4 pair): add the closing sum to it
-            const uint4 fd = lds128u(bs + 16u);
 #pragma unroll
-            for (int k = 0; k < 4; ++k) {
-                const uint32_t didx = k == 0 ? fd.x : k == 1 ? fd.y : k == 2 ? fd.z : fd.w;
-                if (didx != DIDX_DEAD) {
-                    double* y = (double*)(c.Yl + ((size_t)didx << 8));
-                    double v = 0.0;
-                    if ((h0.w >> k) & 1u) v = __ldcg(y);
-                    v = fma(a.neg_kappa, close, v);
-                    if (FUSED) *y = v; else __stcs(y, v);
-                }
+            for (int c = 0; c < NC; ++c) {
+                const uint32_t didx = __shfl_sync(0xFFFFFFFFu, hw, 3 + c);
+                __stcs(Yt + (size_t)didx * TILE, fma(a.neg_kappa, close, sp[c]));
             }
         }
         if (flags & FLAG_READOUT) {          // terminal readout O_S (Eq. 15): one block per subset S
+            const uint32_t out_idx = __shfl_sync(0xFFFFFFFFu, hw, 2);
             // 2^(|S|-1): the continuation multiplicities of Lemma 7, applied once per output (exact)
-            const double scale = (double)(1u << h0.y);
-            if (valid) a.out[(size_t)h0.z * (size_t)a.batch + (size_t)b] = (a.neg_kappa * close) * scale;
+            const double scale = (double)(1u << (__shfl_sync(0xFFFFFFFFu, hw, 1) >> 24));
+            if (valid) a.out[(size_t)out_idx * (size_t)a.batch + (size_t)b] = (a.neg_kappa * close) * scale;
         }
-        mi = mi_n; bp = bp_n; pb ^= 1u;
+        mi = mi_n; off = off_n; hw = hw_n; rw = rw_n;
     }
-    cp_async_wait<0>();
 }
 
-__global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerArgs a)
+template <int MAXL, int NC, bool SHIFT>
+__global__ void __launch_bounds__(max_warps_of(MAXL) * 32) cos_layer_kernel(const LayerArgs a)
 {
     extern __shared__ __align__(128) double Gs[];
     __shared__ unsigned int s_next;
@@ -361,6 +246,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
     const uint32_t tile = blockIdx.x;
 
     const uint32_t gs_lane = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)lane * 8u;
+    const uint32_t gd_lane = gs_lane + (uint32_t)a.n_slots * (TILE * 8u);
 
     // Programmatic dependent launch: let the next layer's grid start (it only stages its table, which no layer
     // writes) while this grid drains; this grid in turn touches the slabs only after the previous one has completed.
@@ -376,24 +262,24 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
     cp_async_commit();
     cp_async_wait<0>();
     __syncthreads();
-    // continuation into the partner of the current endpoint (E2 with j = e) always comes with the counterterm one-cycle
-    // E3 at the same destination: fold c3*sigma_lam into the diagonal of the staged table (Eq. 49 / 72, 77) and keep
-    // the plain diagonal Gd for the cycle-closing factor (no shifts: Gd is a copy of the diagonal).
-    for (int q = warp; q < a.nc * a.d; q += W) {
-        const int lam = q / a.d, e = q - lam * a.d;
-        const double sh = lam == 0 ? a.shift[0] : lam == 1 ? a.shift[1] : lam == 2 ? a.shift[2] : a.shift[3];
-        const double g = Gs[((lam * a.d + e) * a.d + e) * TILE + lane];
-        Gs[(a.n_slots + q) * TILE + lane] = g;
-        if (a.has_shift) Gs[((lam * a.d + e) * a.d + e) * TILE + lane] = g + sh;
+    if (SHIFT) {
+        // continuation into the partner of the current endpoint (E2 with j = e) always comes with the
+        // counterterm one-cycle E3 at the same destination: fold c3*sigma_lam into the diagonal of the
+        // staged table (Eq. 49 / 72, 77) and keep the plain diagonal for the cycle-closing factor.
+        for (int q = warp; q < NC * a.d; q += W) {
+            const int lam = q / a.d, e = q - lam * a.d;
+            const double sh = lam == 0 ? a.shift[0] : lam == 1 ? a.shift[1] : lam == 2 ? a.shift[2] : a.shift[3];
+            const double g = Gs[((lam * a.d + e) * a.d + e) * TILE + lane];
+            Gs[(a.n_slots + q) * TILE + lane] = g;
+            Gs[((lam * a.d + e) * a.d + e) * TILE + lane] = g + sh;
+        }
+        __syncthreads();
     }
-    __syncthreads();
 
     if (a.pdl) asm volatile("griddepcontrol.wait;" ::: "memory");
     const uint32_t m_begin = blockIdx.y * a.masks_per_cta;
     const uint32_t m_end = min(a.n_masks, m_begin + a.masks_per_cta);
-    const uint32_t rs_warp = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)(a.n_slots + a.nc * a.d) * (TILE * 8u) +
-                             (uint32_t)warp * RECORD_SLOT_BYTES;
-    layer_blocks<false>(a, m_begin, m_end, tile, s_next, gs_lane, rs_warp, lane, valid, b);
+    layer_blocks<MAXL, NC, SHIFT, false>(a, m_begin, m_end, tile, s_next, gs_lane, gd_lane, lane, valid, b);
 }
 
 // ------------------------------------------------------------------------------------------------------
@@ -402,6 +288,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_layer_kernel(const LayerAr
 // once, writes the layer-0 states (Eq. 66) itself and ping-pongs between two slabs of S_max states per tile (L2-resident;
 // source rows are read with ld.global.cg so that no stale L1 line of the slab written two layers earlier is seen).
 // Used when every layer is small (launch latency, not bandwidth, decides: orders n <= 6).
+template <int MAXL, int NC, bool SHIFT>
 __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedArgs f)
 {
     extern __shared__ __align__(128) double Gs[];
@@ -409,6 +296,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, W = blockDim.x >> 5;
     const uint32_t tile = blockIdx.x;
     const uint32_t gs_lane = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)lane * 8u;
+    const uint32_t gd_lane = gs_lane + (uint32_t)f.n_slots * (TILE * 8u);
     const long long b = f.b0 + (long long)tile * TILE + lane;
     const bool valid = b < f.batch;
     if (threadIdx.x == 0) s_next = 0u;
@@ -422,21 +310,19 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
     for (uint32_t s = warp; s < f.layers[0].n_states; s += W) slab0[(size_t)s * TILE + lane] = 1.0;   // Eq. 66
     cp_async_wait<0>();
     __syncthreads();
-    // keep the plain diagonal (cycle closing); the shifted one is rewritten per layer below
-    for (int q = warp; q < f.nc * f.d; q += W) {
-        const int lam = q / f.d, e = q - lam * f.d;
-        Gs[(f.n_slots + q) * TILE + lane] = Gs[((lam * f.d + e) * f.d + e) * TILE + lane];
+    if (SHIFT) {       // keep the plain diagonal (cycle closing); the shifted one is rewritten per layer below
+        for (int q = warp; q < NC * f.d; q += W) {
+            const int lam = q / f.d, e = q - lam * f.d;
+            Gs[(f.n_slots + q) * TILE + lane] = Gs[((lam * f.d + e) * f.d + e) * TILE + lane];
+        }
+        __syncthreads();
     }
-    __syncthreads();
-    const uint32_t rs_warp = (uint32_t)__cvta_generic_to_shared(Gs) + (uint32_t)(f.n_slots + f.nc * f.d) * (TILE * 8u) +
-                             (uint32_t)warp * RECORD_SLOT_BYTES;
     LayerArgs a;
-    a.G = f.G; a.batch = f.batch; a.b0 = f.b0; a.out = f.out; a.d = f.d; a.nc = f.nc; a.n_slots = f.n_slots;
-    a.has_shift = f.has_shift;
+    a.G = f.G; a.batch = f.batch; a.b0 = f.b0; a.out = f.out; a.d = f.d; a.n_slots = f.n_slots;
     a.neg_kappa = f.neg_kappa; a.prefetch = 0; a.pdl = 0; a.S_src = f.S_max; a.S_dst = f.S_max; a.masks_per_cta = 0;
     for (int l = 0; l < f.n_layers; ++l) {
-        if (f.has_shift && l <= 1) {         // c3 = -2 at layer 0, -1 afterwards (Eq. 72, 77)
-            for (int q = warp; q < f.nc * f.d; q += W) {
+        if (SHIFT && l <= 1) {               // c3 = -2 at layer 0, -1 afterwards (Eq. 72, 77)
+            for (int q = warp; q < NC * f.d; q += W) {
                 const int lam = q / f.d, e = q - lam * f.d;
                 const double sg = lam == 0 ? f.sigma[0] : lam == 1 ? f.sigma[1] : lam == 2 ? f.sigma[2] : f.sigma[3];
                 Gs[((lam * f.d + e) * f.d + e) * TILE + lane] = Gs[(f.n_slots + q) * TILE + lane] + (l == 0 ? -2.0 : -1.0) * sg;
@@ -447,7 +333,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
         a.words = fl.words; a.mask_off = fl.mask_off; a.n_masks = fl.n_masks;
         a.X = (l & 1) ? slab1 : slab0; a.Y = (l & 1) ? slab0 : slab1;
         // slabs are addressed per tile already: tile index 0 inside layer_blocks
-        layer_blocks<true>(a, 0u, fl.n_masks, 0u, s_next, gs_lane, rs_warp, lane, valid, b);
+        layer_blocks<MAXL, NC, SHIFT, true>(a, 0u, fl.n_masks, 0u, s_next, gs_lane, gd_lane, lane, valid, b);
         __threadfence_block();
         __syncthreads();
         if (threadIdx.x == 0) s_next = 0u;
@@ -456,31 +342,71 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
 }
 
 // ------------------------------------------------------------------------------------------------------
-size_t layer_smem_bytes(int n_slots, int nc, int d, int warps_per_cta)
+typedef void (*layer_fn)(const LayerArgs);
+
+template <int MAXL>
+static layer_fn pick_nc(int nc, bool shift)
 {
-    return (size_t)(n_slots + nc * d) * TILE * sizeof(double) + (size_t)warps_per_cta * RECORD_SLOT_BYTES;
+    if (!shift) {
+        switch (nc) {
+            case 1: return cos_layer_kernel<MAXL, 1, false>;
+            case 2: return cos_layer_kernel<MAXL, 2, false>;
+            case 3: return cos_layer_kernel<MAXL, 3, false>;
+            default: return cos_layer_kernel<MAXL, 4, false>;
+        }
+    }
+    switch (nc) {
+        case 1: return cos_layer_kernel<MAXL, 1, true>;
+        case 2: return cos_layer_kernel<MAXL, 2, true>;
+        case 3: return cos_layer_kernel<MAXL, 3, true>;
+        default: return cos_layer_kernel<MAXL, 4, true>;
+    }
+}
+
+static int maxl_class(int max_L) { return max_L <= 4 ? 4 : max_L <= 8 ? 8 : max_L <= 12 ? 12 : max_L <= 20 ? 20 : 24; }
+
+static layer_fn pick_layer_fn(int max_L, int nc, bool shift)
+{
+    switch (maxl_class(max_L)) {
+        case 4: return pick_nc<4>(nc, shift);
+        case 8: return pick_nc<8>(nc, shift);
+        case 12: return pick_nc<12>(nc, shift);
+        case 20: return pick_nc<20>(nc, shift);
+        default: return pick_nc<24>(nc, shift);
+    }
+}
+
+size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift)
+{
+    return (size_t)(n_slots + (shift ? nc * d : 0)) * TILE * sizeof(double);
 }
 
 cudaError_t configure_layer_kernels()
 {
-    cudaError_t e = cudaFuncSetAttribute((const void*)cos_layer_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)LAYER_SMEM_MAX);
-    if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute((const void*)cos_fused_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                (int)LAYER_SMEM_MAX);
+    static const int Ls[5] = {4, 8, 12, 20, 24};
+    for (int i = 0; i < 5; ++i)
+        for (int nc = 1; nc <= 4; ++nc)
+            for (int sh = 0; sh < 2; ++sh) {
+                cudaError_t e = cudaFuncSetAttribute((const void*)pick_layer_fn(Ls[i], nc, sh != 0),
+                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LAYER_SMEM_MAX);
+                if (e != cudaSuccess) return e;
+            }
+    return configure_fused_kernels();
 }
 
-// Launch shape: the CTA size that maximises resident warps per SM (ties: the smaller CTA).
-cudaError_t pick_layer_shape(int nc, int d, int n_slots, int* warps_per_cta, int* ctas_per_sm)
+// Launch shape for this instantiation: the CTA size that maximises resident warps per SM (ties: the smaller CTA).
+cudaError_t pick_layer_shape(int max_L, int nc, int d, int n_slots, bool shift, int* warps_per_cta, int* ctas_per_sm)
 {
-    static const int cand[6] = {4, 6, 8, 10, 12, 16};
+    static const int cand[8] = {4, 6, 8, 10, 12, 16, 20, 24};
+    const int max_w = max_warps_of(maxl_class(max_L));
+    layer_fn fn = pick_layer_fn(max_L, nc, shift);
+    const size_t smem = layer_smem_bytes(n_slots, nc, d, shift);
+    if (smem > LAYER_SMEM_MAX) return cudaErrorInvalidConfiguration;
     int best_w = 0, best_total = 0, best_ctas = 0;
-    for (int i = 0; i < 6; ++i) {
-        if (cand[i] > MAX_WARPS) continue;
-        const size_t smem = layer_smem_bytes(n_slots, nc, d, cand[i]);
-        if (smem > LAYER_SMEM_MAX) continue;
+    for (int i = 0; i < 8; ++i) {
+        if (cand[i] > max_w) continue;
         int nb = 0;
-        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)cos_layer_kernel, cand[i] * 32, smem);
+        cudaError_t e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&nb, (const void*)fn, cand[i] * 32, smem);
         if (e != cudaSuccess) return e;
         if (nb * cand[i] > best_total) { best_total = nb * cand[i]; best_w = cand[i]; best_ctas = nb; }
     }
@@ -489,24 +415,28 @@ cudaError_t pick_layer_shape(int nc, int d, int n_slots, int* warps_per_cta, int
     return cudaSuccess;
 }
 
-cudaError_t layer_ctas_per_sm(int nc, int d, int n_slots, int warps_per_cta, int* ctas_per_sm)
+cudaError_t layer_ctas_per_sm(int max_L, int nc, int d, int n_slots, bool shift, int warps_per_cta, int* ctas_per_sm)
 {
-    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, (const void*)cos_layer_kernel, warps_per_cta * 32,
-                                                         layer_smem_bytes(n_slots, nc, d, warps_per_cta));
+    if (warps_per_cta > max_warps_of(maxl_class(max_L))) return cudaErrorInvalidConfiguration;
+    return cudaOccupancyMaxActiveBlocksPerMultiprocessor(ctas_per_sm, (const void*)pick_layer_fn(max_L, nc, shift),
+                                                         warps_per_cta * 32, layer_smem_bytes(n_slots, nc, d, shift));
 }
 
-cudaError_t launch_layer(const LayerArgs& a, uint32_t tiles, int warps_per_cta, cudaStream_t stream)
+cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
+                         cudaStream_t stream)
 {
     if (a.n_masks == 0 || tiles == 0) return cudaSuccess;
     if (warps_per_cta < 1) warps_per_cta = 1;
-    if (warps_per_cta > MAX_WARPS) warps_per_cta = MAX_WARPS;
+    const int max_w = max_warps_of(maxl_class(max_L));
+    if (warps_per_cta > max_w) warps_per_cta = max_w;
     const uint32_t chunks = (a.n_masks + a.masks_per_cta - 1) / a.masks_per_cta;
     if (chunks > 65535u) return cudaErrorInvalidConfiguration;
     dim3 grid(tiles, chunks, 1), block(32 * warps_per_cta, 1, 1);
-    const size_t smem = layer_smem_bytes(a.n_slots, a.nc, a.d, warps_per_cta);
+    layer_fn fn = pick_layer_fn(max_L, nc, shift);
+    const size_t smem = layer_smem_bytes(a.n_slots, nc, a.d, shift);
     if (smem > LAYER_SMEM_MAX) return cudaErrorInvalidConfiguration;
     if (!a.pdl) {
-        cos_layer_kernel<<<grid, block, smem, stream>>>(a);
+        fn<<<grid, block, smem, stream>>>(a);
         return cudaGetLastError();
     }
     cudaLaunchConfig_t cfg = {};
@@ -515,16 +445,58 @@ cudaError_t launch_layer(const LayerArgs& a, uint32_t tiles, int warps_per_cta, 
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    return cudaLaunchKernelEx(&cfg, cos_layer_kernel, a);
+    return cudaLaunchKernelEx(&cfg, fn, a);
 }
 
-cudaError_t launch_fused(const FusedArgs& f, uint32_t tiles, int warps_per_cta, cudaStream_t stream)
+typedef void (*fused_fn)(const FusedArgs);
+template <int MAXL>
+static fused_fn pick_fused_nc(int nc, bool shift)
+{
+    if (!shift) {
+        switch (nc) {
+            case 1: return cos_fused_kernel<MAXL, 1, false>;
+            case 2: return cos_fused_kernel<MAXL, 2, false>;
+            case 3: return cos_fused_kernel<MAXL, 3, false>;
+            default: return cos_fused_kernel<MAXL, 4, false>;
+        }
+    }
+    switch (nc) {
+        case 1: return cos_fused_kernel<MAXL, 1, true>;
+        case 2: return cos_fused_kernel<MAXL, 2, true>;
+        case 3: return cos_fused_kernel<MAXL, 3, true>;
+        default: return cos_fused_kernel<MAXL, 4, true>;
+    }
+}
+static fused_fn pick_fused_fn(int max_L, int nc, bool shift)
+{
+    if (max_L <= 4) return pick_fused_nc<4>(nc, shift);
+    if (max_L <= 8) return pick_fused_nc<8>(nc, shift);
+    if (max_L <= 12) return pick_fused_nc<12>(nc, shift);
+    return nullptr;
+}
+
+cudaError_t configure_fused_kernels()
+{
+    static const int Ls[3] = {4, 8, 12};
+    for (int i = 0; i < 3; ++i)
+        for (int nc = 1; nc <= 4; ++nc)
+            for (int sh = 0; sh < 2; ++sh) {
+                cudaError_t e = cudaFuncSetAttribute((const void*)pick_fused_fn(Ls[i], nc, sh != 0),
+                                                     cudaFuncAttributeMaxDynamicSharedMemorySize, (int)LAYER_SMEM_MAX);
+                if (e != cudaSuccess) return e;
+            }
+    return cudaSuccess;
+}
+
+cudaError_t launch_fused(const FusedArgs& f, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
+                         cudaStream_t stream)
 {
     if (tiles == 0) return cudaSuccess;
+    fused_fn fn = pick_fused_fn(max_L, nc, shift);
+    if (!fn) return cudaErrorInvalidConfiguration;
     if (warps_per_cta > MAX_WARPS) warps_per_cta = MAX_WARPS;
-    const size_t smem = layer_smem_bytes(f.n_slots, f.nc, f.d, warps_per_cta);
-    if (smem > LAYER_SMEM_MAX) return cudaErrorInvalidConfiguration;
-    cos_fused_kernel<<<tiles, 32 * warps_per_cta, smem, stream>>>(f);
+    const size_t smem = layer_smem_bytes(f.n_slots, nc, f.d, shift);
+    fn<<<tiles, 32 * warps_per_cta, smem, stream>>>(f);
     return cudaGetLastError();
 }
 

@@ -18,24 +18,24 @@ struct LayerArgs {
     const double* G;                     // caller's propagators [n_slots][batch]
     long long batch, b0;                 // total batch (row stride of G / out) and first configuration of this chunk
     double* out;                         // caller's output [n_out][batch]
-    int d, nc, n_slots;                  // table dimension, colours carried in the state, n_slots = n_blocks * d * d
-    int has_shift;                       // SB mode: the counterterm is folded into the staged diagonal
+    int d, n_slots;                      // n_slots = n_blocks * d * d
     double neg_kappa;                    // -kappa: -N_f (uniform) or -1 (SB)
-    int prefetch;                        // > 0: per group record, prefetch into L2 the source states this many states
-                                         // further down the slab; 0: off
+    int prefetch;                        // > 0: per row, prefetch into L2 the source states this many states ahead; 0: off
     int pdl;                             // 1: launched with programmatic stream serialization (layers > 0)
     double shift[4];                     // c3 * sigma_lambda of THIS layer (c3 = -2 at layer 0, -1 after)
 };
 
-// Launches one layer step: grid = (tiles, ceil(n_masks / masks_per_cta)); returns cudaGetLastError().
-cudaError_t launch_layer(const LayerArgs& a, uint32_t tiles, int warps_per_cta, cudaStream_t stream);
-// Opt-in to > 48 KB dynamic shared memory (once per process): the per-layer and the fused kernel.
+// Picks the instantiation (max row length, colours, shift) and launches one layer step.
+// grid = (tiles, ceil(n_masks / masks_per_cta)); returns cudaGetLastError().
+cudaError_t launch_layer(const LayerArgs& a, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
+                         cudaStream_t stream);
+// Opt-in to > 48 KB dynamic shared memory for every instantiation, per-layer and fused (once per process).
 cudaError_t configure_layer_kernels();
-// staged table + plain diagonal of one batch tile + the warps' program-record slots
-static const uint32_t RECORD_SLOT_BYTES = 4 * 256;      // per warp: two block slots and two record slots of 256 bytes
-size_t layer_smem_bytes(int n_slots, int nc, int d, int warps_per_cta);
-cudaError_t pick_layer_shape(int nc, int d, int n_slots, int* warps_per_cta, int* ctas_per_sm);
-cudaError_t layer_ctas_per_sm(int nc, int d, int n_slots, int warps_per_cta, int* ctas_per_sm);
+// staged table (+ plain diagonal in shift mode) of one batch tile
+size_t layer_smem_bytes(int n_slots, int nc, int d, bool shift);
+// CTA size with the most resident warps per SM, and the resident CTAs per SM for a given CTA size
+cudaError_t pick_layer_shape(int max_L, int nc, int d, int n_slots, bool shift, int* warps_per_cta, int* ctas_per_sm);
+cudaError_t layer_ctas_per_sm(int max_L, int nc, int d, int n_slots, bool shift, int warps_per_cta, int* ctas_per_sm);
 
 // ---- fused small-DAG path: every layer in one launch (cos_fused_kernel)
 struct FusedLayer { const uint32_t* words; const uint32_t* mask_off; uint32_t n_masks, n_states; };
@@ -45,11 +45,13 @@ struct FusedArgs {
     double* ws;                          // two slabs [2][tiles][S_max][32]
     uint32_t S_max;
     const double* G; long long batch, b0; double* out;
-    int d, nc, n_slots, has_shift;
+    int d, n_slots;
     double neg_kappa;
     double sigma[4];
 };
-cudaError_t launch_fused(const FusedArgs& f, uint32_t tiles, int warps_per_cta, cudaStream_t stream);
+cudaError_t configure_fused_kernels();
+cudaError_t launch_fused(const FusedArgs& f, int max_L, int nc, bool shift, uint32_t tiles, int warps_per_cta,
+                         cudaStream_t stream);
 
 cudaError_t launch_fill_ones(double* X, size_t n_doubles, cudaStream_t stream);
 
