@@ -24,6 +24,26 @@ def draw_vertices(w, batch=None):
     return out
 
 
+def draw_clustered_vertices(w, batch=None, spread=1, tau_window=None):
+    """Stress input: the vertices of a configuration sit within +-`spread` sites of a random
+    centre and within a tau window of `tau_window` (default beta/50) around a random time -- the short-distance,
+    short-time clusters a sampler of the paper's kind visits, where the terms of the connected sum
+    cancel hardest.  Same layout as draw_vertices; seeded with w.seed + 7919."""
+    B = w.batch if batch is None else int(batch)
+    win = w.beta / 50.0 if tau_window is None else float(tau_window)
+    rng = np.random.default_rng(w.seed + 7919)
+    centre = rng.integers(0, w.L, size=(B, 1, 2))
+    sites = (centre + rng.integers(-spread, spread + 1, size=(B, w.n, 2))) % w.L
+    t0 = rng.random((B, 1)) * (w.beta - win)
+    tau = t0 + rng.random((B, w.n)) * win
+    out = {}
+    if w.lattice == 1:
+        out["sub"] = np.ascontiguousarray(rng.integers(0, 2, size=(B, w.n)).transpose(1, 0).astype(np.int32))
+    out["sites"] = np.ascontiguousarray(sites.transpose(1, 2, 0).astype(np.int32))
+    out["tau"] = np.ascontiguousarray(tau.transpose(1, 0).astype(np.float64))
+    return out
+
+
 def random_matrices(seed, n_blocks, d, batch, scale=1.0, diag=None):
     """Generic propagator blocks G[n_blocks][d][d][batch] ~ scale * N(0, 1) (unit tests).
     `diag` (float) overrides the diagonal, mimicking g(0, 0^-) = -rho."""

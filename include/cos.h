@@ -160,7 +160,9 @@ const char* cos_last_error(void);
  *   k = min(floor(u), n_tau-2), w = u-k.
  *   sites_dev   device int32 [n][2][batch]   lattice (square) or unit-cell (honeycomb) coordinates in [0,L)
  *   tau_dev     device fp64  [n][batch]      imaginary times in [0, beta)
- * Asynchronous on `stream`. */
+ * Times outside [0, beta) or non-finite times never cause an out-of-bounds table read: the node index is clamped to
+ * [0, n_tau-2] (the value is then a linear extrapolation, or NaN for a NaN time).  Sites are reduced modulo L.
+ * The current CUDA device must be the one the table was built on (COS_EINVAL otherwise).  Asynchronous on `stream`. */
 int cos_tab_build(int lattice, int L, int n_blocks, double beta, int n_tau, const double* table_host, cos_tab* out);
 int cos_tabulate(cos_tab tab, int n, const int* sites_dev, const double* tau_dev, long long batch,
                  double* G_dev, cos_stream stream);

@@ -64,6 +64,7 @@ struct cos_handle_s {
 
 struct cos_tab_s {
     double* T = nullptr;
+    int device = -1;
     int lattice = 0, L = 0, nsub = 1, n_blocks = 1, n_tau = 0;
     double beta = 0.0;
 };
@@ -541,6 +542,7 @@ int cos_tab_build(int lattice, int L, int n_blocks, double beta, int n_tau, cons
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) return fail(COS_ECUDA, "cos_tab_build: no CUDA device");
     cos_tab_s* t = new (std::nothrow) cos_tab_s();
     if (!t) return fail(COS_ENOMEM, "cos_tab_build: out of host memory");
+    cudaGetDevice(&t->device);
     t->lattice = lattice; t->L = L; t->nsub = lattice == COS_LATTICE_HONEYCOMB ? 2 : 1;
     t->n_blocks = n_blocks; t->n_tau = n_tau; t->beta = beta;
     const size_t bytes = (size_t)n_blocks * t->nsub * t->nsub * L * L * n_tau * sizeof(double);
@@ -557,6 +559,11 @@ int cos_tabulate(cos_tab tab, int n, const int* sites_dev, const double* tau_dev
     if (!tab || n < 1 || n > COS_MAX_N || batch < 0) return fail(COS_EINVAL, "cos_tabulate: bad argument");
     if (batch == 0) return COS_OK;
     if (!sites_dev || !tau_dev || !G_dev) return fail(COS_EINVAL, "cos_tabulate: NULL device pointer");
+    {
+        int dev = -1;
+        if (cudaGetDevice(&dev) != cudaSuccess || dev != tab->device)
+            return fail(COS_EINVAL, "cos_tabulate: the current CUDA device is not the one the table was built on");
+    }
     TabArgs a;
     a.T = tab->T; a.L = tab->L; a.nsub = tab->nsub; a.n_blocks = tab->n_blocks; a.n_tau = tab->n_tau; a.beta = tab->beta;
     a.n = n; a.sites = sites_dev; a.tau = tau_dev; a.batch = batch; a.G = G_dev;

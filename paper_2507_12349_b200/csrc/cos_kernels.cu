@@ -537,8 +537,11 @@ __global__ void cos_tabulate_kernel(const TabArgs a)
     if (dt <= 0.0) { dt = __dadd_rn(dt, a.beta); sign = -1.0; }      // anti-periodic; equal times use 0^-
     const double step = a.beta / (double)(a.n_tau - 1);
     const double u = __ddiv_rn(dt, step);
+    // tau outside [0, beta) or not finite: the node index is clamped to the table (no out-of-bounds read; the value is
+    // then an extrapolation or NaN, never a fault).  double -> int conversion saturates and maps NaN to 0.
     int k = (int)floor(u);
     if (k > a.n_tau - 2) k = a.n_tau - 2;
+    if (k < 0) k = 0;
     const double w = __dsub_rn(u, (double)k);
     const int d = a.n * a.nsub, ns2 = a.nsub * a.nsub;
     for (int blk = 0; blk < a.n_blocks; ++blk)

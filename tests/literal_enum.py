@@ -88,15 +88,37 @@ def typed_connected_sum(A, sigma, n_flavors, absolute=False, distinct_colours_on
     return total
 
 
-def uniform_connected_sum(A, n_flavors):
-    """sum over connected pi of sgn(pi) N_f^{#cycles} prod A."""
+def uniform_connected_sum(A, n_flavors, sigma=0.0, absolute=False):
+    """sum over connected pi of sgn(pi) N_f^{#cycles} prod A (Eq. 59).  With a counterterm (PAPER.md:431,
+    reading G12) a true one-cycle v -> v is either a normal loop, N_f A[v][v], or a shift one-cycle, sigma (= N_f times the
+    true-diagonal weight sigma/N_f); a vertex whose two endpoints are BOTH shift one-cycles is excluded (only possible
+    at n = 1, Eq. 83).  absolute: every term enters with its absolute value -- the cancellation scale M of the
+    uniform-mode tolerance (the normal and the shift choice of a one-cycle are separate terms)."""
     n = len(A)
+    N = 2 * n
     total = 0.0
-    for p in itertools.permutations(range(2 * n)):
+    for p in itertools.permutations(range(N)):
         if not _connected(p, n):
             continue
-        w = _sign_by_inversions(p) * n_flavors ** len(_cycles(p))
-        for v in range(2 * n):
-            w *= A[v % n][p[v] % n]
-        total += w
+        sgn = _sign_by_inversions(p)
+        cycles = _cycles(p)
+        fixed = [c[0] for c in cycles if len(c) == 1]
+        long_w = 1.0
+        for c in cycles:
+            if len(c) > 1:
+                w = float(n_flavors)
+                for v in c:
+                    w *= A[v % n][p[v] % n]
+                long_w *= w
+        for k in range(len(fixed) + 1):
+            for Z in itertools.combinations(fixed, k):
+                if k and sigma == 0.0:
+                    continue
+                Zs = set(Z)
+                if any(((v + n) % N) in Zs for v in Zs):
+                    continue
+                w = sgn * long_w
+                for v in fixed:
+                    w *= sigma if v in Zs else n_flavors * A[v % n][v % n]
+                total += abs(w) if absolute else w
     return total

@@ -95,6 +95,30 @@ def test_uniform_matches_literal_enumeration(n, nf):
     assert close(oracle.o3_uniform(A, nf)[0], lit)
 
 
+@pytest.mark.parametrize("n,nf", [(1, 2), (2, 2), (2, 3), (3, 2), (3, 3)])
+@pytest.mark.parametrize("sg", [0.0, 0.35, -0.6])
+def test_uniform_absolute_scale_matches_literal_enumeration(n, nf, sg):
+    """The tolerance scale M of every uniform-mode GPU test is `o3_uniform(absolute=True)` / `o1_connected(sb=False,
+    absolute=True)`: pinned here against the literal enumeration with every term taken in absolute value (PAPER.md:45,
+    Eq. 59; counterterm: PAPER.md:431), single output and every subset, with and without a shift, signed and unsigned."""
+    rng = np.random.default_rng(300 + 10 * n + nf)
+    A = rng.standard_normal((n, n))
+    sig = [sg] if sg else None
+    for absolute in (False, True):
+        lit = uniform_connected_sum(A, nf, sg, absolute=absolute)
+        assert close(oracle.o1_connected(A[None], nf, sig, sb=False, absolute=absolute), lit)
+        assert close(oracle.o3_uniform(A, nf, sg, False, absolute=absolute)[0], lit)
+        allsub = oracle.o3_uniform(A, nf, sg, True, absolute=absolute)
+        o1sub = oracle.o1_all_subsets(A[None], nf, sig, sb=False, absolute=absolute)
+        for S in range(1, 1 << n):
+            idx = [i for i in range(n) if S >> i & 1]
+            lit_S = uniform_connected_sum(A[np.ix_(idx, idx)], nf, sg, absolute=absolute)
+            assert close(allsub[S - 1], lit_S), (S, absolute)
+            assert close(o1sub[S - 1], lit_S), (S, absolute)
+    # the scale dominates the signed value, and strictly so when terms cancel
+    assert oracle.o3_uniform(A, nf, sg, False, absolute=True)[0] >= abs(oracle.o3_uniform(A, nf, sg)[0]) * (1 - 1e-12)
+
+
 # ---------------------------------------------------------------- determinant identities via numpy
 def _moment(Au, Ad, su, sd, T):
     idx = [i for i in range(Au.shape[0]) if T >> i & 1]
