@@ -236,6 +236,13 @@ int cos_det_eval(int n, int n_flavors, int n_blocks, int lattice, const double* 
 int cos_set_profiling(cos_handle h, int on);
 int cos_get_layer_times(cos_handle h, int n_layers, double* ms, long long* n_evals);
 
+/* Self-check build (libcos_b200.so compiled with -DCOS_CHECK_BOUNDS; tests/test_gpu_selfcheck.py builds one): the layer
+ * kernels test every index they derive from the compiled program against the extent of the array it addresses (kinds:
+ * 0 program window, 1 source row, 2 row header, 3 destination state / endpoint, 4 table row, 5 head / colour, 6 fresh-head
+ * destination, 7 output row) and cos_eval fills the workspace with NaN first.  *total = violations counted so far, or -1
+ * when the library was built without the checks (the shipped build); by_kind: host array of 8 counters, or NULL. */
+int cos_debug_check_failures(long long* total, long long* by_kind);
+
 /* fp64 FMA peak of the device (independent FMA chains, no memory traffic).
  * Returns achieved FMA/s in *fma_per_s (synchronous; used by bench.py for the fp64 roofline leg). */
 int cos_measure_fp64_fma_peak(double* fma_per_s);

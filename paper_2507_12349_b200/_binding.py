@@ -8,7 +8,8 @@ import ctypes
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libcos_b200.so")
+# COS_B200_LIB selects another build of the same library (the self-check build of tests/test_gpu_selfcheck.py)
+_LIB_PATH = os.environ.get("COS_B200_LIB") or os.path.join(_HERE, "libcos_b200.so")
 _lib = None
 
 COS_OK, COS_EINVAL, COS_ENOMEM, COS_ECUDA, COS_EUNSUPPORTED = 0, 1, 2, 3, 4
@@ -30,7 +31,7 @@ EXPORTS = [
     "cos_build", "cos_build_ex", "cos_eval", "cos_free", "cos_set_workspace_limit", "cos_info",
     "cos_last_error", "cos_tab_build", "cos_tabulate", "cos_tab_free", "cos_measure_fp64_fma_peak",
     "cos_eval_host", "cos_set_profiling", "cos_get_layer_times", "cos_build_orders", "cos_flux_weights",
-    "cos_det_workspace_bytes", "cos_det_eval", "cos_reserve", "cos_set_tuning",
+    "cos_det_workspace_bytes", "cos_det_eval", "cos_reserve", "cos_set_tuning", "cos_debug_check_failures",
 ]
 
 
@@ -90,6 +91,8 @@ def load_library():
     lib.cos_det_eval.argtypes = [ip, ip, ip, ip, dp, ip, vp, ctypes.c_longlong, vp, vp, ctypes.c_longlong, vp]
     lib.cos_measure_fp64_fma_peak.restype = ctypes.c_int
     lib.cos_measure_fp64_fma_peak.argtypes = [dp]
+    lib.cos_debug_check_failures.restype = ctypes.c_int
+    lib.cos_debug_check_failures.argtypes = [llp, llp]
     lib.cos_reserve.restype = ctypes.c_int
     lib.cos_reserve.argtypes = [vp, ctypes.c_longlong]
     lib.cos_set_tuning.restype = ctypes.c_int
@@ -282,6 +285,14 @@ def cos_get_layer_times(handle):
 
 def cos_tab_free(tab):
     load_library().cos_tab_free(tab)
+
+
+def cos_debug_check_failures():
+    """-> (total, [8 counters by kind]); total = -1 for a library built without COS_CHECK_BOUNDS."""
+    total = ctypes.c_longlong(0)
+    kinds = (ctypes.c_longlong * 8)()
+    _check(load_library().cos_debug_check_failures(ctypes.byref(total), kinds))
+    return total.value, list(kinds)
 
 
 def cos_measure_fp64_fma_peak():

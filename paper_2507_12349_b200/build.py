@@ -36,15 +36,17 @@ def needs_build():
     return any(os.path.getmtime(p) > t for p in deps)
 
 
-def build(force=False, verbose=False):
-    if not force and not needs_build():
+def build(force=False, verbose=False, out=None, extra=()):
+    """Builds libcos_b200.so in-tree; `out` / `extra` build a variant elsewhere (e.g. extra=["-DCOS_CHECK_BOUNDS"])."""
+    lib = out or LIB
+    if out is None and not force and not needs_build():
         return LIB
-    tmp = LIB + ".%d.tmp" % os.getpid()
-    cmd = [_nvcc()] + NVCC_FLAGS + os.environ.get("COS_NVCC_EXTRA", "").split() + (["-Xptxas", "-v"] if verbose else []) + \
-          ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
+    tmp = lib + ".%d.tmp" % os.getpid()
+    cmd = [_nvcc()] + NVCC_FLAGS + list(extra) + os.environ.get("COS_NVCC_EXTRA", "").split() + \
+          (["-Xptxas", "-v"] if verbose else []) + ["-o", tmp] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd)
-    os.replace(tmp, LIB)
-    return LIB
+    os.replace(tmp, lib)
+    return lib
 
 
 if __name__ == "__main__":

@@ -23,7 +23,7 @@ int cuda_fail(cudaError_t e, const char* what)
     return e == cudaErrorMemoryAllocation ? COS_ENOMEM : COS_ECUDA;
 }
 
-struct DeviceLayer { uint32_t* words = nullptr; uint32_t* mask_off = nullptr; };
+struct DeviceLayer { uint32_t* words = nullptr; uint32_t* mask_off = nullptr; uint32_t n_words = 0; };
 
 // compile_dag reports structural limits with this prefix; everything else it returns is an out-of-memory condition
 bool is_unsupported(const std::string& err) { return err.compare(0, 12, "unsupported:") == 0; }
@@ -144,6 +144,7 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
             const LayerProgram& P = D.layers[l];
             const size_t wb = P.words.size() * sizeof(uint32_t), mb = P.mask_off.size() * sizeof(uint32_t);
             if (wb == 0) continue;
+            h->dl[l].n_words = (uint32_t)P.words.size();
             e = cudaMalloc(&h->dl[l].words, wb);
             if (e == cudaSuccess) e = cudaMalloc(&h->dl[l].mask_off, mb);
             if (e == cudaSuccess) e = cudaMemcpy(h->dl[l].words, P.words.data(), wb, cudaMemcpyHostToDevice);
@@ -158,7 +159,7 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
             std::vector<FusedLayer> fl(D.layers.size());
             for (size_t l = 0; l < D.layers.size(); ++l) {
                 fl[l].words = h->dl[l].words; fl[l].mask_off = h->dl[l].mask_off;
-                fl[l].n_masks = D.layers[l].n_masks; fl[l].n_states = D.layers[l].n_states;
+                fl[l].n_masks = D.layers[l].n_masks; fl[l].n_states = D.layers[l].n_states; fl[l].n_words = h->dl[l].n_words;
             }
             e = cudaMalloc(&h->fused_layers, fl.size() * sizeof(FusedLayer));
             if (e == cudaSuccess) e = cudaMemcpy(h->fused_layers, fl.data(), fl.size() * sizeof(FusedLayer), cudaMemcpyHostToDevice);
@@ -303,6 +304,10 @@ static int eval_range(cos_handle h, const double* G_dev, long long batch, double
     int rc = grow_workspace(h, need, "cos_eval: workspace allocation");
     if (rc != COS_OK) return rc;
     double* slab[2] = {h->ws, h->ws + (size_t)D.max_layer_states * TILE * (size_t)tiles_chunk};
+#ifdef COS_CHECK_BOUNDS
+    // self-check build: the slabs start as NaN, so a state that is read before it was written shows in the outputs
+    if (cudaMemsetAsync(h->ws, 0xFF, need, stream) != cudaSuccess) cudaGetLastError();
+#endif
 
     if (clear && D.all_subsets && D.order_mask != (((2u << D.n) - 1u) & ~1u)) {     // partial readout set: other rows are zeros
         cudaError_t e = cudaMemsetAsync(out_dev, 0, (size_t)D.n_out * (size_t)batch * sizeof(double), stream);
@@ -315,7 +320,7 @@ static int eval_range(cos_handle h, const double* G_dev, long long batch, double
             FusedArgs f;
             f.layers = h->fused_layers; f.n_layers = NL; f.ws = h->ws; f.S_max = D.max_layer_states;
             f.G = G_dev; f.batch = batch; f.b0 = t0 * TILE; f.out = out_dev; f.d = D.d; f.n_slots = n_slots;
-            f.neg_kappa = -D.kappa;
+            f.neg_kappa = -D.kappa; f.n_out = (uint32_t)D.n_out;
             for (int c = 0; c < 4; ++c) f.sigma[c] = D.sigma[c];
             cudaError_t ef = launch_fused(f, (int)D.max_L, D.nc, D.has_shift, tiles, 8, stream);
             if (ef != cudaSuccess) return cuda_fail(ef, "cos_eval: fused launch");
@@ -342,7 +347,7 @@ static int eval_range(cos_handle h, const double* G_dev, long long batch, double
             const LayerProgram& P = D.layers[l];
             LayerArgs a;
             a.words = h->dl[l].words; a.mask_off = h->dl[l].mask_off;
-            a.n_masks = P.n_masks;
+            a.n_masks = P.n_masks; a.n_words = h->dl[l].n_words; a.n_out = (uint32_t)D.n_out;
             {   // blocks per CTA: amortise the table staging but keep >= 4 waves of CTAs on the GPU
                 const long long resident = (long long)h->n_sm * h->ctas_per_sm;
                 long long mpc = (long long)P.n_masks * tiles / (resident * 4);
@@ -652,6 +657,16 @@ int cos_det_eval(int n, int n_flavors, int n_blocks, int lattice, const double* 
     a.order = (uint32_t*)p;
     cudaError_t e = launch_det_route(a, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, "cos_det_eval: launch");
+    return COS_OK;
+}
+
+int cos_debug_check_failures(long long* total, long long* by_kind)
+{
+    if (!total) return fail(COS_EINVAL, "cos_debug_check_failures: NULL argument");
+    long long kinds[8];
+    cudaError_t e = read_check_failures(total, kinds);
+    if (e != cudaSuccess) return cuda_fail(e, "cos_debug_check_failures");
+    if (by_kind) for (int k = 0; k < 8; ++k) by_kind[k] = kinds[k];
     return COS_OK;
 }
 

@@ -32,6 +32,17 @@ __device__ __forceinline__ double lds64(uint32_t addr)
     asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
     return v;
 }
+// Self-check build (-DCOS_CHECK_BOUNDS; compute-sanitizer is closed on the pool this was developed on): every index the
+// layer kernels derive from the program -- source rows, destination states, table rows and columns, output rows, the
+// program windows themselves -- is tested against the extent of the array it addresses; violations are counted per kind
+// (cos_debug_check_failures) instead of faulting.  The shipped build compiles the checks out.
+#ifdef COS_CHECK_BOUNDS
+__device__ unsigned long long g_check_fail[8];
+#define COS_CHECK(cond, kind) do { if (!(cond)) atomicAdd(&g_check_fail[kind], 1ull); } while (0)
+#else
+#define COS_CHECK(cond, kind) do { } while (0)
+#endif
+
 __device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 // asynchronous 8-byte global -> shared copy (LDGSTS): no register staging, completion by commit / wait groups
 __device__ __forceinline__ void cp_async8(uint32_t dst, const void* src)
@@ -192,11 +203,26 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
         for (int c = 0; c < NC; ++c) sp[c] = 0.0;
 
         const uint32_t* rp = a.words + off + HDR;
+        // the 32-word windows of the header and of every row stay inside the program (64 words of padding included)
+        COS_CHECK((size_t)off + HDR + (size_t)n_rows * stride + 32u <= (size_t)a.n_words && stride >= 2 + e_words + nJ, 0);
         for (int r = 0; r < n_rows; ++r) {
             uint32_t rw_next = 0u;
             if (r + 1 < n_rows) rw_next = __ldg(rp + (size_t)(r + 1) * stride + lane);
             const uint32_t base = __shfl_sync(0xFFFFFFFFu, rw, 0), rh = __shfl_sync(0xFFFFFFFFu, rw, 1);
             const int L = (int)(rh & 31u);
+#ifdef COS_CHECK_BOUNDS
+            {
+                const int n_dst = (int)((rh >> 17) & 31u) + (int)((rh >> 22) & 1u);
+                COS_CHECK(L >= 1 && L <= MAXL && (size_t)base + L <= (size_t)a.S_src, 1);              // source row
+                COS_CHECK(n_dst <= nJ && (((rh >> 12) & 31u) == 31u || (int)((rh >> 12) & 31u) < L), 2);
+                if (lane >= 2 + e_words && lane < 2 + e_words + (int)((rh >> 17) & 31u))                // destinations
+                    COS_CHECK((rw & DIDX_MASK) < a.S_dst && (rw >> 24) < (uint32_t)a.d, 3);
+                if (lane >= 2 && lane < 2 + e_words)                                                     // table rows
+                    for (int k = 4 * (lane - 2); k < 4 * (lane - 1) && k < L; ++k)
+                        COS_CHECK(((rw >> (8 * (k & 3))) & 0xFFu) < (uint32_t)(NC * a.d), 4);
+                COS_CHECK(((rh >> 5) & 31u) < (uint32_t)a.d && ((rh >> 10) & 3u) < (uint32_t)NC, 5);
+            }
+#endif
             const double* xp = Xt + (size_t)base * TILE;
             if (a.prefetch > 0) {            // L2 look-ahead: the L states `prefetch` states further down the slab
                 for (int q = lane; q < 2 * L; q += 32) {
@@ -224,11 +250,13 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
 #pragma unroll
             for (int c = 0; c < NC; ++c) {
                 const uint32_t didx = __shfl_sync(0xFFFFFFFFu, hw, 3 + c);
+                COS_CHECK(didx < a.S_dst, 6);
                 __stcs(Yt + (size_t)didx * TILE, fma(a.neg_kappa, close, sp[c]));
             }
         }
         if (flags & FLAG_READOUT) {          // terminal readout O_S (Eq. 15): one block per subset S
             const uint32_t out_idx = __shfl_sync(0xFFFFFFFFu, hw, 2);
+            COS_CHECK(out_idx < a.n_out, 7);
             // 2^(|S|-1): the continuation multiplicities of Lemma 7, applied once per output (exact)
             const double scale = (double)(1u << (__shfl_sync(0xFFFFFFFFu, hw, 1) >> 24));
             if (valid) a.out[(size_t)out_idx * (size_t)a.batch + (size_t)b] = (a.neg_kappa * close) * scale;
@@ -320,6 +348,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
     LayerArgs a;
     a.G = f.G; a.batch = f.batch; a.b0 = f.b0; a.out = f.out; a.d = f.d; a.n_slots = f.n_slots;
     a.neg_kappa = f.neg_kappa; a.prefetch = 0; a.pdl = 0; a.S_src = f.S_max; a.S_dst = f.S_max; a.masks_per_cta = 0;
+    a.n_out = f.n_out;
     for (int l = 0; l < f.n_layers; ++l) {
         if (SHIFT && l <= 1) {               // c3 = -2 at layer 0, -1 afterwards (Eq. 72, 77)
             for (int q = warp; q < NC * f.d; q += W) {
@@ -330,7 +359,7 @@ __global__ void __launch_bounds__(MAX_WARPS * 32) cos_fused_kernel(const FusedAr
             __syncthreads();
         }
         const FusedLayer fl = f.layers[l];
-        a.words = fl.words; a.mask_off = fl.mask_off; a.n_masks = fl.n_masks;
+        a.words = fl.words; a.mask_off = fl.mask_off; a.n_masks = fl.n_masks; a.n_words = fl.n_words;
         a.X = (l & 1) ? slab1 : slab0; a.Y = (l & 1) ? slab0 : slab1;
         // slabs are addressed per tile already: tile index 0 inside layer_blocks
         layer_blocks<MAXL, NC, SHIFT, true>(a, 0u, fl.n_masks, 0u, s_next, gs_lane, gd_lane, lane, valid, b);
@@ -498,6 +527,22 @@ cudaError_t launch_fused(const FusedArgs& f, int max_L, int nc, bool shift, uint
     const size_t smem = layer_smem_bytes(f.n_slots, nc, f.d, shift);
     fn<<<tiles, 32 * warps_per_cta, smem, stream>>>(f);
     return cudaGetLastError();
+}
+
+// Self-check counters: -1 when the library was built without COS_CHECK_BOUNDS.
+cudaError_t read_check_failures(long long* total, long long* by_kind)
+{
+#ifdef COS_CHECK_BOUNDS
+    unsigned long long h[8];
+    cudaError_t e = cudaMemcpyFromSymbol(h, g_check_fail, sizeof(h));
+    if (e != cudaSuccess) return e;
+    *total = 0;
+    for (int k = 0; k < 8; ++k) { by_kind[k] = (long long)h[k]; *total += (long long)h[k]; }
+#else
+    *total = -1;
+    for (int k = 0; k < 8; ++k) by_kind[k] = 0;
+#endif
+    return cudaSuccess;
 }
 
 // ------------------------------------------------------------------------------------------------------

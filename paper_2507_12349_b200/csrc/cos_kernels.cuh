@@ -12,6 +12,7 @@ struct LayerArgs {
     const uint32_t* words;               // layer program (cos_compile.h)
     const uint32_t* mask_off;            // [n_masks+1][2]: {header word offset, first state}
     uint32_t n_masks, masks_per_cta;
+    uint32_t n_words, n_out;             // extent of `words` (padding included) and of the output rows (self-check build)
     const double* X;                     // source slab  [tile][S_src][32]
     double* Y;                           // destination slab [tile][S_dst][32]
     uint32_t S_src, S_dst;
@@ -38,7 +39,7 @@ cudaError_t pick_layer_shape(int max_L, int nc, int d, int n_slots, bool shift, 
 cudaError_t layer_ctas_per_sm(int max_L, int nc, int d, int n_slots, bool shift, int warps_per_cta, int* ctas_per_sm);
 
 // ---- fused small-DAG path: every layer in one launch (cos_fused_kernel)
-struct FusedLayer { const uint32_t* words; const uint32_t* mask_off; uint32_t n_masks, n_states; };
+struct FusedLayer { const uint32_t* words; const uint32_t* mask_off; uint32_t n_masks, n_states, n_words; };
 struct FusedArgs {
     const FusedLayer* layers;            // device array [n_layers]
     int n_layers;
@@ -46,6 +47,7 @@ struct FusedArgs {
     uint32_t S_max;
     const double* G; long long batch, b0; double* out;
     int d, n_slots;
+    uint32_t n_out;
     double neg_kappa;
     double sigma[4];
 };
@@ -88,5 +90,6 @@ struct DetArgs {
 cudaError_t launch_det_route(const DetArgs& a, cudaStream_t stream);
 
 cudaError_t measure_fp64_fma(double* fma_per_s);
+cudaError_t read_check_failures(long long* total, long long* by_kind);
 
 }  // namespace cosb

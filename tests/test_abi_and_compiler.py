@@ -140,3 +140,66 @@ def test_det_route_argument_checks_need_no_gpu(cos):
         assert lib.cos_det_eval(*args) == code, args
         assert cos.cos_last_error()
     assert lib.cos_det_eval(4, 3, 3, 0, None, 0, p, 0, p, p, 0, None) == cos.COS_OK                  # batch 0: no-op
+
+
+def test_structural_limits_are_unsupported_not_out_of_memory(cos):
+    """include/cos.h, cos_build: structural limits come back as COS_EUNSUPPORTED with the reason, COS_ENOMEM is memory
+    exhaustion only.  Honeycomb SB-CoS at n = 11 exceeds the 24-bit destination index of the layer program (north_star
+    asks for orders up to 12 on both lattices: the honeycomb range of this build ends at n = 10 for SB-CoS; the uniform
+    honeycomb DAG still compiles at n = 11)."""
+    with pytest.raises(cos.CosError) as ei:
+        cos.cos_build_ex(11, 2, cos.COS_LATTICE_HONEYCOMB, [0.3, -0.3], 0, flags=cos.COS_BUILD_HOST_ONLY)
+    assert ei.value.code == cos.COS_EUNSUPPORTED and "24-bit" in str(ei.value)
+    with pytest.raises(cos.CosError) as ei:
+        cos.cos_build_ex(4, 5, cos.COS_LATTICE_SQUARE, [0.1] * 5, 0, flags=cos.COS_BUILD_HOST_ONLY)
+    assert ei.value.code == cos.COS_EUNSUPPORTED
+    # the largest BASELINE-shaped honeycomb order this build supports compiles host-only (3.9e7 states)
+    h = cos.cos_build_ex(10, 2, cos.COS_LATTICE_HONEYCOMB, [0.3, -0.3], 0, flags=cos.COS_BUILD_HOST_ONLY)
+    assert cos.cos_info(h, "n_states") == 39320580 and cos.cos_info(h, "device") == -1
+    cos.cos_free(h)
+
+
+def test_tuning_and_reserve_argument_checks(cos):
+    """cos_set_tuning / cos_reserve on a host-only handle: value checks are status codes; nothing touches CUDA."""
+    h = cos.cos_build_ex(5, 2, cos.COS_LATTICE_SQUARE, None, 0, flags=cos.COS_BUILD_HOST_ONLY)
+    try:
+        for what, good, bad in (("prefetch", 16, -1), ("prefetch", 0, 5000), ("warps_per_cta", 8, 0),
+                                ("warps_per_cta", 24, 25), ("blocks_per_cta_cap", 0, 70000), ("host_slices", 8, 9),
+                                ("host_slices", 1, 0), ("tiles_per_chunk", 0, -2)):
+            cos.cos_set_tuning(h, what, good)
+            with pytest.raises(cos.CosError) as ei:
+                cos.cos_set_tuning(h, what, bad)
+            assert ei.value.code == cos.COS_EINVAL
+        cos.cos_set_tuning(h, "pdl", 0)
+        cos.cos_set_tuning(h, "fused", 1)
+        assert cos.cos_info(h, "fused") == 0            # host-only handles have no fused path
+        with pytest.raises(cos.CosError) as ei:
+            cos.cos_set_tuning(h, 42, 1)
+        assert ei.value.code == cos.COS_EINVAL
+        with pytest.raises(cos.CosError) as ei:
+            cos.cos_reserve(h, 64)
+        assert ei.value.code == cos.COS_ECUDA
+        with pytest.raises(cos.CosError) as ei:
+            cos.cos_reserve(h, -1)
+        assert ei.value.code == cos.COS_EINVAL
+    finally:
+        cos.cos_free(h)
+
+
+def test_library_reads_no_environment_variable(cos):
+    """The launch tuning goes through cos_set_tuning only (include/cos.h): no getenv in the product sources."""
+    csrc = os.path.join(ROOT, "paper_2507_12349_b200", "csrc")
+    for name in os.listdir(csrc):
+        assert "getenv" not in open(os.path.join(csrc, name)).read(), name
+
+
+def test_host_compiler_under_address_and_ub_sanitizers(tmp_path):
+    """g++ -fsanitize=address,undefined on the host DAG compiler, every mode, n = 1..8 (tests/host_compiler_sanitize.cpp):
+    no report, exit code 0."""
+    import subprocess
+    exe = str(tmp_path / "host_compiler_sanitize")
+    subprocess.check_call(["g++", "-O1", "-g", "-std=c++17", "-fsanitize=address,undefined", "-fno-sanitize-recover=undefined",
+                           "-o", exe, os.path.join(ROOT, "tests", "host_compiler_sanitize.cpp"),
+                           os.path.join(ROOT, "paper_2507_12349_b200", "csrc", "cos_compile.cpp")])
+    r = subprocess.run([exe], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and r.stdout.startswith("ok,") and not r.stderr.strip(), r.stdout + r.stderr
