@@ -32,9 +32,10 @@ from cos_workloads.tables import table_for  # noqa: E402
 
 METRIC = "connected_sum_configs_per_s"
 UNIT = "configs/s"
-# DRAM bytes (read + write) of the layer-kernel launches of ONE step, from a committed ncu capture; per workload at its
-# BASELINE batch.  None = not captured.
-NCU_DRAM_BYTES_PER_STEP = {"cfg4_square_sb3_n10": (244.573e9, 8192, "profiles/r01e_dram_traffic_step.md")}
+# DRAM bytes (read + write) of the layer-kernel launches of ONE step from a committed `ncu --set full` capture of the
+# SHIPPED kernels, per workload and batch: (bytes, batch, launches captured, source).  The value is a citation of that
+# capture, not something this run measures; other workloads / batches report null.  Re-capture after any kernel change.
+NCU_DRAM_BYTES_PER_STEP = {}
 DEFAULT_WORKLOAD = "cfg4"       # n = 10: the order BASELINE.json's target is quoted on
 
 
@@ -47,6 +48,8 @@ def parse_args():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, help="cfg1..cfg5 (BASELINE.json configs, 1-based)")
     ap.add_argument("--batch", type=int, default=0, help="override the configuration count (0 = BASELINE's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-workloads", action="store_true",
+                    help="skip the short timings of the other BASELINE configurations (other_workloads block)")
     ap.add_argument("--layers", action="store_true", help="print the per-layer table to stderr")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
                     help="launch tuning through cos_set_tuning (prefetch, warps_per_cta, blocks_per_cta_cap, pdl, ...)")
@@ -90,11 +93,15 @@ def _oracle_one(task):
 
 
 def oracle_tier_name(w):
+    """The cheapest oracle tier that returns the workload's outputs.  BASELINE.md section 3 names the fp64 O3 recurrences
+    as the CPU evaluator; for the SB workloads at n = 10 literal Algorithm 3 costs ~78 s per configuration and core (cfg4;
+    2^10 sublattice assignments times that for cfg3), outside the bounded-sample budget, so the determinant routes
+    (binary128 arithmetic, 14-16 s per configuration and core) are timed there -- they are the FASTER CPU program."""
     if w.alphas is None and w.n_sub == 1:
-        return "O3 uniform rooted recurrence (Eq. 8-15)"
+        return "O3 uniform rooted recurrence (Eq. 8-15), fp64"
     if w.alphas is not None and w.n_sub == 1 and not w.all_subsets:
-        return "O2b determinant-polynomial route (Eq. 34-38)"
-    return "sum over sublattice assignments of %s" % ("O2a' two-determinant CDet" if w.n_flavors == 2 else "O2b")
+        return "O2b determinant-polynomial route (Eq. 34-38), binary128 (cheaper than O3 / Algorithm 3 fp64 at this size)"
+    return "sum over sublattice assignments of %s, binary128" % ("O2a' two-determinant CDet" if w.n_flavors == 2 else "O2b")
 
 
 def time_oracle(w, n_sample, procs):
@@ -209,6 +216,51 @@ def run_reference(args):
 
 
 # ------------------------------------------------------------------------------------------ our arm
+def quick_measure(cos, torch, cfg, steps, warmup, peak_gbs, local_rank):
+    """Short device-resident timing of another BASELINE configuration at its full size (same step: tabulate + evaluate):
+    ms per step, configurations/s, whole-step fraction of the HBM roofline, clocks."""
+    w = get_config(cfg)
+    table = table_for(w)
+    v = draw_vertices(w)
+    tab = cos.cos_tab_build(w.lattice, w.L, table.n_blocks, w.beta, w.n_tau, table.data)
+    h = cos.cos_build(w.n, w.n_flavors, w.lattice, w.sigmas, w.n if w.all_subsets else 0)
+    try:
+        info = cos.dag_summary(h)
+        B = w.batch
+        n_slots = info["n_blocks"] * info["d"] ** 2
+        dev = torch.device("cuda", local_rank)
+        sites, tau = torch.from_numpy(v["sites"]).to(dev), torch.from_numpy(v["tau"]).to(dev)
+        G = torch.empty((n_slots, B), dtype=torch.float64, device=dev)
+        out = torch.empty((w.n_out, B), dtype=torch.float64, device=dev)
+        stream = torch.cuda.current_stream()
+        cos.cos_reserve(h, B)
+        for _ in range(warmup):
+            cos.cos_tabulate(tab, w.n, sites, tau, B, G, stream)
+            cos.cos_eval(h, G, B, out, stream)
+        torch.cuda.synchronize()
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            cos.cos_tabulate(tab, w.n, sites, tau, B, G, stream)
+            cos.cos_eval(h, G, B, out, stream)
+        e1.record(stream)
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        ms = e0.elapsed_time(e1) / steps
+        assert bool(torch.isfinite(out).all())
+        alg = (16 * info["n_states"] + 8 * n_slots + 8 * w.n_out) * B + info["program_bytes"]
+        return {"workload": w.name, "n": w.n, "batch": B, "steps": steps, "warmup": warmup, "ms_per_step": ms,
+                "configs_per_s": B / (ms * 1e-3),
+                "edge_evals_per_s": (info["n_edges"] + info["n_readout_edges"]) * B / (ms * 1e-3),
+                "algorithmic_bytes_per_step": alg, "frac_whole_step": alg / (ms * 1e-3) / (peak_gbs * 1e9),
+                "clocks": clocks}
+    finally:
+        cos.cos_free(h)
+        cos.cos_tab_free(tab)
+
+
 def run_ours(args):
     import torch
     import torch.distributed as dist
@@ -265,6 +317,7 @@ def run_ours(args):
             dist.barrier()
         torch.cuda.synchronize()
 
+    cos.cos_reserve(h, B)               # cos_eval then only enqueues kernels
     for _ in range(max(args.warmup, 3)):
         step()
     barrier()
@@ -340,7 +393,7 @@ def run_ours(args):
         traffic, traffic_src = None, None
         cap = NCU_DRAM_BYTES_PER_STEP.get(w.name)
         if cap and cap[1] == B:
-            traffic, traffic_src = cap[0] / NL, cap[2] + " (per launch = step total / %d launches)" % NL
+            traffic, traffic_src = cap[0] / cap[2], cap[3] + " (per launch = captured total / %d launches)" % cap[2]
         fma_peak = cos.cos_measure_fp64_fma_peak()
         t_hbm = alg_bytes_step / (peak_gbs * 1e9)
         t_fp64 = info["n_fma"] * B / fma_peak
@@ -368,10 +421,16 @@ def run_ours(args):
                 "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K,
                         "h2d_bytes_per_step": B * w.n * (2 * 4 + 8), "d2h_bytes_per_step": B * w.n_out * 8},
                 "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}
+        if world == 1 and not args.no_other_workloads and args.workload == DEFAULT_WORKLOAD and not args.batch:
+            # the other n = 10 configuration (cfg3, the larger and weaker one) and cfg2 / cfg5 / cfg1, driver-timed in the
+            # same run: short timings (>= 3 warm-up steps), whole-step roofline fraction; not the headline `value`
+            line["other_workloads"] = [quick_measure(cos, torch, c, k, 3, peak_gbs, local_rank)
+                                       for c, k in ((3, 3), (2, 10), (5, 20), (1, 50))]
         if not args.no_cpu_baseline and world == 1:
             n_sample, procs = oracle_sample_plan(args)
             rate, dt = time_oracle(workload_of(args), n_sample, procs)
             line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": procs, "kind": "oracle", "seconds": dt,
+                                    "tier": oracle_tier_name(w),
                                     "sample": "%d configurations of %s, %s" % (n_sample, w.name, oracle_tier_name(w))}
         if args.layers:
             sys.stderr.write("layer  states      ms/step   GB/s(alg)\n")

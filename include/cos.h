@@ -81,6 +81,18 @@ int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int re
 int cos_build_orders(int n, int n_flavors, int lattice, const double* shifts, unsigned int order_mask, int flags,
                      cos_handle* out);
 
+/* Compiler analysis (host only, no CUDA): future / past equivalence classes of the pruned DAG.
+ * States with equal future signature Sigma+ (Eq. 25-26) could be merged by adding their values, states with equal past
+ * signature Sigma- (Eq. 27-28) carry equal values and need to be stored once; operators are compared as SYMBOLS (the
+ * propagator entry G_lambda[a][b] or the counterterm of colour lambda, with the integer coefficient of Eq. 17), i.e. for
+ * generic numeric propagators.  One backward and one forward refinement pass.  Arguments as cos_build_ex (flags:
+ * COS_BUILD_UNIFORM_SHIFT only).  out6 (host, 6 values): states, edges (E1..E4 uncoalesced + readouts), future classes,
+ * edges after the future merge, past classes, edges after the past merge.  Limited to DAGs of at most 6e7 states
+ * (COS_EUNSUPPORTED beyond).  DESIGN.md section 9 reports the result: the only equivalences of the reduced recurrence
+ * are the N_c fresh-head states of a close-and-open step and the initial states -- both already exploited. */
+int cos_equivalence_stats(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope, int flags,
+                          long long* out6);
+
 /* ---- (3)+(4) layer propagation and terminal readouts: Eq. 16, Eq. 11-15 ----------------------------
  *   G_dev    device, fp64, read-only: G_dev[((blk*d + a)*d + b) * batch + c] = propagator of block blk
  *            from endpoint a to endpoint b (A[vbar, pi(v)bar] of Eq. 59) of configuration c;

@@ -32,6 +32,7 @@ EXPORTS = [
     "cos_last_error", "cos_tab_build", "cos_tabulate", "cos_tab_free", "cos_measure_fp64_fma_peak",
     "cos_eval_host", "cos_set_profiling", "cos_get_layer_times", "cos_build_orders", "cos_flux_weights",
     "cos_det_workspace_bytes", "cos_det_eval", "cos_reserve", "cos_set_tuning", "cos_debug_check_failures",
+    "cos_equivalence_stats",
 ]
 
 
@@ -91,6 +92,8 @@ def load_library():
     lib.cos_det_eval.argtypes = [ip, ip, ip, ip, dp, ip, vp, ctypes.c_longlong, vp, vp, ctypes.c_longlong, vp]
     lib.cos_measure_fp64_fma_peak.restype = ctypes.c_int
     lib.cos_measure_fp64_fma_peak.argtypes = [dp]
+    lib.cos_equivalence_stats.restype = ctypes.c_int
+    lib.cos_equivalence_stats.argtypes = [ip, ip, ip, dp, ip, ip, llp]
     lib.cos_debug_check_failures.restype = ctypes.c_int
     lib.cos_debug_check_failures.argtypes = [llp, llp]
     lib.cos_reserve.restype = ctypes.c_int
@@ -285,6 +288,16 @@ def cos_get_layer_times(handle):
 
 def cos_tab_free(tab):
     load_library().cos_tab_free(tab)
+
+
+def cos_equivalence_stats(n, n_flavors, lattice, shifts, readout_envelope, flags=0):
+    """Future / past equivalence classes of the compiled DAG (Eq. 25-28), host only.
+    -> dict(states, edges, future_classes, edges_after_future_merge, past_classes, edges_after_past_merge)."""
+    keep, p = _shifts_arg(shifts)
+    out = (ctypes.c_longlong * 6)()
+    _check(load_library().cos_equivalence_stats(int(n), int(n_flavors), int(lattice), p, int(readout_envelope), int(flags), out))
+    return dict(zip(("states", "edges", "future_classes", "edges_after_future_merge", "past_classes",
+                     "edges_after_past_merge"), [int(x) for x in out]))
 
 
 def cos_debug_check_failures():

@@ -660,6 +660,26 @@ int cos_det_eval(int n, int n_flavors, int n_blocks, int lattice, const double* 
     return COS_OK;
 }
 
+int cos_equivalence_stats(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope, int flags,
+                          long long* out6)
+{
+    if (!out6) return fail(COS_EINVAL, "cos_equivalence_stats: out is NULL");
+    if (n < 1 || n > COS_MAX_N || n_flavors < 1 || (lattice != COS_LATTICE_SQUARE && lattice != COS_LATTICE_HONEYCOMB) ||
+        (readout_envelope != 0 && readout_envelope != n))
+        return fail(COS_EINVAL, "cos_equivalence_stats: bad argument");
+    const bool uniform_shift = (flags & COS_BUILD_UNIFORM_SHIFT) != 0;
+    if (uniform_shift && !shifts) return fail(COS_EINVAL, "cos_equivalence_stats: COS_BUILD_UNIFORM_SHIFT needs shifts[0]");
+    CompiledDag D;
+    EquivalenceStats eq;
+    std::string err = compile_dag(n, n_flavors, lattice == COS_LATTICE_HONEYCOMB ? 2 : 1, shifts, uniform_shift,
+                                  readout_envelope == n, 0u, D, &eq);
+    if (!err.empty()) return fail(is_unsupported(err) ? COS_EUNSUPPORTED : COS_ENOMEM, "cos_equivalence_stats: " + err);
+    out6[0] = (long long)eq.n_states; out6[1] = (long long)eq.n_edges;
+    out6[2] = (long long)eq.future_classes; out6[3] = (long long)eq.edges_after_future_merge;
+    out6[4] = (long long)eq.past_classes; out6[5] = (long long)eq.edges_after_past_merge;
+    return COS_OK;
+}
+
 int cos_debug_check_failures(long long* total, long long* by_kind)
 {
     if (!total) return fail(COS_EINVAL, "cos_debug_check_failures: NULL argument");

@@ -16,6 +16,7 @@
 
 #include <algorithm>
 #include <cstring>
+#include <map>
 
 namespace cosb {
 namespace {
@@ -82,7 +83,7 @@ struct Builder {
 }  // namespace
 
 std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool uniform_shift, bool all_subsets,
-                        uint32_t order_mask, CompiledDag& out)
+                        uint32_t order_mask, CompiledDag& out, EquivalenceStats* eq)
 {
     const bool uniform = (sigma == nullptr) || uniform_shift;
     if (n < 1 || n > 12) return "n must be in [1, 12]";
@@ -205,6 +206,114 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
             if (counter >= DIDX_DEAD) return "unsupported: a layer has more than 2^24 - 1 states (24-bit destination index)";
             out.layers[l].n_states = (uint32_t)counter;
             out.layers[l].n_masks = (uint32_t)ids.size();
+        }
+
+        // ---- optional analysis: future / past equivalence classes of the pruned DAG (Eq. 25-28)
+        if (eq) {
+            *eq = EquivalenceStats();
+            // global numbering: layer offsets + index inside the layer; edges enumerated exactly as the emission does
+            std::vector<uint64_t> layer_off(NL + 1, 0);
+            for (int l = 0; l < NL; ++l) layer_off[l + 1] = layer_off[l] + out.layers[l].n_states;
+            const uint64_t S = layer_off[NL];
+            if (S > 60000000ull) return "unsupported: equivalence analysis is limited to 6e7 states";
+            // an edge = (label, coefficient, other end): label = the factor SYMBOL (G_lambda[a][b], or the counterterm of
+            // colour lambda); two edges carry the same operator iff label and integer coefficient agree (Eq. 17)
+            struct Edge { uint32_t src, dst; uint32_t label; int32_t coeff; };
+            std::vector<Edge> edges;
+            std::vector<std::pair<uint32_t, uint64_t>> readouts;     // (state, label | out_idx << 32)
+            const uint32_t SHIFT_LABEL = (uint32_t)(nc * d * d);
+            for (int l = 0; l < NL; ++l)
+                for (uint32_t id : b.by_layer[l]) {
+                    const uint32_t code = b.codes[id];
+                    const int jm = b.jmin(code);
+                    const int nJ = (l + 1 < NL) ? b.jlist(code, J) : 0;
+                    int32_t fresh_did = -1; uint32_t fresh_a = 0; bool fresh = false;
+                    if (jm >= 0 && l + 1 < NL) {
+                        fresh_a = (uint32_t)(jm * nsub + (Builder::cell(code, jm) - 1));
+                        fresh_did = b.index_of[code | (3u << (2 * jm))];
+                        fresh = fresh_did >= 0 && ((b.alive[(size_t)fresh_did * d + fresh_a] >> fresh_a) & 1u);
+                    }
+                    const bool readout = jm < 0 && requested(b.full_set(code));
+                    for (int h = 0; h < d; ++h) {
+                        const uint32_t a = b.alive[(size_t)id * d + h];
+                        for (int e = 0; e < d && a; ++e) {
+                            if (!((a >> e) & 1u)) continue;
+                            for (int lam = 0; lam < nc; ++lam) {
+                                const uint32_t src = (uint32_t)(layer_off[l] + b.state_index(id, h, lam, e));
+                                for (int q = 0; q < nJ; ++q) {
+                                    const int32_t did = b.index_of[J[q].dest_code];
+                                    if (did < 0 || !((b.alive[(size_t)did * d + h] >> J[q].j_a) & 1u)) continue;
+                                    const uint32_t dst = (uint32_t)(layer_off[l + 1] + b.state_index((uint32_t)did, h, lam, J[q].j_a));
+                                    edges.push_back({src, dst, (uint32_t)((lam * d + e) * d + J[q].j_a), J[q].mult2 ? 2 : 1});
+                                    if (b.has_shift && !J[q].mult2 && J[q].j_a == e)      // E3 shares E2's destination
+                                        edges.push_back({src, dst, SHIFT_LABEL + (uint32_t)lam, l == 0 ? -2 : -1});
+                                }
+                                if (fresh)
+                                    for (int l2 = 0; l2 < nc; ++l2)
+                                        edges.push_back({src, (uint32_t)(layer_off[l + 1] + b.state_index((uint32_t)fresh_did, (int)fresh_a, l2, (int)fresh_a)),
+                                                         (uint32_t)((lam * d + e) * d + h), -(int32_t)out.kappa});
+                                if (readout)
+                                    readouts.push_back({src, (uint64_t)((lam * d + e) * d + h) |
+                                                                 ((uint64_t)(all_subsets ? b.full_set(code) : 1u) << 32)});
+                            }
+                        }
+                    }
+                }
+            eq->n_states = S; eq->n_edges = edges.size() + readouts.size();
+            auto key = [](uint32_t label, int32_t coeff, uint32_t cls) {
+                return ((uint64_t)label << 40) | ((uint64_t)(uint32_t)(coeff + 8) << 36) | (uint64_t)cls;
+            };
+            // future classes (Eq. 25-26): last layer first; signature = sorted (label, coefficient, class of the child)
+            std::vector<std::vector<uint64_t>> sig(S);
+            std::vector<uint32_t> cls(S, 0);
+            for (auto& r : readouts) sig[r.first].push_back((1ull << 63) | r.second);
+            std::vector<uint32_t> order(edges.size());
+            for (size_t i = 0; i < edges.size(); ++i) order[i] = (uint32_t)i;
+            std::stable_sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) { return edges[x].src > edges[y].src; });
+            {
+                size_t pos = 0;
+                uint64_t n_cls = 0, n_edges_after = 0;
+                for (int l = NL - 1; l >= 0; --l) {
+                    // edges are sorted by decreasing source: the sources of layer l come after those of layer l + 1
+                    while (pos < order.size() && edges[order[pos]].src >= layer_off[l]) {
+                        const Edge& E = edges[order[pos++]];
+                        sig[E.src].push_back(key(E.label, E.coeff, cls[E.dst]));
+                    }
+                    std::map<std::vector<uint64_t>, uint32_t> ids;
+                    for (uint64_t x = layer_off[l]; x < layer_off[l + 1]; ++x) {
+                        std::sort(sig[x].begin(), sig[x].end());
+                        auto it = ids.find(sig[x]);
+                        if (it == ids.end()) { it = ids.emplace(sig[x], (uint32_t)ids.size()).first; n_edges_after += sig[x].size(); }
+                        cls[x] = (uint32_t)(layer_off[l] + it->second);
+                        std::vector<uint64_t>().swap(sig[x]);
+                    }
+                    n_cls += ids.size();
+                }
+                eq->future_classes = n_cls; eq->edges_after_future_merge = n_edges_after;
+            }
+            // past classes (Eq. 27-28): first layer first; signature = sorted (label, coefficient, class of the parent);
+            // the initial states (value 1, Eq. 66) share the empty signature
+            std::stable_sort(order.begin(), order.end(), [&](uint32_t x, uint32_t y) { return edges[x].dst < edges[y].dst; });
+            {
+                size_t pos = 0;
+                uint64_t n_cls = 0, n_edges_after = readouts.size();
+                for (int l = 0; l < NL; ++l) {
+                    while (pos < order.size() && edges[order[pos]].dst < layer_off[l + 1]) {
+                        const Edge& E = edges[order[pos++]];
+                        sig[E.dst].push_back(key(E.label, E.coeff, cls[E.src]));
+                    }
+                    std::map<std::vector<uint64_t>, uint32_t> ids;
+                    for (uint64_t x = layer_off[l]; x < layer_off[l + 1]; ++x) {
+                        std::sort(sig[x].begin(), sig[x].end());
+                        auto it = ids.find(sig[x]);
+                        if (it == ids.end()) { it = ids.emplace(sig[x], (uint32_t)ids.size()).first; n_edges_after += sig[x].size(); }
+                        cls[x] = (uint32_t)(layer_off[l] + it->second);
+                        std::vector<uint64_t>().swap(sig[x]);
+                    }
+                    n_cls += ids.size();
+                }
+                eq->past_classes = n_cls; eq->edges_after_past_merge = n_edges_after;
+            }
         }
 
         // ---- emission

@@ -55,12 +55,23 @@ struct CompiledDag {
     int hdr_words() const { return 3 + nc; }
 };
 
+// Future / past equivalence classes of the pruned DAG: states with the same future signature
+// Sigma+ (Eq. 25-26: the set of (operator, class of the child) over their out-edges and readouts) can be merged by adding
+// their values; states with the same past signature Sigma- (Eq. 27-28: (operator, class of the parent) over their
+// in-edges) carry the same value and need to be stored once.  One backward and one forward refinement pass each.
+struct EquivalenceStats {
+    uint64_t n_states = 0, n_edges = 0;                           // E1..E4 uncoalesced + readout edges
+    uint64_t future_classes = 0, edges_after_future_merge = 0;
+    uint64_t past_classes = 0, edges_after_past_merge = 0;
+};
+
 // Returns "" on success, else an error message ("unsupported: ..." for a structural limit, otherwise out of memory).
 // n in [1,12]; nsub in {1,2}.  sigma == nullptr -> uniform CoS without counterterm; sigma != nullptr -> SB-CoS with nf
 // colours and shift-close weights sigma[0..nf), or, with uniform_shift, uniform CoS (one colour, loop factor nf) whose
 // counterterm one-cycle has weight sigma[0] (reading G12).
 // order_mask (all_subsets only): bit k set <=> subsets of order k are requested outputs (0 = every order).
+// eq != nullptr: additionally fill the equivalence statistics (host time and memory ~ the edge count; <= 6e7 states).
 std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool uniform_shift, bool all_subsets,
-                        uint32_t order_mask, CompiledDag& out);
+                        uint32_t order_mask, CompiledDag& out, EquivalenceStats* eq = nullptr);
 
 }  // namespace cosb

@@ -203,3 +203,33 @@ def test_host_compiler_under_address_and_ub_sanitizers(tmp_path):
                            os.path.join(ROOT, "paper_2507_12349_b200", "csrc", "cos_compile.cpp")])
     r = subprocess.run([exe], capture_output=True, text=True, timeout=600)
     assert r.returncode == 0 and r.stdout.startswith("ok,") and not r.stderr.strip(), r.stdout + r.stderr
+
+
+def test_future_and_past_equivalence_classes(cos):
+    """Compiler compression, PAPER.md:219-241 (Eq. 25-28), evaluated on the reduced recurrence (cos_equivalence_stats):
+    with propagator entries compared as symbols NO two states of a layer share a future signature (the closing factor
+    G_lambda[e][h] and the continuation factors G_lambda[e][j] pin colour, endpoint, head and mask), and the only past
+    equivalences are the N_c fresh-head states of a close-and-open step (Eq. 12, 70-71: equal in-edges for every colour)
+    and the initial states (value 1, Eq. 66) -- both already exploited by the kernel (one closing sum fanned out to the
+    N_c states; edge count after the past merge = the executed multiply-adds before E2/E4 coalescing)."""
+    sb3 = [0.2, 0.0, -0.2]
+    for args in [(4, 2, 0, None, 0), (6, 2, 0, None, 0), (8, 2, 0, None, 0), (5, 3, 0, None, 0)]:
+        r = cos.cos_equivalence_stats(*args)
+        h = cos.cos_build_ex(*args, flags=cos.COS_BUILD_HOST_ONLY)
+        assert r["states"] == cos.cos_info(h, "n_states")
+        assert r["edges"] == cos.cos_info(h, "n_edges") + cos.cos_info(h, "n_readout_edges")
+        cos.cos_free(h)
+        assert r["future_classes"] == r["states"] and r["edges_after_future_merge"] == r["edges"]
+        assert r["past_classes"] == r["states"] and r["edges_after_past_merge"] == r["edges"]      # uniform, one root
+    r = cos.cos_equivalence_stats(4, 2, 0, None, 4)            # all subsets: the 4 initial states (roots 0..3) are equal
+    assert r["future_classes"] == r["states"] == 245 and r["past_classes"] == 242
+    for n, want_states, want_past in ((6, 9465, 9041), (8, 135213, 131093)):
+        r = cos.cos_equivalence_stats(n, 3, 0, sb3, 0)
+        assert r["states"] == want_states and r["future_classes"] == want_states
+        assert r["past_classes"] == want_past and r["edges_after_past_merge"] < r["edges"]
+    r = cos.cos_equivalence_stats(4, 2, 1, [0.3, -0.3], 0)     # honeycomb, sublattice labels in the mask
+    assert r["future_classes"] == r["states"] == 2292 and r["past_classes"] == 2233
+    r = cos.cos_equivalence_stats(5, 3, 0, [0.4], 0, flags=cos.COS_BUILD_UNIFORM_SHIFT)
+    assert r["future_classes"] == r["states"] == r["past_classes"]
+    with pytest.raises(cos.CosError):
+        cos.cos_equivalence_stats(4, 2, 0, None, 3)
