@@ -35,7 +35,12 @@ UNIT = "configs/s"
 # DRAM bytes (read + write) of the layer-kernel launches of ONE step from a committed `ncu --set full` capture of the
 # SHIPPED kernels, per workload and batch: (bytes, batch, launches captured, source).  The value is a citation of that
 # capture, not something this run measures; other workloads / batches report null.  Re-capture after any kernel change.
-NCU_DRAM_BYTES_PER_STEP = {}
+NCU_DRAM_BYTES_PER_STEP = {
+    ("cfg4_square_sb3_n10", 8192): (244.663e9, 20, "profiles/r02b_layer_kernel_all_layers.md (ncu --set full, all 20 "
+                                    "layer launches of one step, round-2 row kernel)"),
+    ("cfg3_honeycomb_sb2_n10", 576): (377.628e9, 20, "profiles/r02b_layer_kernel_all_layers.md (ncu --set full, the 20 "
+                                      "layer launches of one 576-configuration workspace chunk)"),
+}
 DEFAULT_WORKLOAD = "cfg4"       # n = 10: the order BASELINE.json's target is quoted on
 
 
@@ -391,9 +396,9 @@ def run_ours(args):
             peak_gbs, peak_src = 6650.0, "fallback (B200_PROFILING.md)"
         achieved_gbs = alg_bytes_step / layer_s_step / 1e9
         traffic, traffic_src = None, None
-        cap = NCU_DRAM_BYTES_PER_STEP.get(w.name)
-        if cap and cap[1] == B:
-            traffic, traffic_src = cap[0] / cap[2], cap[3] + " (per launch = captured total / %d launches)" % cap[2]
+        cap = NCU_DRAM_BYTES_PER_STEP.get((w.name, B))
+        if cap:
+            traffic, traffic_src = cap[0] / cap[1], cap[2] + "; per launch = captured total / %d launches" % cap[1]
         fma_peak = cos.cos_measure_fp64_fma_peak()
         t_hbm = alg_bytes_step / (peak_gbs * 1e9)
         t_fp64 = info["n_fma"] * B / fma_peak
