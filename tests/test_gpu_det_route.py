@@ -360,7 +360,8 @@ def test_det_route_edge_cases_and_errors(cos):
     with pytest.raises(cos.CosError) as e:
         cos.cos_det_eval(n, 3, 3, None, 0, Gd, 4, out, work, lattice=2)
     assert e.value.code == cos.COS_EINVAL
-    for args, code in (((n, 4, 4, None, 0, Gd, 4, out, work), cos.COS_EUNSUPPORTED),
+    Gd4 = torch.zeros((4 * n * n, 4), dtype=torch.float64, device="cuda")     # the binding checks tensor sizes first
+    for args, code in (((n, 4, 4, None, 0, Gd4, 4, out, work), cos.COS_EUNSUPPORTED),
                        ((n, 3, 2, None, 0, Gd, 4, out, work), cos.COS_EINVAL),
                        ((n, 3, 3, None, 7, Gd, 4, out, work), cos.COS_EINVAL),
                        ((n, 3, 3, None, 1, Gd, 4, out, work[:8]), cos.COS_EINVAL),
