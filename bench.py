@@ -56,7 +56,6 @@ def parse_args():
     ap.add_argument("--no-other-workloads", action="store_true",
                     help="skip the short timings of the other BASELINE configurations (other_workloads block)")
     ap.add_argument("--layers", action="store_true", help="print the per-layer table to stderr")
-    ap.add_argument("--build-flags", type=int, default=0, help="extra cos_build_ex flags (e.g. 8 = COS_BUILD_PAIR_ROWS)")
     ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
                     help="launch tuning through cos_set_tuning (prefetch, warps_per_cta, blocks_per_cta_cap, pdl, ...)")
     ap.add_argument("--route", default="dag", choices=["dag", "det"],
@@ -295,7 +294,7 @@ def run_ours(args):
     v = draw_vertices(w)
     tab = cos.cos_tab_build(w.lattice, w.L, table.n_blocks, w.beta, w.n_tau, table.data)
     t0 = time.perf_counter()
-    h = cos.cos_build_ex(w.n, w.n_flavors, w.lattice, w.sigmas, w.n if w.all_subsets else 0, args.build_flags)
+    h = cos.cos_build(w.n, w.n_flavors, w.lattice, w.sigmas, w.n if w.all_subsets else 0)
     build_s = time.perf_counter() - t0
     for kv in args.tune:
         k, val = kv.split("=")

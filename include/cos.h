@@ -42,8 +42,7 @@ enum { COS_LATTICE_SQUARE = 0, COS_LATTICE_HONEYCOMB = 1 };
 enum {
     COS_BUILD_HOST_ONLY = 1,       /* compile the DAG, do not touch CUDA (cos_eval then fails) */
     COS_BUILD_NO_FUSED = 2,        /* small DAGs: use the per-layer kernels instead of the single fused launch */
-    COS_BUILD_UNIFORM_SHIFT = 4,   /* uniform CoS WITH a counterterm: shifts[0] = sigma = alpha/U (see cos_build) */
-    COS_BUILD_PAIR_ROWS = 8        /* pair records: two heads of a block and colour share their factor loads (Eq. 29-31) */
+    COS_BUILD_UNIFORM_SHIFT = 4    /* uniform CoS WITH a counterterm: shifts[0] = sigma = alpha/U (see cos_build) */
 };
 
 /* ---- (1) DAG compiler: PAPER.md:160-265 (canonical keys Eq. 17, 79-80; pruning Eq. 19-24) ----------

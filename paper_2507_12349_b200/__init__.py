@@ -4,7 +4,7 @@ kernels of libcos_b200.so.  There is no CPU fallback and this package never impo
 """
 from ._binding import (  # noqa: F401
     COS_OK, COS_EINVAL, COS_ENOMEM, COS_ECUDA, COS_EUNSUPPORTED,
-    COS_LATTICE_SQUARE, COS_LATTICE_HONEYCOMB, COS_BUILD_HOST_ONLY, COS_BUILD_NO_FUSED, COS_BUILD_UNIFORM_SHIFT, COS_BUILD_PAIR_ROWS,
+    COS_LATTICE_SQUARE, COS_LATTICE_HONEYCOMB, COS_BUILD_HOST_ONLY, COS_BUILD_NO_FUSED, COS_BUILD_UNIFORM_SHIFT,
     COS_DET_FP64, COS_DET_DD, INFO, TUNE, cos_reserve, cos_set_tuning, cos_debug_check_failures, cos_equivalence_stats,
     CosError, lib_path, load_library,
     cos_build, cos_build_ex, cos_eval, cos_free, cos_info, cos_last_error, cos_set_workspace_limit,

@@ -14,7 +14,7 @@ _lib = None
 
 COS_OK, COS_EINVAL, COS_ENOMEM, COS_ECUDA, COS_EUNSUPPORTED = 0, 1, 2, 3, 4
 COS_LATTICE_SQUARE, COS_LATTICE_HONEYCOMB = 0, 1
-COS_BUILD_HOST_ONLY, COS_BUILD_NO_FUSED, COS_BUILD_UNIFORM_SHIFT, COS_BUILD_PAIR_ROWS = 1, 2, 4, 8
+COS_BUILD_HOST_ONLY, COS_BUILD_NO_FUSED, COS_BUILD_UNIFORM_SHIFT = 1, 2, 4
 COS_DET_FP64, COS_DET_DD = 0, 1
 TUNE = {"prefetch": 0, "warps_per_cta": 1, "blocks_per_cta_cap": 2, "pdl": 3, "fused": 4, "host_slices": 5,
         "tiles_per_chunk": 6}

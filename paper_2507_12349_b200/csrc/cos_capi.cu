@@ -112,8 +112,7 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
 
     cos_handle_s* h = new (std::nothrow) cos_handle_s();
     if (!h) return fail(COS_ENOMEM, "cos_build: out of host memory");
-    std::string err = compile_dag(n, n_flavors, nsub, shifts, uniform_shift, readout_envelope == n, order_mask, h->dag, nullptr,
-                                  (flags & COS_BUILD_PAIR_ROWS) != 0);
+    std::string err = compile_dag(n, n_flavors, nsub, shifts, uniform_shift, readout_envelope == n, order_mask, h->dag);
     if (!err.empty()) {
         delete h;
         return fail(is_unsupported(err) ? COS_EUNSUPPORTED : COS_ENOMEM, "cos_build: " + err);

@@ -83,7 +83,7 @@ struct Builder {
 }  // namespace
 
 std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool uniform_shift, bool all_subsets,
-                        uint32_t order_mask, CompiledDag& out, EquivalenceStats* eq, bool pair_rows)
+                        uint32_t order_mask, CompiledDag& out, EquivalenceStats* eq)
 {
     const bool uniform = (sigma == nullptr) || uniform_shift;
     if (n < 1 || n > 12) return "n must be in [1, 12]";
@@ -337,48 +337,19 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                     out_idx = all_subsets ? b.full_set(code) - 1u : 0u;
                 }
                 const bool need_close = flags != 0;
-                uint32_t Lmax = 0;
-                int heads[24], n_heads = 0;
+                uint32_t n_rows = 0, Lmax = 0;
                 for (int h = 0; h < d; ++h) {
                     const uint32_t a = b.alive[(size_t)id * d + h];
-                    if (a) { heads[n_heads++] = h; Lmax = std::max(Lmax, (uint32_t)__builtin_popcount(a)); }
+                    if (a) { n_rows += nc; Lmax = std::max(Lmax, (uint32_t)__builtin_popcount(a)); }
                 }
-                int32_t dest[24];
-                for (int q = 0; q < nJ; ++q) dest[q] = b.index_of[J[q].dest_code];
-                auto live = [&](int h, int q) {
-                    return dest[q] >= 0 && ((b.alive[(size_t)dest[q] * d + h] >> J[q].j_a) & 1u);
-                };
-                // Pair records (factor-application sharing, Eq. 29-31): two heads of the block share, colour by
-                // colour, every factor load G_lambda[e][j] -- it does not depend on the head.  Consecutive heads are paired
-                // when their union of destination endpoints fits the kernel's 2 x PAIR_MAX_COLS register tile.
-                struct Pair { int h1, h2; int cols[PAIR_MAX_COLS + 1]; int n_cols; };
-                std::vector<Pair> pairs;
-                std::vector<int> singles;
-                for (int k = 0; k < n_heads;) {
-                    bool paired = false;
-                    if (pair_rows && k + 1 < n_heads) {
-                        Pair pr; pr.h1 = heads[k]; pr.h2 = heads[k + 1]; pr.n_cols = 0;
-                        bool fits = true;
-                        for (int q = 0; q < nJ && fits; ++q)
-                            if (live(pr.h1, q) || live(pr.h2, q)) {
-                                if (pr.n_cols == PAIR_MAX_COLS) fits = false; else pr.cols[pr.n_cols++] = q;
-                            }
-                        if (fits) { pairs.push_back(pr); paired = true; }
-                    }
-                    if (paired) k += 2; else singles.push_back(heads[k++]);
-                }
-                uint32_t pair_cols = 0;
-                for (const Pair& pr : pairs) pair_cols = std::max(pair_cols, std::max(2u, (uint32_t)((pr.n_cols + 1) & ~1)));
-                const uint32_t n_rows = (uint32_t)(singles.size() + pairs.size()) * nc;
-                const uint32_t e_words = (Lmax + 3) / 4;
-                const uint32_t stride = std::max(singles.empty() ? 0u : 2 + e_words + (uint32_t)nJ,
-                                                 pairs.empty() ? 0u : (uint32_t)PAIR_HDR_WORDS + 2u * pair_cols);
+                const uint32_t e_words = (Lmax + 3) / 4, stride = 2 + e_words + (uint32_t)nJ;
                 if (stride > 32) return "unsupported: row record exceeds 32 words";
                 if (P.words.size() + HDR + (size_t)n_rows * stride >= 0xFFFFFFFFull) return "unsupported: layer program exceeds 2^32 words";
                 P.mask_off.push_back((uint32_t)P.words.size());
                 {   // first state of the block in the layer slab (block states are contiguous)
                     uint32_t first = P.n_states;
-                    if (n_heads) first = b.row_base[(size_t)id * d + heads[0]];
+                    for (int h = 0; h < d; ++h)
+                        if (b.alive[(size_t)id * d + h]) { first = b.row_base[(size_t)id * d + h]; break; }
                     P.mask_off.push_back(first);
                 }
                 P.words.push_back(n_rows | ((uint32_t)nJ << 16) | (flags << 24));
@@ -389,66 +360,13 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                 for (int lam = 0; lam < nc; ++lam)
                     P.words.push_back((flags & FLAG_FRESH) ? b.state_index((uint32_t)fresh_did, (int)fresh_a, lam, (int)fresh_a)
                                                             : DIDX_DEAD);
-                // per-row bookkeeping (edge counts of SURVEY's tables) -- independent of the record form
-                for (int k = 0; k < n_heads; ++k) {
-                    const int h = heads[k];
+                int32_t dest[24];
+                for (int q = 0; q < nJ; ++q) dest[q] = b.index_of[J[q].dest_code];
+                for (int h = 0; h < d; ++h) {
                     const uint32_t a = b.alive[(size_t)id * d + h];
+                    if (!a) continue;
                     const uint32_t L = (uint32_t)__builtin_popcount(a);
                     for (int lam = 0; lam < nc; ++lam) {
-                        for (int q = 0; q < nJ; ++q)
-                            if (live(h, q)) { if (J[q].mult2) P.e1 += L; else P.e2 += L; }
-                        if (b.has_shift && l + 1 < NL)      // E3: states whose current interaction is singly occupied
-                            for (int e = 0; e < d; ++e)
-                                if (((a >> e) & 1u)) { int c = Builder::cell(code, e / nsub); if (c == 1 || c == 2) P.e3 += 1; }
-                        if (flags & FLAG_FRESH) P.e4 += (uint64_t)L * nc;
-                        if (flags & FLAG_READOUT) P.readout_edges += L;
-                    }
-                }
-                for (const Pair& pr : pairs) {
-                    const uint32_t a1 = b.alive[(size_t)id * d + pr.h1], a2 = b.alive[(size_t)id * d + pr.h2];
-                    const uint32_t L1 = (uint32_t)__builtin_popcount(a1), L2 = (uint32_t)__builtin_popcount(a2);
-                    const uint32_t Lu = (uint32_t)__builtin_popcount(a1 | a2);
-                    for (int lam = 0; lam < nc; ++lam) {
-                        const size_t w_row = P.words.size();
-                        P.words.push_back(b.row_base[(size_t)id * d + pr.h1] + (uint32_t)lam * L1);
-                        P.words.push_back(0u);           // header, filled below
-                        P.words.push_back(b.row_base[(size_t)id * d + pr.h2] + (uint32_t)lam * L2);
-                        P.words.push_back((uint32_t)pr.h1 | ((uint32_t)pr.h2 << 5));
-                        P.words.push_back(a1);
-                        P.words.push_back(a2);
-                        uint32_t has_defer = 0, defer_head = 0, defer_col = 0;
-                        for (int c = 0; c < pr.n_cols; ++c) {
-                            const int q = pr.cols[c];
-                            for (int t = 0; t < 2; ++t) {
-                                const int h = t ? pr.h2 : pr.h1;
-                                uint32_t w = DIDX_MASK;          // dead for this head
-                                if (live(h, q)) {
-                                    if ((flags & FLAG_FRESH) && (uint32_t)h == fresh_a && J[q].j_a == fresh_a) {
-                                        has_defer = 1; defer_head = (uint32_t)t; defer_col = (uint32_t)c;
-                                    } else w = b.state_index((uint32_t)dest[q], h, lam, J[q].j_a);
-                                }
-                                P.words.push_back(w | ((uint32_t)J[q].j_a << 24));
-                            }
-                        }
-                        // an even number of columns, at least two: padding columns repeat the last endpoint, both heads dead
-                        const uint32_t tj = std::max(2u, (uint32_t)((pr.n_cols + 1) & ~1));
-                        for (uint32_t c = (uint32_t)pr.n_cols; c < tj; ++c) {
-                            const uint32_t ja = pr.n_cols ? (uint32_t)J[pr.cols[pr.n_cols - 1]].j_a : 0u;
-                            P.words.push_back(DIDX_MASK | (ja << 24));
-                            P.words.push_back(DIDX_MASK | (ja << 24));
-                        }
-                        while (P.words.size() - w_row < stride) P.words.push_back(0u);
-                        P.words[w_row + 1] = Lu | ((uint32_t)lam << 10) | (defer_col << 12) | (tj << 17) | (has_defer << 22) |
-                                             (defer_head << 23) | ROW_PAIR;
-                        P.n_fma += (uint64_t)2 * Lu * tj + (need_close ? L1 + L2 : 0u);
-                        ++P.n_pairs;
-                    }
-                }
-                for (int h : singles) {
-                    const uint32_t a = b.alive[(size_t)id * d + h];
-                    const uint32_t L = (uint32_t)__builtin_popcount(a);
-                    for (int lam = 0; lam < nc; ++lam) {
-                        const size_t w_row = P.words.size();
                         P.words.push_back(b.row_base[(size_t)id * d + h] + (uint32_t)lam * L);
                         const uint32_t kh = ((a >> h) & 1u) ? (uint32_t)__builtin_popcount(a & ((1u << h) - 1u)) : 31u;
                         const size_t w_hdr = P.words.size();
@@ -461,7 +379,9 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                         // live destinations only (pruned ones are dropped), the merged E2/E4 destination last
                         uint32_t n_live = 0, defer_word = 0, has_defer = 0;
                         for (int q = 0; q < nJ; ++q) {
-                            if (!live(h, q)) continue;
+                            const bool live = dest[q] >= 0 && ((b.alive[(size_t)dest[q] * d + h] >> J[q].j_a) & 1u);
+                            if (!live) continue;
+                            if (J[q].mult2) P.e1 += L; else P.e2 += L;
                             if ((flags & FLAG_FRESH) && (uint32_t)h == fresh_a && J[q].j_a == fresh_a) {
                                 has_defer = 1; defer_word = (uint32_t)J[q].j_a << 24;
                                 continue;
@@ -470,18 +390,24 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                             ++n_live;
                         }
                         if (has_defer) P.words.push_back(defer_word);
-                        while (P.words.size() - w_row < stride) P.words.push_back(0u);
+                        for (uint32_t q = n_live + has_defer; q < (uint32_t)nJ; ++q) P.words.push_back(0u);
                         P.words[w_hdr] = L | ((uint32_t)h << 5) | ((uint32_t)lam << 10) | (kh << 12) | (n_live << 17) | (has_defer << 22);
-                        P.n_fma += (uint64_t)L * (n_live + has_defer + (need_close ? 1u : 0u));
+                        const uint32_t alive_j = n_live + has_defer;
+                        if (b.has_shift && l + 1 < NL)      // E3: states whose current interaction is singly occupied
+                            for (int e = 0; e < d; ++e)
+                                if (((a >> e) & 1u)) { int c = Builder::cell(code, e / nsub); if (c == 1 || c == 2) P.e3 += 1; }
+                        if (flags & FLAG_FRESH) P.e4 += (uint64_t)L * nc;
+                        if (flags & FLAG_READOUT) P.readout_edges += L;
+                        P.n_fma += (uint64_t)L * (alive_j + (need_close ? 1u : 0u));
                     }
                 }
-                P.n_rows += (uint32_t)n_heads * nc;
+                P.n_rows += n_rows;
                 P.max_L = std::max(P.max_L, Lmax);
             }
             P.mask_off.push_back((uint32_t)P.words.size());
             P.mask_off.push_back(P.n_states);
             P.words.resize(P.words.size() + 64, 0u);          // padding: the kernel reads whole 32-word windows
-            out.n_states += P.n_states; out.n_masks += P.n_masks; out.n_rows += P.n_rows; out.n_pairs += P.n_pairs;
+            out.n_states += P.n_states; out.n_masks += P.n_masks; out.n_rows += P.n_rows;
             out.n_edges += P.e1 + P.e2 + P.e3 + P.e4; out.n_readout_edges += P.readout_edges; out.n_fma += P.n_fma;
             out.max_layer_states = std::max(out.max_layer_states, P.n_states);
             out.max_L = std::max(out.max_L, P.max_L);

@@ -35,21 +35,9 @@ namespace cosb {
 static const uint32_t DIDX_MASK = 0x00FFFFFFu;
 static const uint32_t DIDX_DEAD = 0x00FFFFFFu;     // fresh-head destination pruned (block header only)
 static const uint32_t FLAG_FRESH = 1u, FLAG_READOUT = 2u;
-// pair record (two heads h1 < h2 of one block and colour that share every factor load, Eq. 29-31); same stride
-// as the block's rows:
-//   w0 : slab index of head 1's first state      w2 : ... of head 2's
-//   w1 : L_u[0:5) (size of the union of the two endpoint sets) | lambda[10:12) | defer_col[12:17) | TJ[17:22) (destination
-//        columns, even: an odd count is padded with a dead column) | defer[22] | defer_head[23] | ROW_PAIR[31]
-//        (defer: the value of (defer_head, defer_col) merges with the fresh-head state instead of being stored)
-//   w3 : h1_a[0:5) | h2_a[5:10)
-//   w4 : live endpoints of head 1 (bit e_a)      w5 : ... of head 2
-//   w6.. : TJ x 2 words, column by column: dj of head 1, dj of head 2 (didx = DIDX_MASK: not live for that head)
-static const uint32_t ROW_PAIR = 0x80000000u;
-static const int PAIR_HDR_WORDS = 6;
-static const int PAIR_MAX_COLS = 6;                // 2 x 6 register tile of the kernel
 
 struct LayerProgram {
-    uint32_t n_states = 0, n_masks = 0, n_rows = 0, n_pairs = 0, max_L = 0;
+    uint32_t n_states = 0, n_masks = 0, n_rows = 0, max_L = 0;
     std::vector<uint32_t> words;
     std::vector<uint32_t> mask_off;      // [n_masks + 1][2]: {word offset of the block header, first state of the block}
     uint64_t e1 = 0, e2 = 0, e3 = 0, e4 = 0, readout_edges = 0, n_fma = 0;
@@ -62,7 +50,7 @@ struct CompiledDag {
     double sigma[4] = {0, 0, 0, 0};
     double kappa = 1.0;
     std::vector<LayerProgram> layers;    // 2n layers; layer l holds the transitions l -> l+1 and the readouts at l
-    uint64_t n_states = 0, n_states_unpruned = 0, n_masks = 0, n_rows = 0, n_pairs = 0, n_edges = 0, n_readout_edges = 0, n_fma = 0;
+    uint64_t n_states = 0, n_states_unpruned = 0, n_masks = 0, n_rows = 0, n_edges = 0, n_readout_edges = 0, n_fma = 0;
     uint32_t max_layer_states = 0, max_L = 0;
     int hdr_words() const { return 3 + nc; }
 };
@@ -84,6 +72,6 @@ struct EquivalenceStats {
 // order_mask (all_subsets only): bit k set <=> subsets of order k are requested outputs (0 = every order).
 // eq != nullptr: additionally fill the equivalence statistics (host time and memory ~ the edge count; <= 6e7 states).
 std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool uniform_shift, bool all_subsets,
-                        uint32_t order_mask, CompiledDag& out, EquivalenceStats* eq = nullptr, bool pair_rows = false);
+                        uint32_t order_mask, CompiledDag& out, EquivalenceStats* eq = nullptr);
 
 }  // namespace cosb

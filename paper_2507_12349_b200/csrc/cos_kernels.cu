@@ -24,7 +24,7 @@ namespace cosb {
 static const int MAX_WARPS = 16;
 // CTA size bound per instantiation: the long-row kernels (honeycomb, d = 20) are shared-memory limited to one CTA
 // per SM, so they take 24 warps (<= 85 registers) instead of 16.
-__host__ __device__ constexpr int max_warps_of(int maxl) { return maxl == 20 ? 20 : maxl <= 12 ? 24 : MAX_WARPS; }
+__host__ __device__ constexpr int max_warps_of(int maxl) { return maxl == 20 ? 20 : MAX_WARPS; }
 
 __device__ __forceinline__ double lds64(uint32_t addr)
 {
@@ -155,118 +155,6 @@ __device__ __forceinline__ void row_body(const uint32_t rw, const uint32_t rh, c
     }
 }
 
-// ------------------------------------------------------------------------------------------------------
-// One PAIR record (cos_compile.h): two heads of a block and colour share every factor load (factor-application sharing,
-// PAPER.md Eq. 29-31: G_lambda[e][j] does not depend on the head), Y[t][j] = sum_e X[t][e] * G_lambda[e][j] for t = 0, 1
-// on a 2 x TJ register tile.  The source values stream through COS_PAIR_STAGES statically named register stages: the
-// loads of union endpoint k + STAGES - 1 are in flight while endpoint k is applied (a head without that state contributes
-// x = 0).  The record words are broadcast with shuffles like a row's.
-#ifndef COS_PAIR_STAGES
-#define COS_PAIR_STAGES 3
-#endif
-template <int TJ, int NC, bool SHIFT, bool FUSED>
-__device__ __forceinline__ void pair_body(const uint32_t rw, const uint32_t rh, const char* __restrict__ Xl,
-                                          const bool need_close, const uint32_t d, const uint32_t gs_lane,
-                                          const uint32_t gd_lane, char* __restrict__ Yb, double& close, double (&sp)[NC])
-{
-    constexpr int D = COS_PAIR_STAGES;
-    const uint32_t lam = (rh >> 10) & 3u;
-    uint32_t idx[2], al[2], hoff[2];
-    idx[0] = __shfl_sync(0xFFFFFFFFu, rw, 0); idx[1] = __shfl_sync(0xFFFFFFFFu, rw, 2);
-    {
-        const uint32_t w3 = __shfl_sync(0xFFFFFFFFu, rw, 3);
-        hoff[0] = (w3 & 31u) << 8; hoff[1] = ((w3 >> 5) & 31u) << 8;
-    }
-    al[0] = __shfl_sync(0xFFFFFFFFu, rw, 4); al[1] = __shfl_sync(0xFFFFFFFFu, rw, 5);
-    const uint32_t dstride = d * (TILE * 8u);
-    const uint32_t row0 = gs_lane + lam * d * dstride;
-    const uint32_t gdl = gd_lane + ((lam * d) << 8);
-    uint32_t colq[TJ];                       // column j of table row 0 of this colour
-#pragma unroll
-    for (int q = 0; q < TJ; ++q)
-        colq[q] = row0 + __byte_perm(__shfl_sync(0xFFFFFFFFu, rw, PAIR_HDR_WORDS + 2 * q), 0u, 0x4434u);   // + j_a * 256
-    double acc[2][TJ];
-#pragma unroll
-    for (int q = 0; q < TJ; ++q) { acc[0][q] = 0.0; acc[1][q] = 0.0; }
-    double cl = 0.0;
-    uint32_t em = al[0] | al[1];
-    uint32_t bq[D];
-    double xs[D][2];
-#pragma unroll
-    for (int s = 0; s < D; ++s) {
-        bq[s] = em & (0u - em);                        // 0 after the last endpoint: nothing is loaded then
-        em ^= bq[s];
-#pragma unroll
-        for (int t = 0; t < 2; ++t) {
-            xs[s][t] = 0.0;
-            if (al[t] & bq[s]) {
-                const double* p = (const double*)(Xl + ((size_t)idx[t] << 8));
-                xs[s][t] = FUSED ? __ldcg(p) : __ldcs(p);
-                ++idx[t];
-            }
-        }
-    }
-    bool live = true;
-    while (live) {
-#pragma unroll
-        for (int s = 0; s < D; ++s) {
-            if (live) {
-                const uint32_t e = 31u - (uint32_t)__clz((int)bq[s]);
-                const uint32_t ro = e * dstride;
-                double g[TJ];
-#pragma unroll
-                for (int q = 0; q < TJ; ++q) g[q] = lds64(colq[q] + ro);
-#pragma unroll
-                for (int q = 0; q < TJ; ++q) {
-                    acc[0][q] = fma(g[q], xs[s][0], acc[0][q]);
-                    acc[1][q] = fma(g[q], xs[s][1], acc[1][q]);
-                }
-                if (need_close) {    // closing factor G_lambda[e][h] per head (Eq. 12, 15), never shifted; x = 0 if absent
-#pragma unroll
-                    for (int t = 0; t < 2; ++t) {
-                        uint32_t p = row0 + ro + hoff[t];
-                        if (SHIFT) p = (hoff[t] == (e << 8)) ? gdl + hoff[t] : p;
-                        cl = fma(lds64(p), xs[s][t], cl);
-                    }
-                }
-                bq[s] = em & (0u - em);
-                em ^= bq[s];
-#pragma unroll
-                for (int t = 0; t < 2; ++t) {
-                    xs[s][t] = 0.0;
-                    if (al[t] & bq[s]) {
-                        const double* p = (const double*)(Xl + ((size_t)idx[t] << 8));
-                        xs[s][t] = FUSED ? __ldcg(p) : __ldcs(p);
-                        ++idx[t];
-                    }
-                }
-                live = bq[(s + 1) % D] != 0u;
-            }
-        }
-    }
-    if (need_close) close += cl;
-#pragma unroll
-    for (int q = 0; q < TJ; ++q)
-#pragma unroll
-        for (int t = 0; t < 2; ++t) {
-            const uint32_t w = __shfl_sync(0xFFFFFFFFu, rw, PAIR_HDR_WORDS + 2 * q + t);
-            if ((w & DIDX_MASK) != DIDX_MASK) {
-                double* y = (double*)(Yb + (size_t)(w << 8));             // didx * 256 bytes: the shift drops j_a
-                if (FUSED) *y = acc[t][q]; else __stcs(y, acc[t][q]);
-            }
-        }
-    if ((rh >> 22) & 1u) {                  // the destination that merges with the fresh-head state (E2/E4 pair)
-        const uint32_t sel = ((rh >> 12) & 31u) * 2u + ((rh >> 23) & 1u);
-        double v = 0.0;
-#pragma unroll
-        for (int q = 0; q < TJ; ++q)
-#pragma unroll
-            for (int t = 0; t < 2; ++t) v = (sel == (uint32_t)(2 * q + t)) ? acc[t][q] : v;
-#pragma unroll
-        for (int c = 0; c < NC; ++c) sp[c] = ((uint32_t)c == lam) ? v : sp[c];
-    }
-}
-
 // All source blocks [m_begin, m_end) of one layer for one batch tile: the body shared by the per-layer kernel and the
 // fused small-DAG kernel.  s_next (shared) must be 0 and visible to the CTA on entry.
 template <int MAXL, int NC, bool SHIFT, bool FUSED>
@@ -323,18 +211,7 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
             const uint32_t base = __shfl_sync(0xFFFFFFFFu, rw, 0), rh = __shfl_sync(0xFFFFFFFFu, rw, 1);
             const int L = (int)(rh & 31u);
 #ifdef COS_CHECK_BOUNDS
-            if (rh & ROW_PAIR) {
-                const uint32_t tj = (rh >> 17) & 31u;
-                const uint32_t b1 = __shfl_sync(0xFFFFFFFFu, rw, 0), b2 = __shfl_sync(0xFFFFFFFFu, rw, 2);
-                const uint32_t a1 = __shfl_sync(0xFFFFFFFFu, rw, 4), a2 = __shfl_sync(0xFFFFFFFFu, rw, 5);
-                const uint32_t w3 = __shfl_sync(0xFFFFFFFFu, rw, 3);
-                COS_CHECK((size_t)b1 + __popc(a1) <= (size_t)a.S_src && (size_t)b2 + __popc(a2) <= (size_t)a.S_src, 1);
-                COS_CHECK(tj >= 2u && tj <= (uint32_t)PAIR_MAX_COLS && !(tj & 1u) && PAIR_HDR_WORDS + 2 * (int)tj <= stride &&
-                          __popc(a1 | a2) == L && ((a1 | a2) >> a.d) == 0u, 2);
-                if (lane >= PAIR_HDR_WORDS && lane < PAIR_HDR_WORDS + 2 * (int)tj)
-                    COS_CHECK(((rw & DIDX_MASK) == DIDX_MASK || (rw & DIDX_MASK) < a.S_dst) && (rw >> 24) < (uint32_t)a.d, 3);
-                COS_CHECK((w3 & 31u) < (uint32_t)a.d && ((w3 >> 5) & 31u) < (uint32_t)a.d && ((rh >> 10) & 3u) < (uint32_t)NC, 5);
-            } else {
+            {
                 const int n_dst = (int)((rh >> 17) & 31u) + (int)((rh >> 22) & 1u);
                 COS_CHECK(L >= 1 && L <= MAXL && (size_t)base + L <= (size_t)a.S_src, 1);              // source row
                 COS_CHECK(n_dst <= nJ && (((rh >> 12) & 31u) == 31u || (int)((rh >> 12) & 31u) < L), 2);
@@ -353,14 +230,6 @@ __device__ __forceinline__ void layer_blocks(const LayerArgs& a, const uint32_t 
                     if (st < a.S_src) prefetch_l2(Xt0 + (size_t)st * (TILE * 8) + (size_t)(q & 1) * 128);
                 }
             }
-            if (rh & ROW_PAIR) {             // two heads sharing their factor loads
-                switch ((rh >> 17) & 31u) {
-                    case 2: pair_body<2, NC, SHIFT, FUSED>(rw, rh, (const char*)Xt, need_close, (uint32_t)a.d, gs_lane, gd_lane, (char*)Yt, close, sp); break;
-                    case 4: pair_body<4, NC, SHIFT, FUSED>(rw, rh, (const char*)Xt, need_close, (uint32_t)a.d, gs_lane, gd_lane, (char*)Yt, close, sp); break;
-                    case 6: pair_body<6, NC, SHIFT, FUSED>(rw, rh, (const char*)Xt, need_close, (uint32_t)a.d, gs_lane, gd_lane, (char*)Yt, close, sp); break;
-                    default: break;
-                }
-            } else
 #define COS_ROW_CASE(LL)                                                                                        \
     case LL:                                                                                                    \
         if (LL <= MAXL)                                                                                         \

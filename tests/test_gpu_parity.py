@@ -20,7 +20,6 @@ pytestmark = pytest.mark.gpu
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 TOL = 1e-10
-EXTRA_BUILD_FLAGS = int(os.environ.get("COS_TEST_BUILD_FLAGS", "0"))      # e.g. 8: every gpu_eval case with pair records
 
 
 @pytest.fixture(scope="module")
@@ -37,7 +36,7 @@ def gpu_eval(cos, G, n, n_flavors, lattice, sigmas, all_subsets, ws_limit=None, 
     """G: numpy [n_blocks][d][d][B] -> numpy [n_out][B] through cos_build / cos_eval / cos_free."""
     import torch
     B = G.shape[-1]
-    h = cos.cos_build_ex(n, n_flavors, lattice, sigmas, n if all_subsets else 0, flags | EXTRA_BUILD_FLAGS)
+    h = cos.cos_build_ex(n, n_flavors, lattice, sigmas, n if all_subsets else 0, flags)
     try:
         if ws_limit is not None:
             cos.cos_set_workspace_limit(h, ws_limit)
