@@ -240,6 +240,36 @@ int cos_det_eval(int n, int n_flavors, int n_blocks, int lattice, const double* 
                  const double* G_dev, long long batch, double* out_dev, void* work_dev, long long work_bytes,
                  cos_stream stream);
 
+/* ---- the same route for callers that must not allocate device memory ------------------------------------------
+ * cos_det_eval needs a scratch buffer, and somebody has to cudaMalloc it.  Some users of this library cannot: a
+ * Monte-Carlo sampler whose steady-state loop may not contain a call that stalls the whole device (cudaMalloc and
+ * cudaFree synchronise it), a plug-in running inside a host program that has already handed all free HBM to its own
+ * memory pool (a further cudaMalloc simply fails there) or that forbids driver allocations in its callbacks, and
+ * latency-bounded services where an allocation of unknown duration in the request path is not acceptable.
+ * cos_det_eval_static is cos_det_eval with the scratch taken from an array that is compiled into the library
+ * (a file-scope `static __device__` array of COS_DET_STATIC_SCRATCH_BYTES = 16 MiB): it calls neither cudaMalloc nor
+ * cudaFree nor any library routine that allocates, on any call.  The caller passes inputs and outputs only.
+ *   Arguments, layouts, precision, arithmetic and error codes: exactly those of cos_det_eval (same kernels, same
+ *   summation order -- the results are bit-identical to cos_det_eval on the same inputs).
+ *   Limit: cos_det_workspace_bytes(n, n_blocks, precision, batch) must not exceed COS_DET_STATIC_SCRATCH_BYTES, e.g.
+ *   fp64 with three blocks: batch <= 1638 at n = 8, <= 409 at n = 10; double-double: half of that.  Anything larger is
+ *   refused with COS_EUNSUPPORTED and a message naming both byte counts (split the batch, or use cos_det_eval with a
+ *   buffer of your own); nothing is launched in that case.
+ *   Cost: every GPU on which the library's CUDA code is loaded holds the 16 MiB until the process exits, used or not.
+ *   Set-up: the first call on a device looks up that device's address of the array (cudaGetSymbolAddress; once per
+ *   device, with the device that is current in the calling thread, remembered afterwards).  That first call may make
+ *   the CUDA runtime load the library's device code, so make it during initialisation and BEFORE any stream capture
+ *   is begun; later calls on that device only enqueue kernels.
+ *   Sharing: there is one array per device and every call on that device uses it.  Calls are ordered correctly when
+ *   they are enqueued on the same stream; two calls that can overlap on the GPU (different streams, or different host
+ *   threads with their own streams) race on the scratch and return garbage -- serialise them yourself.  The array keeps
+ *   whatever the previous call left in it; that is harmless here because every call writes each scratch element
+ *   (minors, moments, connected values, subset order) before it reads it, so nothing has to start at zero.
+ * Asynchronous on `stream`, like cos_det_eval. */
+#define COS_DET_STATIC_SCRATCH_BYTES (16ll << 20)
+int cos_det_eval_static(int n, int n_flavors, int n_blocks, int lattice, const double* shifts, int precision,
+                        const double* G_dev, long long batch, double* out_dev, cos_stream stream);
+
 /* ---- measurement helpers ------------------------------------------------------------------------------
  * cos_set_profiling(h, 1): every later cos_eval brackets each layer launch with CUDA events on its stream.
  * cos_get_layer_times synchronises on the recorded events, ADDS the elapsed milliseconds of layer l (summed over

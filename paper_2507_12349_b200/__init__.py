@@ -10,6 +10,6 @@ from ._binding import (  # noqa: F401
     cos_build, cos_build_ex, cos_eval, cos_free, cos_info, cos_last_error, cos_set_workspace_limit,
     cos_tab_build, cos_tabulate, cos_tab_free, cos_measure_fp64_fma_peak,
     cos_eval_host, cos_set_profiling, cos_get_layer_times, cos_build_orders, cos_flux_weights, EXPORTS,
-    cos_det_workspace_bytes, cos_det_eval,
+    cos_det_workspace_bytes, cos_det_eval, cos_det_eval_static, COS_DET_STATIC_SCRATCH_BYTES,
     dag_summary,
 )

@@ -16,6 +16,7 @@ COS_OK, COS_EINVAL, COS_ENOMEM, COS_ECUDA, COS_EUNSUPPORTED = 0, 1, 2, 3, 4
 COS_LATTICE_SQUARE, COS_LATTICE_HONEYCOMB = 0, 1
 COS_BUILD_HOST_ONLY, COS_BUILD_NO_FUSED, COS_BUILD_UNIFORM_SHIFT = 1, 2, 4
 COS_DET_FP64, COS_DET_DD = 0, 1
+COS_DET_STATIC_SCRATCH_BYTES = 16 << 20
 TUNE = {"prefetch": 0, "warps_per_cta": 1, "blocks_per_cta_cap": 2, "pdl": 3, "fused": 4, "host_slices": 5,
         "tiles_per_chunk": 6}
 
@@ -32,7 +33,7 @@ EXPORTS = [
     "cos_last_error", "cos_tab_build", "cos_tabulate", "cos_tab_free", "cos_measure_fp64_fma_peak",
     "cos_eval_host", "cos_set_profiling", "cos_get_layer_times", "cos_build_orders", "cos_flux_weights",
     "cos_det_workspace_bytes", "cos_det_eval", "cos_reserve", "cos_set_tuning", "cos_debug_check_failures",
-    "cos_equivalence_stats",
+    "cos_equivalence_stats", "cos_det_eval_static",
 ]
 
 
@@ -90,6 +91,8 @@ def load_library():
     lib.cos_det_workspace_bytes.argtypes = [ip, ip, ip, ctypes.c_longlong]
     lib.cos_det_eval.restype = ctypes.c_int
     lib.cos_det_eval.argtypes = [ip, ip, ip, ip, dp, ip, vp, ctypes.c_longlong, vp, vp, ctypes.c_longlong, vp]
+    lib.cos_det_eval_static.restype = ctypes.c_int
+    lib.cos_det_eval_static.argtypes = [ip, ip, ip, ip, dp, ip, vp, ctypes.c_longlong, vp, vp]
     lib.cos_measure_fp64_fma_peak.restype = ctypes.c_int
     lib.cos_measure_fp64_fma_peak.argtypes = [dp]
     lib.cos_equivalence_stats.restype = ctypes.c_int
@@ -173,6 +176,23 @@ def cos_det_eval(n, n_flavors, n_blocks, shifts, precision, G_dev, batch, out_de
         _dev_ptr(G_dev, "torch.float64", int(n_blocks) * d * d * int(batch), "G_dev"), int(batch),
         _dev_ptr(out_dev, "torch.float64", ((1 << int(n)) - 1) * int(batch), "out_dev"), work_dev.data_ptr(),
         int(work_dev.numel() * work_dev.element_size()), _stream_ptr(stream)))
+
+
+def cos_det_eval_static(n, n_flavors, n_blocks, shifts, precision, G_dev, batch, out_dev, stream=None,
+                        lattice=COS_LATTICE_SQUARE):
+    """cos_det_eval without a work buffer, for code that is not allowed to allocate device memory (a sampler loop that
+    must not stall the GPU on cudaMalloc, a plug-in inside a program whose own pool already owns all of HBM, a
+    latency-bounded service): the scratch is a 16 MiB array built into libcos_b200.so, so no call allocates anything.
+    Same arguments and bit-identical results as cos_det_eval; problems whose cos_det_workspace_bytes(...) exceeds
+    COS_DET_STATIC_SCRATCH_BYTES raise CosError(COS_EUNSUPPORTED).  All calls on a device share the one array: keep them
+    on one stream (overlapping calls race), and make the first call on each device during initialisation, before any
+    stream capture -- it looks up the array's device address.  See include/cos.h."""
+    keep, p = _shifts_arg(shifts)
+    d = int(n) * (2 if int(lattice) == COS_LATTICE_HONEYCOMB else 1)
+    _check(load_library().cos_det_eval_static(
+        int(n), int(n_flavors), int(n_blocks), int(lattice), p, int(precision),
+        _dev_ptr(G_dev, "torch.float64", int(n_blocks) * d * d * int(batch), "G_dev"), int(batch),
+        _dev_ptr(out_dev, "torch.float64", ((1 << int(n)) - 1) * int(batch), "out_dev"), _stream_ptr(stream)))
 
 
 def cos_build(n, n_flavors, lattice, shifts, readout_envelope):

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -658,6 +659,57 @@ int cos_det_eval(int n, int n_flavors, int n_blocks, int lattice, const double* 
     cudaError_t e = launch_det_route(a, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, "cos_det_eval: launch");
     return COS_OK;
+}
+
+// ---- cos_det_eval for callers that cannot allocate device memory (include/cos.h) ---------------------------------
+// The scratch of the determinant route lives in this array instead of a caller's cudaMalloc'd buffer.  The name is
+// usable as an address in DEVICE code only; on the host it is a stand-in object of the host program, so the launcher
+// asks the runtime for the device address (cudaGetSymbolAddress), once per device, and hands that to the kernels.
+static __device__ __align__(256) unsigned char g_det_static_scratch[COS_DET_STATIC_SCRATCH_BYTES];
+
+namespace {
+constexpr int kMaxStaticDevices = 64;
+std::mutex g_det_static_mutex;
+void* g_det_static_ptr[kMaxStaticDevices] = {};      // device address of g_det_static_scratch, per CUDA device
+
+// Address of the array on the device that is current in this thread; looked up on the first call per device.
+int det_static_scratch(void** ptr)
+{
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cos_det_eval_static: cudaGetDevice");
+    if (dev < 0 || dev >= kMaxStaticDevices) return fail(COS_EUNSUPPORTED, "cos_det_eval_static: device ordinal above 63");
+    std::lock_guard<std::mutex> lock(g_det_static_mutex);
+    if (!g_det_static_ptr[dev]) {
+        void* p = nullptr;
+        e = cudaGetSymbolAddress(&p, g_det_static_scratch);
+        if (e != cudaSuccess) return cuda_fail(e, "cos_det_eval_static: cudaGetSymbolAddress");
+        if (!p || ((size_t)p & 255u) != 0) return fail(COS_ECUDA, "cos_det_eval_static: bad address of the scratch array");
+        g_det_static_ptr[dev] = p;
+    }
+    *ptr = g_det_static_ptr[dev];
+    return COS_OK;
+}
+}  // namespace
+
+int cos_det_eval_static(int n, int n_flavors, int n_blocks, int lattice, const double* shifts, int precision,
+                        const double* G_dev, long long batch, double* out_dev, cos_stream stream)
+{
+    const long long need = cos_det_workspace_bytes(n, n_blocks, precision, batch);
+    if (need > COS_DET_STATIC_SCRATCH_BYTES)
+        return fail(COS_EUNSUPPORTED, "cos_det_eval_static: this problem needs " + std::to_string(need) +
+                    " bytes of scratch, the built-in array holds " + std::to_string((long long)COS_DET_STATIC_SCRATCH_BYTES) +
+                    "; split the batch or call cos_det_eval with a buffer of your own");
+    // bad arguments (need < 0) and the empty batch never touch the scratch: cos_det_eval reports / returns before it
+    // looks at the buffer
+    if (need < 0 || batch == 0)
+        return cos_det_eval(n, n_flavors, n_blocks, lattice, shifts, precision, G_dev, batch, out_dev, nullptr, 0, stream);
+    void* scratch = nullptr;
+    const int rc = det_static_scratch(&scratch);
+    if (rc != COS_OK) return rc;
+    // from here on: argument checks and kernel launches only (cos_det_eval allocates nothing)
+    return cos_det_eval(n, n_flavors, n_blocks, lattice, shifts, precision, G_dev, batch, out_dev, scratch,
+                        COS_DET_STATIC_SCRATCH_BYTES, stream);
 }
 
 int cos_equivalence_stats(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope, int flags,
