@@ -17,6 +17,7 @@
 #include <algorithm>
 #include <cstring>
 #include <map>
+#include <utility>
 
 namespace cosb {
 namespace {
@@ -260,8 +261,12 @@ std::string compile_dag(int n, int nf, int nsub, const double* sigma, bool unifo
                     }
                 }
             eq->n_states = S; eq->n_edges = edges.size() + readouts.size();
-            auto key = [](uint32_t label, int32_t coeff, uint32_t cls) {
-                return ((uint64_t)label << 40) | ((uint64_t)(uint32_t)(coeff + 8) << 36) | (uint64_t)cls;
+            // operator symbol = (label, integer coefficient) pair, interned into a dense id (< 2^31: bit 63 marks readouts);
+            // the coefficient is a full int32 (-kappa = -N_f has no upper bound in uniform mode)
+            std::map<std::pair<uint32_t, int32_t>, uint32_t> symbols;
+            auto key = [&symbols](uint32_t label, int32_t coeff, uint32_t cls) {
+                const auto it = symbols.emplace(std::make_pair(label, coeff), (uint32_t)symbols.size()).first;
+                return ((uint64_t)it->second << 32) | (uint64_t)cls;
             };
             // future classes (Eq. 25-26): last layer first; signature = sorted (label, coefficient, class of the child)
             std::vector<std::vector<uint64_t>> sig(S);

@@ -231,5 +231,11 @@ def test_future_and_past_equivalence_classes(cos):
     assert r["future_classes"] == r["states"] == 2292 and r["past_classes"] == 2233
     r = cos.cos_equivalence_stats(5, 3, 0, [0.4], 0, flags=cos.COS_BUILD_UNIFORM_SHIFT)
     assert r["future_classes"] == r["states"] == r["past_classes"]
+    # the fresh-head coefficient -N_f is kept as a full integer in the signature: many flavours (uniform mode has no upper
+    # bound on N_f) must give the same class structure as two flavours, not spurious merges
+    base = cos.cos_equivalence_stats(5, 2, 0, None, 0)
+    for nf in (9, 40, 100000):
+        r = cos.cos_equivalence_stats(5, nf, 0, None, 0)
+        assert r == base and r["future_classes"] == r["states"] == r["past_classes"]
     with pytest.raises(cos.CosError):
         cos.cos_equivalence_stats(4, 2, 0, None, 3)
