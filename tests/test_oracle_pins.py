@@ -382,6 +382,31 @@ def test_determinant_route_precision_at_n10():
         assert abs(oracle.o2b_polynomial(As, None)[-1] - b) <= 1e-10 * M
 
 
+# ---------------------------------------------------------------- the tolerance scale of the n = 10 GPU tests
+@pytest.mark.parametrize("n_sub", [1, 2])
+def test_m_lower_bound_is_below_M(n_sub):
+    """The two full-size n = 10 GPU parity tests (cfg4, cfg3) cannot afford the true cancellation scale M (O1 / O3 with
+    absolute=True) and use test_gpu_parity.M_lower_bound / test_gpu_parity_wide._m_lower_sb instead, claimed to be
+    <= M (which makes those tests stricter).  Pinned here on small orders against the definition itself (O1,
+    absolute=True: every connected typed contraction of Eq. 58-63 with |weight|), square and honeycomb, two and three
+    flavours, random non-uniform matrices and shifts."""
+    from cos_workloads import random_matrices
+    from test_gpu_parity import M_lower_bound
+    from test_gpu_parity_wide import _m_lower_sb
+    rng = np.random.default_rng(77 + n_sub)
+    for n in ((2, 3, 4) if n_sub == 1 else (2, 3)):
+        for nf in (2, 3):
+            for rep in range(3):
+                sig = list(rng.standard_normal(nf) * 0.5)
+                G = random_matrices(7000 + 100 * n + 10 * nf + rep, nf, n * n_sub, 1, scale=0.8)[..., 0]
+                M = oracle.connected_reference(G, n, n_sub, nf, sig, uniform=False, all_subsets=False, tier="o1",
+                                               absolute=True)[0]
+                lb = M_lower_bound(G, n, n_sub, nf, False, n_assign=4, seed=rep)
+                assert 0.0 < lb <= M * (1 + 1e-12), (n, nf, n_sub, rep, lb, M)
+                if n_sub == 1:
+                    assert _m_lower_sb((G, nf)) == lb
+
+
 # ---------------------------------------------------------------- structural counts of the printed recurrences
 def test_readout_layers_and_counts():
     """2^n - 1 outputs, every one nonzero for a generic matrix."""
