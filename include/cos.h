@@ -103,8 +103,15 @@ int cos_equivalence_stats(int n, int n_flavors, int lattice, const double* shift
  *   stream   CUDA stream the kernels are enqueued on.  The call is asynchronous: it returns after
  *            enqueueing (launch errors only).  The handle owns the layer-slab workspace; one cos_eval in
  *            flight per handle.  After cos_reserve(h, B) every cos_eval with batch <= B only enqueues
- *            kernels (no allocation, no synchronisation: it can be captured into a CUDA graph); without
- *            it the workspace is grown on demand by a synchronising cudaFree + cudaMalloc.
+ *            kernels (no allocation, no synchronisation: it can be captured into a CUDA graph) AS LONG AS the
+ *            workspace need does not rise afterwards; without the reserve the workspace is grown on demand by a
+ *            synchronising cudaFree + cudaMalloc.  The need rises with a larger batch, a larger
+ *            cos_set_workspace_limit, or a change of COS_TUNE_TILES_PER_CHUNK: call cos_reserve again after any of
+ *            these.  A cos_eval that would have to grow the workspace while `stream` is being captured does not
+ *            allocate: it returns COS_EINVAL, enqueues nothing, and leaves the capture intact.
+ *            Captured graphs hold the workspace address: a later regrowth (any of the causes above) or cos_free
+ *            invalidates every graph captured from this handle -- replaying one then writes to freed memory;
+ *            re-capture after cos_reserve.  cos_eval_host allocates staging buffers and synchronises: never capture it.
  * The current CUDA device must be the one the handle was built on (COS_EINVAL otherwise).
  * Large batches are processed in chunks that fit the workspace budget (cos_set_workspace_limit). */
 int cos_eval(cos_handle h, const double* G_dev, long long batch, double* out_dev, cos_stream stream);
@@ -119,12 +126,14 @@ void cos_free(cos_handle h);
 /* Upper bound (bytes) for the layer-slab workspace of a handle; default 64 GiB. */
 int cos_set_workspace_limit(cos_handle h, long long bytes);
 
-/* Launch tuning of a handle.  These are the ONLY knobs; the library reads no environment variable.  Results do not
+/* Launch tuning of a handle.  These are the ONLY knobs; the library reads no environment variable (the Python binding
+ * does read one, COS_B200_LIB, to pick which build of this library it loads -- nothing else).  Results do not
  * depend on them (same arithmetic, same summation order).  Bad parameter or value: COS_EINVAL. */
 enum {
     COS_TUNE_PREFETCH = 0,           /* L2 look-ahead of the layer kernel, in states (0 = off; default 8) */
-    COS_TUNE_WARPS_PER_CTA = 1,      /* 1..24 (what fits the handle's kernel); default: the CTA size with the most resident
-                                        warps per SM */
+    COS_TUNE_WARPS_PER_CTA = 1,      /* 1..24 (what fits the handle's kernel: at most 16, or 20 for rows of 20 endpoints);
+                                        default: the CTA size with the most resident warps per SM.  The handle's device
+                                        must be current (COS_EINVAL otherwise) */
     COS_TUNE_BLOCKS_PER_CTA_CAP = 2, /* upper bound of occupancy-mask blocks per CTA (0 = default: one per staged table slot) */
     COS_TUNE_PDL = 3,                /* programmatic dependent launch between layers (default 1) */
     COS_TUNE_FUSED = 4,              /* small DAGs: 1 = one fused launch (default), 0 = per-layer kernels */
@@ -151,6 +160,7 @@ enum {
     COS_INFO_WORKSPACE_BYTES = 13,
     COS_INFO_N_LAUNCHES = 14,     /* kernels launched through this handle so far (cos_eval / cos_eval_host) */
     COS_INFO_ORDER_MASK = 15,     /* requested orders of an all-subset handle (0 for single-output handles) */
+    COS_INFO_RESERVED_BATCH = 16, /* largest batch passed to a successful cos_reserve so far (0: none) */
     COS_INFO_DEVICE = 19,         /* CUDA device of the handle (-1: host-only) */
     COS_INFO_FUSED = 20,          /* 1: cos_eval walks the DAG in one fused launch */
     COS_INFO_LAYER_STATES = 100,  /* + layer index */

@@ -23,7 +23,7 @@ TUNE = {"prefetch": 0, "warps_per_cta": 1, "blocks_per_cta_cap": 2, "pdl": 3, "f
 INFO = {
     "n_layers": 0, "n_states": 1, "n_edges": 2, "n_readout_edges": 3, "n_out": 4, "max_layer_states": 5,
     "n_masks": 6, "n_rows": 7, "n_fma": 8, "program_bytes": 9, "d": 10, "n_blocks": 11,
-    "n_states_unpruned": 12, "workspace_bytes": 13, "n_launches": 14, "order_mask": 15,
+    "n_states_unpruned": 12, "workspace_bytes": 13, "n_launches": 14, "order_mask": 15, "reserved_batch": 16,
     "device": 19, "fused": 20,
     "layer_states": 100, "layer_edges": 200, "layer_masks": 300,
 }
@@ -130,6 +130,7 @@ def cos_build_ex(n, n_flavors, lattice, shifts, readout_envelope, flags=0):
     keep, p = _shifts_arg(shifts)
     h = ctypes.c_void_p()
     _check(lib.cos_build_ex(int(n), int(n_flavors), int(lattice), p, int(readout_envelope), int(flags), ctypes.byref(h)))
+    _shape_cache.pop(h.value, None)               # a new handle may reuse the address of one freed outside the binding
     return h.value
 
 
@@ -139,6 +140,7 @@ def cos_build_orders(n, n_flavors, lattice, shifts, order_mask, flags=0):
     keep, p = _shifts_arg(shifts)
     h = ctypes.c_void_p()
     _check(lib.cos_build_orders(int(n), int(n_flavors), int(lattice), p, int(order_mask), int(flags), ctypes.byref(h)))
+    _shape_cache.pop(h.value, None)               # a new handle may reuse the address of one freed outside the binding
     return h.value
 
 
@@ -219,9 +221,10 @@ def _dev_ptr(t, dtype_name, numel=0, what="tensor"):
 def cos_eval(handle, G_dev, batch, out_dev, stream=None):
     """G_dev: torch.float64 CUDA tensor [n_blocks*d*d, batch] (batch contiguous); out_dev: [n_out, batch]."""
     lib = load_library()
-    B, d = int(batch), cos_info(handle, "d")
-    _check(lib.cos_eval(handle, _dev_ptr(G_dev, "torch.float64", cos_info(handle, "n_blocks") * d * d * B, "G_dev"), B,
-                        _dev_ptr(out_dev, "torch.float64", cos_info(handle, "n_out") * B, "out_dev"),
+    B, sh = int(batch), _shape(handle)
+    d = sh["d"]
+    _check(lib.cos_eval(handle, _dev_ptr(G_dev, "torch.float64", sh["n_blocks"] * d * d * B, "G_dev"), B,
+                        _dev_ptr(out_dev, "torch.float64", sh["n_out"] * B, "out_dev"),
                         _stream_ptr(stream)))
 
 
@@ -237,7 +240,21 @@ def cos_set_tuning(handle, what, value):
     _check(load_library().cos_set_tuning(handle, code, int(value)))
 
 
+# constants of a handle that the size checks of cos_eval / cos_eval_host need on every call: fetched once per handle
+# (three cos_info round trips otherwise sit inside the timed step of launch-bound workloads), dropped by cos_free
+_shape_cache = {}
+
+
+def _shape(handle):
+    s = _shape_cache.get(handle)
+    if s is None:
+        s = {k: cos_info(handle, k) for k in ("d", "n_blocks", "n_out", "n_layers")}
+        _shape_cache[handle] = s
+    return s
+
+
 def cos_free(handle):
+    _shape_cache.pop(handle, None)
     load_library().cos_free(handle)
 
 
@@ -286,10 +303,11 @@ def cos_eval_host(handle, tab, sites_host, tau_host, batch, out_host, stream=Non
     """Host-buffer pipeline: sites_host int32 [n,2,batch], tau_host fp64 [n,batch], out_host fp64 [n_out,batch]
     (torch CPU tensors, ideally pinned).  Synchronises the stream before returning."""
     B = int(batch)
-    n = cos_info(handle, "n_layers") // 2
+    sh = _shape(handle)
+    n = sh["n_layers"] // 2
     _check(load_library().cos_eval_host(handle, tab, _host_ptr(sites_host, "torch.int32", n * 2 * B, "sites_host"),
                                         _host_ptr(tau_host, "torch.float64", n * B, "tau_host"), B,
-                                        _host_ptr(out_host, "torch.float64", cos_info(handle, "n_out") * B, "out_host"),
+                                        _host_ptr(out_host, "torch.float64", sh["n_out"] * B, "out_host"),
                                         _stream_ptr(stream)))
 
 

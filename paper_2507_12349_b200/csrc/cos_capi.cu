@@ -40,6 +40,7 @@ struct cos_handle_s {
     double* ws = nullptr;                 // two ping-pong layer slabs
     size_t ws_bytes = 0;
     long long ws_limit = 64ll << 30;
+    long long reserved_batch = 0;         // largest batch passed to cos_reserve (COS_INFO_RESERVED_BATCH)
     // launch shape and tuning (cos_set_tuning); nothing here is read from the environment
     int warps_per_cta = 8, ctas_per_sm = 1, n_sm = 148;
     int prefetch = 8;                     // L2 look-ahead distance in states
@@ -123,7 +124,7 @@ static int build_impl(int n, int n_flavors, int lattice, const double* shifts, i
     const size_t smem = layer_smem_bytes(D.n_blocks * D.d * D.d, D.nc, D.d, D.has_shift);
     if (smem > LAYER_SMEM_MAX) {
         delete h;
-        return fail(COS_EUNSUPPORTED, "cos_build: propagator tile does not fit the 227 KB shared memory of one SM");
+        return fail(COS_EUNSUPPORTED, "cos_build: propagator tile does not fit the 226 KB of shared memory a CTA can use for it (227 KB per SM minus 1 KB of bookkeeping)");
     }
 
     if (!(flags & COS_BUILD_HOST_ONLY)) {
@@ -233,9 +234,21 @@ static long long chunk_tiles(cos_handle h, long long batch, size_t* bytes)
     return tiles_chunk;
 }
 
-static int grow_workspace(cos_handle h, size_t need, const char* who)
+// stream: the stream the caller is about to enqueue on, or nullptr when there is none (cos_reserve).  Growing the
+// workspace is a cudaFree + cudaMalloc: never while that stream is being captured -- it would break the capture, and a
+// graph captured earlier holds the old pointer.
+static int grow_workspace(cos_handle h, size_t need, const char* who, cudaStream_t stream, bool have_stream)
 {
     if (need <= h->ws_bytes) return COS_OK;
+    if (have_stream) {
+        cudaStreamCaptureStatus st = cudaStreamCaptureStatusNone;
+        cudaError_t eq = cudaStreamIsCapturing(stream, &st);
+        if (eq != cudaSuccess) return cuda_fail(eq, who);
+        if (st != cudaStreamCaptureStatusNone)
+            return fail(COS_EINVAL, std::string(who) + ": the workspace would have to grow (" + std::to_string(h->ws_bytes) +
+                        " -> " + std::to_string(need) + " bytes) while the stream is being captured; call cos_reserve for this "
+                        "batch before the capture begins");
+    }
     if (h->ws) { cudaFree(h->ws); h->ws = nullptr; h->ws_bytes = 0; }
     cudaError_t e = cudaMalloc(&h->ws, need);
     if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, who); }
@@ -251,7 +264,9 @@ int cos_reserve(cos_handle h, long long batch)
     if (rc != COS_OK || batch == 0) return rc;
     size_t need = 0;
     chunk_tiles(h, batch, &need);
-    return grow_workspace(h, need, "cos_reserve: workspace allocation");
+    rc = grow_workspace(h, need, "cos_reserve: workspace allocation", nullptr, false);
+    if (rc == COS_OK && batch > h->reserved_batch) h->reserved_batch = batch;
+    return rc;
 }
 
 int cos_set_tuning(cos_handle h, int what, long long value)
@@ -264,6 +279,8 @@ int cos_set_tuning(cos_handle h, int what, long long value)
         case COS_TUNE_WARPS_PER_CTA:
             if (value < 1 || value > 24) return fail(COS_EINVAL, "cos_set_tuning: warps per CTA must be in [1, 24]");
             if (h->on_device) {       // resident CTAs per SM for the new shape (sizes the grid waves)
+                const int rcd = check_device(h, "cos_set_tuning");     // the occupancy query is about the handle's device
+                if (rcd != COS_OK) return rcd;
                 const CompiledDag& D = h->dag;
                 int c = 0;
                 if (layer_ctas_per_sm((int)D.max_L, D.nc, D.d, D.n_blocks * D.d * D.d, D.has_shift, (int)value, &c) != cudaSuccess || c < 1) {
@@ -302,7 +319,7 @@ static int eval_range(cos_handle h, const double* G_dev, long long batch, double
     size_t need = 0;
     const long long tiles_chunk = chunk_tiles(h, batch, &need);
     // (cos_reserve hoists this allocation out of the call; growing here synchronises the device)
-    int rc = grow_workspace(h, need, "cos_eval: workspace allocation");
+    int rc = grow_workspace(h, need, "cos_eval: workspace allocation", stream, true);
     if (rc != COS_OK) return rc;
     double* slab[2] = {h->ws, h->ws + (size_t)D.max_layer_states * TILE * (size_t)tiles_chunk};
 #ifdef COS_CHECK_BOUNDS
@@ -487,14 +504,24 @@ int cos_eval_host(cos_handle h, cos_tab tab, const int* sites_host, const double
     for (long long i = 0; i < n_slices; ++i) {
         const long long t_a = tiles_total * i / n_slices, t_b = tiles_total * (i + 1) / n_slices;
         rc = eval_range(h, h->st_G, batch, h->st_out, t_a, t_b, i == 0, stream);
-        if (rc != COS_OK) return rc;
+        if (rc != COS_OK) {                       // no copy into out_host may still be in flight when the caller sees the error
+            const std::string msg = g_err;
+            cudaStreamSynchronize(h->copy_stream);
+            cudaStreamSynchronize(stream);
+            g_err = msg;
+            return rc;
+        }
         const size_t c0 = (size_t)t_a * TILE, c1 = (size_t)(t_b * TILE < batch ? t_b * TILE : batch);
         e = cudaEventRecord(h->copy_events[i], stream);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(h->copy_stream, h->copy_events[i], 0);
         if (e == cudaSuccess)
             e = cudaMemcpy2DAsync(out_host + c0, B * sizeof(double), h->st_out + c0, B * sizeof(double),
                                   (c1 - c0) * sizeof(double), (size_t)D.n_out, cudaMemcpyDeviceToHost, h->copy_stream);
-        if (e != cudaSuccess) return cuda_fail(e, "cos_eval_host: pipelined device-to-host copy");
+        if (e != cudaSuccess) {
+            cudaStreamSynchronize(h->copy_stream);
+            cudaStreamSynchronize(stream);
+            return cuda_fail(e, "cos_eval_host: pipelined device-to-host copy");
+        }
     }
     e = cudaStreamSynchronize(h->copy_stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(stream);
@@ -530,6 +557,7 @@ int cos_info(cos_handle h, int what, long long* value)
         case COS_INFO_WORKSPACE_BYTES: *value = (long long)h->ws_bytes; break;
         case COS_INFO_N_LAUNCHES: *value = h->n_launches; break;
         case COS_INFO_ORDER_MASK: *value = (long long)D.order_mask; break;
+        case COS_INFO_RESERVED_BATCH: *value = h->reserved_batch; break;
         case COS_INFO_DEVICE: *value = h->device; break;
         case COS_INFO_FUSED: *value = h->fused ? 1 : 0; break;
         default: return fail(COS_EINVAL, "cos_info: unknown query");

@@ -23,7 +23,7 @@ namespace cosb {
 
 static const int MAX_WARPS = 16;
 // CTA size bound per instantiation: the long-row kernels (honeycomb, d = 20) are shared-memory limited to one CTA
-// per SM, so they take 24 warps (<= 85 registers) instead of 16.
+// per SM, so they take 20 warps (<= 96 registers) instead of 16.
 __host__ __device__ constexpr int max_warps_of(int maxl) { return maxl == 20 ? 20 : MAX_WARPS; }
 
 __device__ __forceinline__ double lds64(uint32_t addr)

@@ -201,6 +201,44 @@ def test_reserve_makes_eval_capturable_in_a_cuda_graph(cos):
         cos.cos_free(h)
 
 
+def test_eval_that_must_grow_the_workspace_fails_cleanly_under_capture(cos):
+    """A cos_eval whose batch exceeds what cos_reserve prepared would have to cudaFree + cudaMalloc the workspace; while
+    its stream is being captured it must refuse (COS_EINVAL), enqueue nothing and leave the capture usable
+    (include/cos.h, cos_eval)."""
+    import torch
+    n, nf, B, B_big = 7, 2, 64, 256
+    G = random_matrices(93, 1, n, B_big, scale=0.5, diag=-0.4)
+    Gd = torch.from_numpy(G.reshape(-1, B_big)).cuda()
+    Gs = Gd[:, :B].contiguous()
+    h = cos.cos_build_ex(n, nf, cos.COS_LATTICE_SQUARE, None, 0, flags=cos.COS_BUILD_NO_FUSED)
+    try:
+        cos.cos_reserve(h, B)
+        assert cos.cos_info(h, "reserved_batch") == B
+        ws = cos.cos_info(h, "workspace_bytes")
+        ref = torch.empty((1, B), dtype=torch.float64, device="cuda")
+        cos.cos_eval(h, Gs, B, ref)
+        torch.cuda.synchronize()
+        out = torch.zeros((1, B), dtype=torch.float64, device="cuda")
+        big = torch.full((1, B_big), float("nan"), dtype=torch.float64, device="cuda")
+        launches = cos.cos_info(h, "n_launches")
+        graph = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(graph):
+            with pytest.raises(cos.CosError) as ei:
+                cos.cos_eval(h, Gd, B_big, big)                   # needs 4x the reserved workspace
+            assert ei.value.code == cos.COS_EINVAL and "cos_reserve" in str(ei.value)
+            assert cos.cos_info(h, "n_launches") == launches      # nothing enqueued
+            cos.cos_eval(h, Gs, B, out)                           # the capture goes on
+        assert cos.cos_info(h, "workspace_bytes") == ws
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref) and bool(torch.isnan(big).all())
+        cos.cos_eval(h, Gd, B_big, big)                           # outside a capture the same call grows the workspace
+        torch.cuda.synchronize()
+        assert cos.cos_info(h, "workspace_bytes") > ws and torch.equal(big[:, :B], ref)
+    finally:
+        cos.cos_free(h)
+
+
 @pytest.mark.parametrize("n,nf,sb,all_subsets", [(8, 2, False, True), (7, 3, True, False)])
 def test_per_layer_kernels_chunked_workspace(cos, n, nf, sb, all_subsets):
     """Orders above 6 run the per-layer kernels (cos_layer_kernel).  A 1-byte workspace limit makes cos_eval walk the
