@@ -8,7 +8,8 @@ propagator tabulation (A2) -> layer propagation (A3) -> terminal readouts (A4); 
 happens once, outside the timed region.  `value` = configurations / s with the inputs (vertex sites and
 times) resident in HBM; `e2e` = the same through cos_eval_host with HOST buffers (copies inside the timed
 region).  N > 1 (torchrun): configurations are independent, so every rank runs its own batch (seed + rank),
-no data-path collective ("weak" scaling); value = all ranks' configurations / max-over-ranks time.
+no data-path collective ("weak" scaling, the default); `--scaling strong` cuts ONE global batch into per-rank slices
+(paper_2507_12349_b200.sharding.shard_vertices) instead.  value = all ranks' configurations / max-over-ranks time.
 
 `--impl reference` times the CPU oracle (oracle/) on the host cores on a bounded sample of the same
 workload -- the paper ships no code, so the oracle is the reference arm.
@@ -53,6 +54,9 @@ def parse_args():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, help="cfg1..cfg5 (BASELINE.json configs, 1-based)")
     ap.add_argument("--batch", type=int, default=0, help="override the configuration count (0 = BASELINE's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank its own full batch (default, the driver's run); strong = ONE global batch "
+                         "cut into per-rank slices with sharding.shard_vertices")
     ap.add_argument("--no-other-workloads", action="store_true",
                     help="skip the short timings of the other BASELINE configurations (other_workloads block)")
     ap.add_argument("--layers", action="store_true", help="print the per-layer table to stderr")
@@ -74,11 +78,15 @@ def workload_of(args, rank=0):
     return w.scaled(**kw)
 
 
-def config_dict(w, n_gpus, extra=None):
+def config_dict(w, n_gpus, extra=None, global_batch=None):
+    """global_batch: the one batch that was cut over the ranks (--scaling strong); None = every rank ran w.batch."""
     c = {"workload": w.name, "n": w.n, "n_flavors": w.n_flavors, "lattice": "honeycomb" if w.lattice else "square",
          "mode": "uniform" if w.alphas is None else "sb", "all_subsets": w.all_subsets, "batch_per_gpu": w.batch,
-         "global_batch": w.batch * n_gpus, "L": w.L, "beta": w.beta, "n_tau": w.n_tau, "seed": w.seed,
-         "parallelism": "batch-sharded x%d, no collective" % n_gpus}
+         "global_batch": w.batch * n_gpus if global_batch is None else global_batch,
+         "L": w.L, "beta": w.beta, "n_tau": w.n_tau, "seed": w.seed,
+         "parallelism": ("independent batches x%d (one per rank, seed + 1000 rank), no collective" % n_gpus)
+                        if global_batch is None else
+                        ("one global batch cut into %d contiguous slices (shard_vertices), no collective" % n_gpus)}
     if extra:
         c.update(extra)
     return c
@@ -288,10 +296,23 @@ def run_ours(args):
         dist.init_process_group("nccl", device_id=dev)
     cos.load_library()
 
-    w = workload_of(args, rank)
+    strong = args.scaling == "strong"
+    if strong:
+        # one global batch, the same on every rank (same seed); this rank evaluates its contiguous slice only
+        from paper_2507_12349_b200.sharding import shard_vertices
+        w_global = workload_of(args, 0)
+        global_B = w_global.batch
+        _, _, v = shard_vertices(draw_vertices(w_global), global_B, rank, world)
+        w = w_global.scaled(batch=v["tau"].shape[-1])
+        if w.batch == 0:
+            raise SystemExit("--scaling strong: the global batch has fewer configurations than ranks")
+    else:
+        w = workload_of(args, rank)
+        global_B = None
+        v = draw_vertices(w)
     B = w.batch
+    total_B = global_B if strong else world * B          # configurations all ranks process per step
     table = table_for(w)
-    v = draw_vertices(w)
     tab = cos.cos_tab_build(w.lattice, w.L, table.n_blocks, w.beta, w.n_tau, table.data)
     t0 = time.perf_counter()
     h = cos.cos_build(w.n, w.n_flavors, w.lattice, w.sigmas, w.n if w.all_subsets else 0)
@@ -377,8 +398,8 @@ def run_ours(args):
 
     if rank == 0:
         K = args.steps
-        value = world * B * K / (ms_total * 1e-3)
-        e2e_value = world * B * K / (ms_e2e * 1e-3)
+        value = total_B * K / (ms_total * 1e-3)
+        e2e_value = total_B * K / (ms_e2e * 1e-3)
         edges = info["n_edges"] + info["n_readout_edges"]
         # ---- roofline of the dominant kernel (cos_layer_kernel, NL launches per step); DESIGN.md section 6
         S = info["n_states"]
@@ -415,14 +436,14 @@ def run_ours(args):
                     "fp64_fma_peak_measured_tflops": 2 * fma_peak / 1e12,
                     "fp64_fma_achieved_tflops": 2 * info["n_fma"] * B / layer_s_step / 1e12}
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": max(args.warmup, 3),
-                "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": config_dict(w, world, {"l2": "inputs larger than L2: the two layer slabs hold %.1f GB per step"
+                "config": config_dict(w, world, global_batch=global_B, extra={"l2": "inputs larger than L2: the two layer slabs hold %.1f GB per step"
                                                  % (16 * info["max_layer_states"] * B / 1e9),
                                                  "dag": {k: info[k] for k in ("n_states", "n_edges", "n_readout_edges",
                                                                                "n_fma", "max_layer_states", "program_bytes")},
                                                  "build_s": build_s}),
-                "edge_evals_per_s": world * edges * B * K / (ms_total * 1e-3),
+                "edge_evals_per_s": total_B * edges * K / (ms_total * 1e-3),
                 "e2e": {"value": e2e_value, "unit": UNIT, "ms_per_step": ms_e2e / K,
                         "h2d_bytes_per_step": B * w.n * (2 * 4 + 8), "d2h_bytes_per_step": B * w.n_out * 8},
                 "gpu_launches": int(launches), "clocks": clocks, "roofline": roofline}

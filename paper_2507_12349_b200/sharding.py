@@ -14,6 +14,15 @@ def shard_bounds(batch, rank, world):
     return begin, begin + q + (1 if rank < r else 0)
 
 
+def shard_vertices(vertices, batch, rank, world):
+    """This rank's slice of a global batch of vertex configurations: `vertices` is the dict of batch-innermost arrays
+    (sites [n][2][B], tau [n][B], ...) every rank draws from the same seed; returns (begin, end, dict of contiguous
+    slices [..., begin:end]).  Used by `bench.py --scaling strong` and by the 2-rank gloo test: the same code."""
+    import numpy as np
+    b0, b1 = shard_bounds(batch, rank, world)
+    return b0, b1, {k: np.ascontiguousarray(a[..., b0:b1]) for k, a in vertices.items()}
+
+
 def max_over_ranks(values, device=None):
     """Element-wise MAX over ranks of a list of floats (identity when torch.distributed is not initialised)."""
     import torch

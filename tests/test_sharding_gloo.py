@@ -15,14 +15,17 @@ sys.path.insert(0, %r)
 import numpy as np
 import torch
 import torch.distributed as dist
-from paper_2507_12349_b200.sharding import shard_bounds, max_over_ranks
+from paper_2507_12349_b200.sharding import shard_bounds, shard_vertices, max_over_ranks
 from cos_workloads import get_config, draw_vertices
 dist.init_process_group("gloo")
 rank, world = dist.get_rank(), dist.get_world_size()
 w = get_config(1).scaled(batch=101)
 v = draw_vertices(w)
-b0, b1 = shard_bounds(w.batch, rank, world)
-local = v["tau"][:, b0:b1]
+b0, b1, mine = shard_vertices(v, w.batch, rank, world)      # the slicing `bench.py --scaling strong` does
+assert (b0, b1) == shard_bounds(w.batch, rank, world)
+assert mine["sites"].shape == (w.n, 2, b1 - b0) and mine["sites"].flags["C_CONTIGUOUS"]
+assert np.array_equal(mine["sites"], v["sites"][..., b0:b1])
+local = mine["tau"]
 # every rank reports (bounds, checksum of its slice); gathered only for the TEST, not on the data path
 objs = [None] * world
 dist.all_gather_object(objs, (b0, b1, float(local.sum())))
