@@ -216,6 +216,99 @@ def test_config4_full_64_configurations(cos):
         assert abs(got[0, c] - ref) <= TOL * M, (c, got[0, c], ref, M)
 
 
+def _uniform3_ref(task):
+    A, sg = task
+    return oracle.o3_uniform(A, 3, sg, False)[0], oracle.o3_uniform(A, 3, sg, False, absolute=True)[0]
+
+
+@pytest.mark.parametrize("n", [11, 12])
+def test_sb3_square_orders_11_and_12(cos, n, capsys):
+    """The top of the order range north_star names ("two and three flavors, orders n = 4-12"): SB-CoS with three
+    flavours on the square lattice (Algorithm 3), config-4-shaped tabulated propagators and shifts, at
+    n = 11 (6.3 M states) and n = 12 (21.8 M states), 64 configurations = two batch tiles.
+      (a) oracle parity, both orders: with the three blocks equal and equal shifts the SB value is the uniform one with
+          that shift (Eq. 33) -- the SB program (colours, fan-out, shift closes) against the uniform recurrence O3 of the
+          oracle, bound 1e-10 M;
+      (b) oracle parity, n = 11, non-uniform blocks and shifts: the polynomial route Eq. 34-38 in binary128 (7^11 terms,
+          ~2 core-minutes per configuration) on three configurations, bound 1e-10 M_lower;
+      (c) both orders, every configuration: the determinant route on the device in double-double.  That route loses
+          log10(R / |C|) of its ~32 digits (include/cos.h), so it is a corroboration, not an oracle; the observed
+          agreement (printed) is ~1e-12 relative at n = 11 and ~1e-11 at n = 12 in the median."""
+    import torch
+    w = get_config(4).scaled(n=n, batch=64, seed=300 + n)
+    v = draw_vertices(w)
+    G, got = _run(cos, w, v)
+    assert got.shape == (1, w.batch) and np.all(np.isfinite(got)) and np.all(got != 0.0)
+    Gh = G.reshape(3, n, n, w.batch)
+    # (c) device determinant route, double-double
+    Gd = torch.from_numpy(G).cuda()
+    sub = torch.full(((1 << n) - 1, w.batch), float("nan"), dtype=torch.float64, device="cuda")
+    work = torch.empty((cos.cos_det_workspace_bytes(n, 3, cos.COS_DET_DD, w.batch) + 7) // 8, dtype=torch.float64,
+                       device="cuda")
+    cos.cos_det_eval(n, 3, 3, w.sigmas, cos.COS_DET_DD, Gd, w.batch, sub, work)
+    torch.cuda.synchronize()
+    det_full = sub[-1].cpu().numpy()
+    del sub, work
+    rel = np.abs(det_full - got[0]) / np.abs(got[0])
+    with capsys.disabled():
+        print("\n[sb3 n=%d] DAG vs device det route (dd): median rel %.2e, max rel %.2e" % (n, np.median(rel), rel.max()))
+    assert np.all(np.isfinite(det_full))
+    # observed on a B200: n = 11 median 5.2e-13, max 1.4e-10; n = 12 median 9.3e-12, max 2.1e-8
+    assert np.median(rel) <= (1e-10 if n == 11 else 1e-9) and rel.max() <= (1e-7 if n == 11 else 1e-5), \
+        (np.median(rel), rel.max())
+    # (a) Eq. 33 reduction against the uniform oracle
+    sg = 0.3
+    G1 = np.ascontiguousarray(np.broadcast_to(Gh[:1], Gh.shape)).reshape(-1, w.batch)
+    h = cos.cos_build(n, 3, cos.COS_LATTICE_SQUARE, [sg, sg, sg], 0)
+    try:
+        out = torch.empty((1, w.batch), dtype=torch.float64, device="cuda")
+        cos.cos_eval(h, torch.from_numpy(G1).cuda(), w.batch, out)
+        torch.cuda.synchronize()
+        eq = out.cpu().numpy()[0]
+    finally:
+        cos.cos_free(h)
+    cols = [0, 31, 32, 63]
+    with _pool() as pool:
+        uni = pool.map(_uniform3_ref, [(np.ascontiguousarray(Gh[0, :, :, c]), sg) for c in cols], chunksize=1)
+        if n == 11:
+            cols_b = [1, 33, 62]
+            mats = [np.ascontiguousarray(Gh[..., c]) for c in cols_b]
+            refs = pool.map(_o2b_full, [(A, w.sigmas) for A in mats], chunksize=1)
+            Ms = pool.map(_m_lower_sb, [(A, 3) for A in mats], chunksize=1)
+    for c, (ref, M) in zip(cols, uni):
+        assert abs(eq[c] - ref) <= TOL * M, ("Eq. 33 reduction", n, c, eq[c], ref, M)
+    if n == 11:
+        for c, ref, M in zip(cols_b, refs, Ms):
+            assert abs(got[0, c] - ref) <= TOL * M, ("o2b", c, got[0, c], ref, M)
+
+
+def _honeycomb_uniform_ref(task):
+    Gc, n = task
+    return oracle.connected_reference(Gc, n, 2, 2, None, True, False, tier="o2a")[0]
+
+
+def test_honeycomb_uniform_order_11(cos):
+    """The largest honeycomb DAG the layer program can address (include/cos.h: 92 M states, largest layer 15,990,424 of
+    the 2^24 - 1 a 24-bit destination index allows): uniform CoS with the sublattice sum (Algorithm 2, PAPER.md:517-544;
+    mask refinement PAPER.md:77-84, Eq. 4; sum Eq. 54-55) at n = 11, d = 22 endpoints, config-3-shaped tabulated
+    propagators without shifts, one batch tile.  Three configurations against the sum over the 2^11 sublattice assignments
+    of the two-determinant route O2a (binary128), bound 1e-10 M_lower."""
+    from test_gpu_parity import M_lower_bound
+    n = 11
+    w = get_config(3).scaled(n=n, alphas=None, batch=32, seed=311)
+    v = draw_vertices(w)
+    G, got = _run(cos, w, v)
+    assert got.shape == (1, w.batch) and np.all(np.isfinite(got)) and np.all(got != 0.0)
+    Gh = G.reshape(1, w.d, w.d, w.batch)
+    cols = [0, 17, 31]
+    mats = [np.ascontiguousarray(Gh[..., c]) for c in cols]
+    with _pool() as pool:
+        refs = pool.map(_honeycomb_uniform_ref, [(A, n) for A in mats], chunksize=1)
+    for c, A, ref in zip(cols, mats, refs):
+        M = M_lower_bound(A, n, 2, 2, True, n_assign=8, seed=c)
+        assert abs(got[0, c] - ref) <= TOL * M, (c, got[0, c], ref, M)
+
+
 def _cfg3_ref(task):
     Gc, n, sig = task
     return oracle.connected_reference(Gc, n, 2, 2, sig, False, False, tier="o2a")[0]
