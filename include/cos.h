@@ -68,7 +68,13 @@ enum {
  * flavours; a propagator tile (n_blocks * d * d, + n_colours * d with shifts, entries of 256 bytes) that exceeds the
  * 226 KB of shared memory of one SM (e.g. honeycomb SB-CoS beyond n = 10 with two flavours); a layer of 2^24 - 1 or more
  * states (24-bit destination index of the layer program: honeycomb n >= 11).  COS_ENOMEM is host or device memory
- * exhaustion only.  */
+ * exhaustion only.
+ * What that covers: the square lattice at every order 1..12, uniform or SB with 2-4 flavours (tested on the GPU up to
+ * n = 12 in both modes); honeycomb up to n = 10 in SB mode (two flavours: table 2*20*20 + 2*20 entries = 215 KB) and up
+ * to n = 11 in uniform mode (92 M states, largest layer 15,990,424 < 2^24 - 1; tested on the GPU).  Beyond: SB honeycomb
+ * n = 11 has a layer above 2^24 - 1 states AND a table of 2*22*22*256 B = 242 KB > 226 KB; uniform honeycomb n = 12 has a
+ * layer above 2^24 - 1 states.  Both are limits of the layer program / kernel, not of device memory (a 16 M-state layer
+ * needs 2 * 16 M * 256 B = 8.2 GB of slabs per batch tile, which fits many times).  */
 int cos_build(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope, cos_handle* out);
 int cos_build_ex(int n, int n_flavors, int lattice, const double* shifts, int readout_envelope,
                  int flags, cos_handle* out);
