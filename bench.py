@@ -54,6 +54,8 @@ def parse_args():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD, help="cfg1..cfg5 (BASELINE.json configs, 1-based)")
     ap.add_argument("--batch", type=int, default=0, help="override the configuration count (0 = BASELINE's)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-alg3-baseline", action="store_true",
+                    help="skip cpu_baseline_alg3 (literal Algorithm 3 in fp64 on the host, ~80 s at cfg4)")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank its own full batch (default, the driver's run); strong = ONE global batch "
                          "cut into per-rank slices with sharding.shard_vertices")
@@ -138,6 +140,31 @@ def time_oracle(w, n_sample, procs):
             _oracle_one(t)
     dt = time.perf_counter() - t0
     return n_sample / dt, dt
+
+
+def _alg3_one(task):
+    import oracle
+    G, sigmas = task
+    return oracle.o3_alg3(G, sigmas)
+
+
+def time_alg3(w, procs):
+    """The paper's own recurrence on the host ("the practical CPU evaluator"): literal Algorithm 3
+     in fp64, oracle.o3_alg3 as it stands, ONE configuration of workload `w` per process.
+    Returns (configs/s, seconds)."""
+    import multiprocessing as mp
+    import oracle
+    oracle.build_oracle()
+    ws = w.scaled(batch=procs)
+    table = table_for(ws)
+    v = draw_vertices(ws)
+    G = oracle.tabulate_reference(table, v["sites"], v["tau"])
+    tasks = [(np.ascontiguousarray(G[..., c]), w.sigmas) for c in range(procs)]
+    t0 = time.perf_counter()
+    with mp.get_context("fork").Pool(procs) as pool:
+        pool.map(_alg3_one, tasks, chunksize=1)
+    dt = time.perf_counter() - t0
+    return procs / dt, dt
 
 
 ORACLE_SECONDS_PER_CONFIG = {"cfg1": 2e-4, "cfg2": 0.12, "cfg3": 16.0, "cfg4": 12.0, "cfg5": 16.0}   # rough, one core
@@ -470,6 +497,13 @@ def run_ours(args):
             line["cpu_baseline"] = {"value": rate, "unit": UNIT, "cores": procs, "kind": "oracle", "seconds": dt,
                                     "tier": oracle_tier_name(w),
                                     "sample": "%d configurations of %s, %s" % (n_sample, w.name, oracle_tier_name(w))}
+            # the paper's own algorithm on the host cores as well (square-lattice SB workloads: ~80 s for one configuration
+            # per core at n = 10; the honeycomb workload would need 2^10 times that per configuration and is left out)
+            if w.alphas is not None and w.n_sub == 1 and not w.all_subsets and not args.no_alg3_baseline:
+                rate3, dt3 = time_alg3(workload_of(args), procs)
+                line["cpu_baseline_alg3"] = {"value": rate3, "unit": UNIT, "cores": procs, "kind": "oracle", "seconds": dt3,
+                                             "tier": "O3 literal Algorithm 3 (PAPER.md:546-595), fp64",
+                                             "sample": "%d configurations of %s, one per process" % (procs, w.name)}
         if args.layers:
             sys.stderr.write("layer  states      ms/step   GB/s(alg)\n")
             for l in range(NL):
